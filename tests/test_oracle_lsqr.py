@@ -1,0 +1,202 @@
+"""Pins for the oracle's LSQR (CPU only): dense least squares, normal equations, the Krylov
+minimiser at a fixed iteration count, consistent-system recovery, the block-diagonal special
+case (per-star 5x5 solves), LSQR's own norm estimates, scaling invariances, stop rules 0/3/7
+and scipy.sparse.linalg.lsqr used as a black box."""
+import numpy as np
+import pytest
+import scipy.sparse.linalg as spla
+
+from paper_2212_11675_b200 import inputs
+from tests.helpers import csr_from_raw, make_oracle, small_system
+
+
+def _sys(seed=7, **kw):
+    cfg, star, att, instr, vals = small_system(seed=seed, **kw)
+    o = make_oracle(cfg, star, att, instr, vals)
+    A, _ = csr_from_raw(cfg, star, att, instr, vals)
+    return cfg, o, A
+
+
+def _rhs(A, seed, sigma=1e-3):
+    rng = np.random.default_rng(seed)
+    xt = rng.standard_normal(A.shape[1])
+    return xt, A @ xt + sigma * rng.standard_normal(A.shape[0])
+
+
+def test_matches_dense_lstsq_and_normal_equations():
+    cfg, o, A = _sys()
+    _, b = _rhs(A, 1)
+    r = o.lsqr(b, 500, 1e-14, 1e-14, 1e12)
+    Ad = A.toarray()
+    x_ls = np.linalg.lstsq(Ad, b, rcond=None)[0]
+    x_ne = np.linalg.solve(Ad.T @ Ad, Ad.T @ b)
+    assert r.istop in (1, 2, 4, 5)
+    assert np.linalg.norm(r.x - x_ls) <= 1e-10 * np.linalg.norm(x_ls)
+    assert np.linalg.norm(r.x - x_ne) <= 1e-9 * np.linalg.norm(x_ne)
+
+
+def test_preconditioned_solve_matches_lstsq_after_unscaling():
+    """PC-LSQR: solve on A diag(p), return p (.) z."""
+    cfg, o, A = _sys(seed=9)
+    _, b = _rhs(A, 2)
+    o.precondition()
+    r = o.lsqr(b, 500, 1e-14, 1e-14, 1e12)
+    x_ls = np.linalg.lstsq(A.toarray(), b, rcond=None)[0]
+    assert np.linalg.norm(r.x - x_ls) <= 1e-10 * np.linalg.norm(x_ls)
+
+
+def test_consistent_system_recovers_x_true():
+    cfg, o, A = _sys(seed=3)
+    xt, b = _rhs(A, 3, sigma=0.0)
+    r = o.lsqr(b, 500, 1e-14, 1e-14, 1e12)
+    assert r.istop in (1, 4)
+    assert r.rnorm <= 1e-12 * r.bnorm
+    assert np.linalg.norm(r.x - xt) <= 1e-10 * np.linalg.norm(xt)
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5, 6])
+def test_iterate_k_is_the_krylov_minimiser(k):
+    """In exact arithmetic x_k minimises ||b - A x|| over span{A^T b, (A^T A) A^T b, ...}."""
+    cfg, o, A = _sys(seed=5)
+    _, b = _rhs(A, 4, sigma=0.1)
+    Ad = A.toarray()
+    K = np.empty((Ad.shape[1], k))
+    v = Ad.T @ b
+    for j in range(k):
+        K[:, j] = v / np.linalg.norm(v)
+        v = Ad.T @ (Ad @ K[:, j])
+    Q, _ = np.linalg.qr(K)
+    c = np.linalg.lstsq(Ad @ Q, b, rcond=None)[0]
+    xk = Q @ c
+    r = o.lsqr(b, k, force_itnlim=True)
+    assert r.istop == 7 and r.itn == k
+    assert np.linalg.norm(r.x - xk) <= 1e-8 * np.linalg.norm(xk)
+
+
+def test_finite_termination_small_n():
+    """n = 5*1+3*4+2+1 = 20 columns: LSQR terminates in at most n steps (exact arithmetic)."""
+    cfg, o, A = _sys(seed=6, counts=(60,), n_dfa=4, n_instr=2)
+    _, b = _rhs(A, 5, sigma=0.05)
+    r = o.lsqr(b, 200, 1e-13, 1e-13, 1e12)
+    rank = np.linalg.matrix_rank(A.toarray())
+    assert r.itn <= rank + 2
+    x_ls = np.linalg.lstsq(A.toarray(), b, rcond=None)[0]   # minimum norm
+    assert np.linalg.norm(r.x - x_ls) <= 1e-9 * np.linalg.norm(x_ls)
+
+
+def test_own_estimates_against_direct_norms():
+    cfg, o, A = _sys(seed=8)
+    _, b = _rhs(A, 6, sigma=0.05)
+    fro = np.sqrt((A.toarray() ** 2).sum())
+    prev = None
+    for k in (1, 2, 4, 8, 16, 32):
+        r = o.lsqr(b, k, force_itnlim=True, want_hist=True)
+        res = b - A @ r.x
+        assert abs(r.rnorm - np.linalg.norm(res)) <= 1e-8 * np.linalg.norm(res)
+        assert abs(r.arnorm - np.linalg.norm(A.T @ res)) <= 1e-7 * r.anorm * r.rnorm + 1e-12
+        assert abs(r.xnorm - np.linalg.norm(r.x)) <= 1e-8 * np.linalg.norm(r.x)
+        assert r.anorm <= fro * (1 + 1e-12)
+        h = r.hist
+        assert (np.diff(h[:, 0]) <= 1e-12 * h[0, 0]).all()   # rnorm non-increasing
+        assert (np.diff(h[:, 2]) >= 0).all()                 # anorm non-decreasing
+        assert (np.diff(h[:, 4]) >= -1e-12).all()            # xnorm non-decreasing
+        if prev is not None:
+            assert np.allclose(h[:len(prev)], prev, rtol=1e-12, atol=0)   # deterministic prefix
+        prev = h
+
+
+def test_block_diagonal_special_case_is_per_star_5x5():
+    """With attitude/instrumental/global coefficients zero, A is block diagonal by star."""
+    cfg, star, att, instr, vals = small_system(seed=12, counts=(15, 30, 7, 22))
+    vals = vals.copy(); vals[:, 5:] = 0.0
+    o = make_oracle(cfg, star, att, instr, vals)
+    rng = np.random.default_rng(7)
+    b = rng.standard_normal(o.m)
+    r = o.lsqr(b, 300, 1e-14, 1e-14, 1e12)
+    for s in range(cfg.n_stars):
+        rows = star == s
+        As, bs = vals[rows, :5], b[rows]
+        xs = np.linalg.solve(As.T @ As, As.T @ bs)
+        assert np.linalg.norm(r.x[5 * s:5 * s + 5] - xs) <= 1e-10 * np.linalg.norm(xs)
+    assert np.all(r.x[5 * cfg.n_stars:] == 0.0)    # untouched columns stay exactly zero (A16)
+
+
+def test_scaling_invariance_and_empty_columns():
+    cfg, star, att, instr, vals = small_system(seed=13, counts=(25, 0, 25, 40, 0, 30))
+    o = make_oracle(cfg, star, att, instr, vals)
+    A, _ = csr_from_raw(cfg, star, att, instr, vals)
+    _, b = _rhs(A, 8)
+    r1 = o.lsqr(b, 400, 1e-13, 1e-13, 1e12)
+    r2 = o.lsqr(8.0 * b, 400, 1e-13, 1e-13, 1e12)       # power of two: exact scaling
+    assert r1.itn == r2.itn and r1.istop == r2.istop
+    assert np.array_equal(8.0 * r1.x, r2.x)
+    for s in (1, 4):
+        assert np.all(r1.x[5 * s:5 * s + 5] == 0.0)
+    x_ls = np.linalg.lstsq(A.toarray(), b, rcond=None)[0]
+    assert np.linalg.norm(r1.x - x_ls) <= 1e-9 * np.linalg.norm(x_ls)
+
+
+def test_stop_rules_0_3_7():
+    cfg, o, A = _sys(seed=14)
+    r = o.lsqr(np.zeros(o.m), 10, 1e-8, 1e-8, 1e8)
+    assert (r.istop, r.itn) == (0, 0) and np.all(r.x == 0)
+    # b orthogonal to range(A): A^T b = 0 up to rounding -> solution x = 0
+    Ad = A.toarray()
+    Q, _ = np.linalg.qr(Ad, mode="complete")
+    b = Q[:, -1]
+    r = o.lsqr(b, 10, 1e-8, 1e-8, 1e8)
+    assert r.istop in (0, 2) and np.linalg.norm(r.x) <= 1e-12
+    _, b = _rhs(A, 9)
+    r = o.lsqr(b, 50, 0.0, 0.0, 0.5)              # conlim below 1: rule 3 at iteration 1
+    assert (r.istop, r.itn) == (3, 1)
+    # closed form: after one step anorm^2 = alpha1^2 + beta2^2 = rho1^2 and ||w1|| = 1, so acond = 1
+    assert abs(r.acond - 1.0) <= 1e-14
+    r = o.lsqr(b, 50, 0.0, 0.0, 1.5)              # first iteration with acond >= 1.5
+    assert r.istop == 3 and r.itn >= 2 and r.acond >= 1.5
+    r = o.lsqr(b, 3, 0.0, 0.0, 0.0)
+    assert (r.istop, r.itn) == (7, 3)
+    # forced mode records when a natural rule would have fired
+    rs = o.lsqr(b, 500, 1e-10, 1e-10, 1e8)
+    rf = o.lsqr(b, rs.itn + 5, 1e-10, 1e-10, 1e8, force_itnlim=True)
+    assert rf.istop == 7 and rf.itn == rs.itn + 5
+    assert (rf.istop_natural, rf.itn_natural) == (rs.istop, rs.itn)
+
+
+@pytest.mark.parametrize("precond", [False, True])
+def test_scipy_lsqr_black_box(precond):
+    """Independent implementation of the same published algorithm (black-box use)."""
+    cfg = inputs.scaled(inputs.named_config("cfg1"), 10, "cfg1/10")   # 20k rows, 1361 cols
+    s, a, i, v = inputs.gen_all(cfg)
+    o = make_oracle(cfg, s.numpy(), a.numpy(), i.numpy(), v.numpy())
+    A, _ = csr_from_raw(cfg, s.numpy(), a.numpy(), i.numpy(), v.numpy())
+    xt = inputs.x_true(cfg).numpy()
+    b = A @ xt + inputs.noise(cfg, 0, cfg.n_rows).numpy()
+    if precond:
+        p = o.precondition()
+        A = A @ __import__("scipy.sparse").sparse.diags(p)
+    ref = spla.lsqr(A, b, damp=0.0, atol=1e-10, btol=1e-10, conlim=1e8, iter_lim=500)
+    x_ref, istop, itn, r1norm, _, anorm, acond, arnorm, xnorm = ref[:9]
+    if precond:
+        x_ref = p * x_ref
+    r = o.lsqr(b, 500, 1e-10, 1e-10, 1e8)
+    assert r.istop == istop and abs(r.itn - itn) <= 1
+    assert np.linalg.norm(r.x - x_ref) <= 1e-9 * np.linalg.norm(x_ref)
+    if r.itn == itn:
+        # The Lanczos coefficients alpha_k, beta_k (hence anorm, acond) are not forward stable
+        # once Ritz values converge: two correct implementations drift apart by ~1e-7 while x
+        # and rnorm agree (reading A18).
+        assert abs(r.rnorm - r1norm) <= 1e-8 * r1norm
+        assert abs(r.anorm - anorm) <= 1e-5 * anorm
+        assert abs(r.acond - acond) <= 1e-5 * acond
+        assert abs(r.arnorm - arnorm) <= 1e-6 * arnorm + 1e-12 * anorm * r1norm
+    # fixed-count mode against scipy with an unreachable tolerance
+    # Without column scaling the global column (norm ~141 vs ~10) gives an outlier singular
+    # value; once its Ritz value converges (k ~ 8) orthogonality is lost and two correct
+    # implementations may differ by one "ghost" step until both converge (measured: 1e-2 at
+    # k = 12, back to 1e-9 at k = 16).  Compare before that point (reading A20).
+    k = 12 if precond else 4
+    ref = spla.lsqr(A, b, damp=0.0, atol=0.0, btol=0.0, conlim=0.0, iter_lim=k)
+    xk = p * ref[0] if precond else ref[0]
+    rk = o.lsqr(b, k, force_itnlim=True)
+    assert ref[2] == k and rk.itn == k and rk.istop == 7 and ref[1] == 7
+    assert np.linalg.norm(rk.x - xk) <= 1e-10 * np.linalg.norm(xk)
