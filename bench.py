@@ -1,0 +1,282 @@
+#!/usr/bin/env python
+"""bench.py -- LSQR iterations/s of the Gaia AVU-GSR hot path on B200 (BASELINE.json metric).
+
+A "step" is one PC-LSQR iteration: aprod1, beta, aprod2, alpha, plane rotations, fused vector
+update (all rows of SURVEY/DESIGN section 8(a)) over one synthetic system resident in HBM.
+Default workload: BASELINE.json configs[2] ("cfg3", 3e8 rows, the config the >=70 % HBM
+target is quoted on).  Inputs are seeded and synthetic (paper_2212_11675_b200/inputs.py).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg3] [--impl ours|reference]
+
+N > 1 (torchrun): every rank holds an independent system of the same config (weak scaling,
+no data-path collective).  `--impl reference` times the CPU oracle,
+as it stands, on a bounded sample of the workload (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "lsqr_iterations_per_s"
+UNIT = "it/s"
+BYTES_APROD1, BYTES_APROD2 = 240, 232          # algorithmic HBM bytes per row
+GEN_ROWS = 1 << 23                              # rows generated and appended per chunk
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="cfg3")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--oracle-rows", type=int, default=1 << 20)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop_ev = index, [], threading.Event()
+
+    def run(self):
+        while not self._stop_ev.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True,
+                                     text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([f.strip() for f in out.split(",")])
+            except Exception:
+                pass
+            self._stop_ev.wait(0.2)
+
+    def finish(self):
+        self._stop_ev.set()
+        self.join(timeout=6)
+        sm = sorted(int(r[0]) for r in self.rows if r[0].isdigit())
+        mx = [int(r[1]) for r in self.rows if r[1].isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[2 + i] == "Active" for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(self.rows)}
+
+
+def oracle_sample(cfg, rows, steps):
+    """The oracle, as it stands, on the first `rows` rows of the workload (own b, own p)."""
+    import numpy as np
+    from dataclasses import replace
+    from paper_2212_11675_b200 import inputs
+    from oracle import gsr_oracle
+    rows = min(rows, cfg.n_rows)
+    sptr = inputs.star_ptr(cfg)
+    star, att, instr, vals = inputs.gen_rows(cfg, 0, rows, "cpu", sptr=sptr)
+    n_stars = int(star[-1]) + 1
+    sub = replace(cfg, name=cfg.name + "-sample", n_stars=n_stars, rows_per_star=0,
+                  n_rows_total=rows, counts=None)
+    o = gsr_oracle.OracleSystem(n_stars, cfg.n_dfa, cfg.n_instr, star.numpy(), att.numpy(),
+                                instr.numpy(), vals.numpy())
+    xt = np.random.default_rng(cfg.seed).standard_normal(o.n)
+    b = o.aprod1(xt, 1e-3 * np.random.default_rng(cfg.seed + 1).standard_normal(o.m))
+    o.precondition()
+    t0 = time.perf_counter()
+    r = o.lsqr(b, steps, force_itnlim=True)
+    dt = time.perf_counter() - t0
+    assert r.itn == steps
+    it_s_sample = steps / dt
+    return {"value": it_s_sample * rows / cfg.n_rows, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"first {rows} rows ({n_stars} stars) of {cfg.name}, {steps} oracle LSQR "
+                      f"iterations in {dt:.2f} s = {it_s_sample:.3f} it/s on the sample, scaled "
+                      f"linearly by rows to the full {cfg.n_rows}-row system",
+            "seconds": dt}
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import gsr_oracle
+    gsr_oracle.build()
+    steps = max(1, min(args.steps, 20))
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(cfg, min(args.oracle_rows, 1 << 16), 1)
+    cb = oracle_sample(cfg, args.oracle_rows, steps)
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT,
+            "n_gpus": args.gpus, "steps": steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 / cb["value"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "rows": cfg.n_rows, "cols": cfg.n_cols},
+            "cpu_baseline": cb,
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0,
+                    "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def build_system(cfg, g, inputs, torch, dev):
+    """Chunked ingest (gsr_matrix_begin/append/finalize) of rows generated on the device."""
+    sptr = inputs.star_ptr(cfg)
+    scales = inputs.col_scales(cfg, dev)
+    h = g.gsr_matrix_begin(cfg.n_rows, cfg.n_stars, cfg.n_dfa, cfg.n_instr)
+    for r0 in range(0, cfg.n_rows, GEN_ROWS):
+        nr = min(GEN_ROWS, cfg.n_rows - r0)
+        star, att, instr, vals = inputs.gen_rows(cfg, r0, nr, dev, sptr=sptr, scales=scales)
+        g.gsr_matrix_append_rows(h, r0, nr, star, att, instr, vals)
+        torch.cuda.synchronize()
+        del star, att, instr, vals
+    g.gsr_matrix_finalize(h)
+    return h
+
+
+def main():
+    args = parse()
+    from paper_2212_11675_b200 import inputs
+    cfg0 = inputs.named_config(args.config)
+    if args.impl == "reference":
+        return run_reference(args, cfg0)
+
+    import torch
+    import torch.distributed as dist
+    from dataclasses import replace
+    from paper_2212_11675_b200 import binding as g
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    cfg = replace(cfg0, seed=cfg0.seed + 1000 * rank) if rank else cfg0   # independent systems
+    m, n = cfg.n_rows, cfg.n_cols
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    t_setup = time.perf_counter()
+    h = build_system(cfg, g, inputs, torch, dev)
+    # b = A x_true + noise, formed on the device with the library's own aprod1
+    xt = inputs.x_true(cfg, dev)
+    b = torch.empty(m, dtype=torch.float64, device=dev)
+    for r0 in range(0, m, GEN_ROWS):
+        nr = min(GEN_ROWS, m - r0)
+        b[r0:r0 + nr] = inputs.noise(cfg, r0, nr, dev)
+    g.gsr_aprod1(h, xt, b)
+    g.gsr_precondition(h)
+    g.gsr_set_option(h, g.GSR_OPT_FORCE_ITNLIM, 1)
+    x = torch.empty(n, dtype=torch.float64, device=dev)
+    torch.cuda.synchronize()
+    t_setup = time.perf_counter() - t_setup
+
+    # warm-up (untimed): W iterations (>= 3), also builds the CUDA graph
+    W = max(args.warmup, 3)
+    g.gsr_lsqr_solve(h, b, x, W)
+    # timed: exactly K iterations, device-resident inputs
+    K = args.steps
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    l0 = g.gsr_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    res = g.gsr_lsqr_solve(h, b, x, K)
+    e1.record()
+    barrier()
+    launches = g.gsr_launch_count() - l0
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.finish()
+    assert res.itn == K and res.istop == 7, res
+
+    # end to end through the C ABI with HOST buffers: b H2D (pinned) and x D2H inside the call
+    b_host = torch.empty(m, dtype=torch.float64).pin_memory()
+    b_host.copy_(b)
+    x_host = torch.empty(n, dtype=torch.float64).pin_memory()
+    barrier()
+    t0 = time.perf_counter()
+    res2 = g.gsr_lsqr_solve(h, b_host, x_host, K)
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - t0
+    barrier()
+    assert res2.itn == K
+    assert float((x_host.to(dev) - x).abs().max()) <= 1e-9 * float(x.abs().max())
+    del b_host
+
+    # per-kernel device time of the two products, CUDA events on the launching stream
+    reps = 10
+    ms1 = g.gsr_time_product(h, 1, reps)
+    ms2 = g.gsr_time_product(h, 2, reps)
+
+    t = torch.tensor([ms, t_e2e * 1e3, ms1, ms2], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms, ms_e2e, ms1, ms2 = [float(v) for v in t]
+
+    if rank == 0:
+        peak, peak_src = peaks()
+        gb1, gb2 = BYTES_APROD1 * m / ms1 * 1e-6, BYTES_APROD2 * m / ms2 * 1e-6
+        gb12 = (BYTES_APROD1 + BYTES_APROD2) * m / (ms1 + ms2) * 1e-6
+        dom = ("aprod2", gb2, ms2, BYTES_APROD2) if ms2 >= ms1 else ("aprod1", gb1, ms1, BYTES_APROD1)
+        line = {
+            "metric": METRIC, "value": world * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg0.name, "rows": m, "cols": n, "stars": cfg.n_stars,
+                       "knots_per_axis": cfg.n_dfa, "instr_cols": cfg.n_instr,
+                       "preconditioned": True, "mode": "fixed-count (GSR_OPT_FORCE_ITNLIM)",
+                       "l2": "matrix (%.1f GB) is far larger than L2; no flush needed" % (224e-9 * m)
+                             if 224 * m > 1e9 else "matrix fits in or near L2: L2-assisted numbers",
+                       "parallelism": "replicas" if world > 1 else "single"},
+            "e2e": {"value": world * K / (ms_e2e * 1e-3), "unit": UNIT,
+                    "h2d_bytes_per_step": 8 * m / K, "d2h_bytes_per_step": (8 * n + 80) / K,
+                    "note": "gsr_lsqr_solve with pinned host b and host x; matrix resident"},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "roofline": {"bound": "hbm", "kernel": dom[0], "achieved": dom[1], "peak": peak,
+                         "unit": "GB/s", "frac": dom[1] / peak, "traffic": None,
+                         "peak_source": peak_src, "algorithmic_bytes_per_row": dom[3],
+                         "ms_per_launch": dom[2]},
+            "products": {"aprod1_gbs": gb1, "aprod2_gbs": gb2, "aprod1_ms": ms1, "aprod2_ms": ms2,
+                         "combined_gbs": gb12, "combined_frac_of_measured": gb12 / peak,
+                         "combined_frac_of_8tbs": gb12 / 8000.0,
+                         "iteration_gbs": 472 * m / (ms / K) * 1e-6},
+            "lsqr": {"istop": res.istop, "itn": res.itn, "rnorm": res.rnorm, "anorm": res.anorm,
+                     "acond": res.acond, "xnorm": res.xnorm, "istop_natural": res.istop_natural,
+                     "itn_natural": res.itn_natural},
+            "setup_s": t_setup, "matrix_device_gb": g.gsr_matrix_device_bytes(h) * 1e-9,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            from oracle import gsr_oracle
+            gsr_oracle.build()
+            line["cpu_baseline"] = oracle_sample(cfg0, args.oracle_rows, 10)
+        print(json.dumps(line), flush=True)
+    g.gsr_matrix_destroy(h)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,164 @@
+/*
+ * gsr.h -- C ABI of libgsr_b200: the hot path of the Gaia AVU-GSR solver (arxiv 2212.11675)
+ * on one NVIDIA B200 (sm_100a).  Plain C, no C++/torch types, no exceptions, nothing printed.
+ *
+ * The library solves  min_x || A x - b ||_2  (Eq. 1) with the paper's
+ * column-preconditioned LSQR (PC-LSQR), A given in the paper's compressed
+ * form: per observation row i
+ *     star_idx[i]      the "number of the star"                     (first half of M_i)
+ *     att_start[i]     index of the first attitude element, relative to an axis block
+ *                      (second half of M_i; reading A3)
+ *     instr_col[6i+j]  the six instrumental column positions          (I_c)
+ *     values[24i+k]    A_d: 5 astrometric | 3x4 attitude | 6 instrumental | 1 global
+ * Column of coefficient k of row i  (S stars, D = N_DFA knots per axis, I instrumental):
+ *     k = 0..4    5*star_idx[i] + k
+ *     k = 5..16   5S + ((k-5)/4)*D + att_start[i] + (k-5)%4
+ *     k = 17..22  5S + 3D + instr_col[6i + k-17]
+ *     k = 23      5S + 3D + I
+ * n_cols = 5S + 3D + I + 1.
+ *
+ * Conventions
+ *   - Every function returns 0 (GSR_OK) or a negative gsr_status; gsr_strerror() names it.
+ *   - "hd" pointers may be HOST or DEVICE memory; the library detects which
+ *     (cudaPointerGetAttributes).  Host buffers are staged through device memory owned by the
+ *     handle; pinned host memory is copied asynchronously, pageable memory synchronously.
+ *   - "dev" pointers must be device memory of the current device.
+ *   - stream is a cudaStream_t passed as void* (NULL = legacy default stream).  Work is
+ *     enqueued on it; only the functions documented as synchronising wait for it.
+ *   - The handle owns all device memory it allocates (cudaMalloc) until gsr_matrix_destroy.
+ *     Callers keep ownership of every array they pass and may free it once the call returned.
+ *   - There is no CPU fallback: on a device that is not compute capability 10.x every entry
+ *     point returns GSR_EUNSUPPORTED; without a CUDA device, GSR_ECUDA.
+ */
+#ifndef GSR_H
+#define GSR_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gsr_matrix gsr_matrix; /* opaque, library-owned */
+typedef void* gsr_stream;             /* cudaStream_t */
+
+typedef enum {
+    GSR_OK = 0,
+    GSR_EINVAL = -1,       /* null pointer, bad dims, index out of range, star_idx decreasing */
+    GSR_ENOMEM = -2,       /* cudaMalloc failed */
+    GSR_ECUDA = -3,        /* a CUDA runtime call failed (sticky error is cleared) */
+    GSR_ESTATE = -4,       /* call not legal in the handle's state */
+    GSR_EUNSUPPORTED = -5  /* device is not sm_100 */
+} gsr_status;
+
+typedef struct {
+    int64_t n_rows;  /* m  observations                                   */
+    int64_t n_stars; /* S  -> 5*S astrometric columns  */
+    int64_t n_dfa;   /* D  knots per axis -> 3*D attitude columns; D >= 4 */
+    int64_t n_instr; /* I  instrumental columns, I >= 1                   */
+    int32_t n_glob;  /* must be 1                           */
+} gsr_dims;
+
+typedef struct {
+    int32_t istop;         /* 0..7, Paige-Saunders stop reason (C3)                */
+    int32_t istop_natural; /* first of rules 1-6 that fired (0: none); differs from istop
+                              only with GSR_OPT_FORCE_ITNLIM                                   */
+    int64_t itn;           /* iterations done                                                  */
+    int64_t itn_natural;   /* iteration at which istop_natural fired (0: none)                 */
+    double rnorm;          /* ||b - A x||   estimate                                          */
+    double arnorm;         /* ||A^T (b - A x)|| estimate                                      */
+    double anorm;          /* Frobenius-norm estimate of the iterated matrix                   */
+    double acond;          /* condition estimate                                               */
+    double xnorm;          /* ||z||, norm of the iterate of the system actually iterated       */
+    double bnorm;          /* ||b||                                                            */
+} gsr_lsqr_result;
+
+/* ---- matrix ingest (SURVEY/DESIGN row a0) -------------------- */
+
+/* One-shot build.  Copies and re-lays the four arrays (hd: host or device) into the device
+ * layout, validates them on the device, SYNCHRONISES the stream before returning.
+ * Rows must be grouped by star: star_idx non-decreasing.  att_start in
+ * [0, D-4]; instr_col in [0, I) (duplicates inside a row are legal and add).
+ * Errors: GSR_EINVAL (nothing is leaked, *out = NULL), GSR_ENOMEM, GSR_ECUDA. */
+int gsr_matrix_create(gsr_matrix** out, const gsr_dims* dims,
+                      const int32_t* star_idx_hd,  /* [m]     */
+                      const int32_t* att_start_hd, /* [m]     */
+                      const int32_t* instr_col_hd, /* [m*6]   row-major */
+                      const double* values_hd,     /* [m*24]  row-major, paper's A_d order */
+                      gsr_stream stream);
+
+/* Chunked build for systems whose caller-form arrays do not fit beside the device copy
+ * (config 3: 67 GB): begin, append consecutive row ranges in order, finalize.
+ * append: row0 must equal the number of rows appended so far; arrays cover nrows rows.
+ * finalize synchronises, reports validation errors (GSR_EINVAL) and makes the handle usable. */
+int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* dims, gsr_stream stream);
+int gsr_matrix_append_rows(gsr_matrix* A, int64_t row0, int64_t nrows,
+                           const int32_t* star_idx_hd, const int32_t* att_start_hd,
+                           const int32_t* instr_col_hd, const double* values_hd);
+int gsr_matrix_finalize(gsr_matrix* A);
+
+int gsr_matrix_destroy(gsr_matrix* A); /* NULL is legal */
+int gsr_matrix_dims(const gsr_matrix* A, gsr_dims* out, int64_t* n_cols);
+int64_t gsr_matrix_device_bytes(const gsr_matrix* A); /* device memory owned by the handle */
+
+/* ---- the two products (rows a3, a5-a8; Algorithms 1 and 2) ----------- */
+
+/* aprod mode 1:  y[i] = y[i] + sum_k A[i,k] x[col(i,k)]   ("b[i] = b[i] + sum").
+ * x_dev [n_cols], y_dev [m], device pointers, caller-owned.  Asynchronous on stream. */
+int gsr_aprod1(const gsr_matrix* A, const double* x_dev, double* y_dev, gsr_stream stream);
+
+/* aprod mode 2:  x[col(i,k)] = x[col(i,k)] + A[i,k] y[i].
+ * y_dev [m], x_dev [n_cols].  Asynchronous on stream.  Uses scratch inside the handle: calls
+ * on the same handle must be stream-ordered. */
+int gsr_aprod2(const gsr_matrix* A, const double* y_dev, double* x_dev, gsr_stream stream);
+
+/* ---- preconditioner (row a1; Algorithm 3 line 2) ---------------------- */
+
+/* p_j = 1/||A_j||_2 (1 for an empty column); every stored coefficient is multiplied by
+ * p[col] in place; p is kept in the handle and, if p_out_hd != NULL, copied out ([n_cols],
+ * host or device).  A second call returns GSR_ESTATE.  Asynchronous unless p_out_hd is host. */
+int gsr_precondition(gsr_matrix* A, double* p_out_hd, gsr_stream stream);
+
+/* ---- LSQR (rows a2, a4, a9-a12; Algorithm 3; C3) --------- */
+
+/* Solves min ||A x - b||.  If A was preconditioned the iteration runs on A.diag(p) and the
+ * returned x is p (.) z ("we re-multiply the solution ... by the preconditioning vector",
+ * PAPER.md:67); the norms in *result refer to the system actually iterated.
+ * b_hd [m] and x_hd [n_cols] may each be host or device.  itnlim >= 1.  atol, btol, conlim
+ * as in Paige & Saunders; conlim = 0 disables rule 3.  SYNCHRONISES the stream: when it
+ * returns, x and *result (host) are valid.  The whole iteration runs on the device from a
+ * captured CUDA graph; the host only launches it. */
+int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnlim, double atol,
+                   double btol, double conlim, gsr_lsqr_result* result, gsr_stream stream);
+
+/* Options (per handle). */
+enum {
+    GSR_OPT_FORCE_ITNLIM = 1, /* 1: rules 1-6 are evaluated and recorded in *_natural but only
+                                 the iteration limit stops the loop (fixed-count mode, A9)    */
+    GSR_OPT_DETERMINISTIC = 2 /* 1: aprod2 uses no floating-point atomics (bit-reproducible)  */
+};
+int gsr_set_option(gsr_matrix* A, int key, int64_t value);
+
+const char* gsr_strerror(int code);
+
+/* ---- test / measurement exports -------------------------------------------------------- */
+
+/* The 24 (column, value) pairs of rows [row0, row0+nrows) in CALLER row order, read back from
+ * the device layout (after preconditioning: the scaled values).  Host output arrays.
+ * Synchronous.  Used by the "index construction bit-exact" parity test. */
+int gsr_debug_expand_rows(const gsr_matrix* A, int64_t row0, int64_t nrows, int64_t* cols_host,
+                          double* vals_host);
+
+/* Average device time (ms, CUDA events on `stream`) of `reps` back-to-back launches of the
+ * product kernels as the solver runs them (internal row order, fused coefficients):
+ * which = 1: aprod1 (u <- A v - c u, + norm partials), which = 2: aprod2 (v += A^T u/beta).
+ * Scratch vectors inside the handle are used; results are discarded.  Synchronous. */
+int gsr_time_product(gsr_matrix* A, int which, int reps, float* ms_avg, gsr_stream stream);
+
+/* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */
+int64_t gsr_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GSR_H */

@@ -1,0 +1,481 @@
+// LSQR iteration on the device (rows a2, a4, a9-a12): Paige & Saunders 1982 as cited by the
+// paper (loop skeleton Algorithm 3), written
+// out in DESIGN.md reading C3.  All scalars live in device memory (LsqrState); one iteration
+// is a fixed kernel sequence captured in a CUDA graph (row a11).
+//
+// Deferred normalisation: u is stored unnormalised (u_hat = beta*u); the factor 1/beta is
+// folded into aprod2's input and -alpha/beta into aprod1's update, so the m-sized vector is
+// read and written exactly once per product.
+#include <math.h>
+#include <string.h>
+
+#include "gsr_internal.h"
+
+namespace gsr {
+
+constexpr int NB_N = 592;     // CTAs of the n-sized kernels (4 per SM on 148 SMs)
+constexpr int TB_N = 256;
+
+__device__ __forceinline__ double block_sum_256(double v, double* red) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int w = 0; w < TB_N / 32; ++w) t += red[w];
+    }
+    return t;  // valid in thread 0
+}
+
+// Deterministic second stage: one CTA sums `np` partials in a fixed order.
+__device__ double reduce_partials_1024(const double* __restrict__ part, int64_t np, double* red) {
+    double t = 0.0;
+    for (int64_t i = threadIdx.x; i < np; i += 1024) t += part[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = t;
+    __syncthreads();
+    double r = 0.0;
+    if (threadIdx.x < 32) {
+        r = red[threadIdx.x];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
+    }
+    __syncthreads();
+    return r;  // valid in warp 0
+}
+
+__device__ __forceinline__ double hyp(double a, double b) { return sqrt(a * a + b * b); }
+
+// u_hat = b (pad rows zero), per-CTA partial sums of b^2
+__global__ void __launch_bounds__(TB_N) k_copy_sumsq(const double* __restrict__ src,
+                                                     double* __restrict__ dst, int64_t len,
+                                                     int64_t len_pad, double* __restrict__ part) {
+    __shared__ double red[TB_N / 32];
+    double q = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * TB_N + threadIdx.x; i < len_pad; i += (int64_t)gridDim.x * TB_N) {
+        double t = i < len ? src[i] : 0.0;
+        dst[i] = t;
+        q = fma(t, t, q);
+    }
+    q = block_sum_256(q, red);
+    if (threadIdx.x == 0) part[blockIdx.x] = q;
+}
+
+__global__ void __launch_bounds__(TB_N) k_sumsq(const double* __restrict__ v, int64_t len,
+                                                double* __restrict__ part, const int* __restrict__ stop) {
+    if (*stop) return;
+    __shared__ double red[TB_N / 32];
+    double q = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * TB_N + threadIdx.x; i < len; i += (int64_t)gridDim.x * TB_N) {
+        double t = v[i];
+        q = fma(t, t, q);
+    }
+    q = block_sum_256(q, red);
+    if (threadIdx.x == 0) part[blockIdx.x] = q;
+}
+
+// v <- vscale * v   (v = -beta v before aprod2 adds A^T u)
+__global__ void __launch_bounds__(TB_N) k_prescale(double* __restrict__ v, int64_t len,
+                                                   const LsqrState* __restrict__ st) {
+    if (st->stop) return;
+    const double c = st->vscale;
+    for (int64_t i = (int64_t)blockIdx.x * TB_N + threadIdx.x; i < len; i += (int64_t)gridDim.x * TB_N)
+        v[i] = c * v[i];
+}
+
+// fused n-sized update (row a10): v <- v*inv_alpha ; x += t1 w ; w = v + t2 w ; partials of
+// the NEW w squared (used as ||w||^2 by the next iteration's ddnorm, reading A10).
+// INIT: w = v (first step), x untouched (already zero).
+template <bool INIT>
+__global__ void __launch_bounds__(TB_N) k_update(double* __restrict__ v, double* __restrict__ w,
+                                                 double* __restrict__ x, int64_t len,
+                                                 const LsqrState* __restrict__ st,
+                                                 double* __restrict__ part_w) {
+    if (st->stop) return;
+    __shared__ double red[TB_N / 32];
+    const double ia = st->inv_alpha, t1 = st->t1, t2 = st->t2;
+    double q = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * TB_N + threadIdx.x; i < len; i += (int64_t)gridDim.x * TB_N) {
+        double vn = v[i] * ia;
+        v[i] = vn;
+        double wn;
+        if (INIT) {
+            wn = vn;
+        } else {
+            double wo = w[i];
+            x[i] = fma(t1, wo, x[i]);
+            wn = fma(t2, wo, vn);
+        }
+        w[i] = wn;
+        q = fma(wn, wn, q);
+    }
+    q = block_sum_256(q, red);
+    if (threadIdx.x == 0) part_w[blockIdx.x] = q;
+}
+
+// x_out = p (.) z  ("re-multiply the solution by the preconditioning vector")
+__global__ void k_finalize_x(const double* __restrict__ z, const double* __restrict__ p,
+                             double* __restrict__ out, int64_t len) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < len) out[i] = p ? p[i] * z[i] : z[i];
+}
+
+// ---- scalar kernels (rows a4, a9): one CTA, deterministic second-stage sums, then one
+// thread runs the recurrences of reading C3 ------------------------------------------------
+
+// beta_1 = ||b||
+__global__ void __launch_bounds__(1024) k_scalar_init1(LsqrState* __restrict__ st,
+                                                       const double* __restrict__ part_u, int64_t np) {
+    __shared__ double red[32];
+    double ss = reduce_partials_1024(part_u, np, red);
+    if (threadIdx.x != 0) return;
+    double beta = sqrt(ss);
+    st->beta = beta;
+    st->bnorm = beta;
+    st->rnorm = beta;
+    st->beta_pos = beta > 0.0;
+    if (beta == 0.0) {          // x = 0 is the exact solution
+        st->stop = 1;
+        st->istop = 0;
+        st->inv_beta = 0.0;
+    } else {
+        st->inv_beta = 1.0 / beta;
+    }
+}
+
+// alpha_1 = ||A^T u_1||
+__global__ void __launch_bounds__(1024) k_scalar_init2(LsqrState* __restrict__ st,
+                                                       const double* __restrict__ part_v, int64_t np) {
+    if (st->stop) return;
+    __shared__ double red[32];
+    double ss = reduce_partials_1024(part_v, np, red);
+    if (threadIdx.x != 0) return;
+    double alpha = sqrt(ss);
+    st->alpha = alpha;
+    if (alpha == 0.0) {
+        st->stop = 1;
+        st->istop = 0;
+        st->inv_alpha = 1.0;
+        return;
+    }
+    st->inv_alpha = 1.0 / alpha;
+    st->rhobar = alpha;
+    st->phibar = st->beta;
+    st->arnorm = alpha * st->beta;
+    st->ca = -alpha / st->beta;
+}
+
+// beta_{k+1} = ||A v_k - alpha_k u_k||, anorm update
+__global__ void __launch_bounds__(1024) k_scalar_beta(LsqrState* __restrict__ st,
+                                                      const double* __restrict__ part_u, int64_t np) {
+    if (st->stop) return;
+    __shared__ double red[32];
+    double ss = reduce_partials_1024(part_u, np, red);
+    if (threadIdx.x != 0) return;
+    st->itn += 1;
+    double beta = sqrt(ss);
+    st->beta = beta;
+    if (beta > 0.0) {
+        st->beta_pos = 1;
+        st->anorm = hyp(hyp(st->anorm, st->alpha), beta);   // uses the OLD alpha
+        st->inv_beta = 1.0 / beta;
+        st->vscale = -beta;
+    } else {
+        st->beta_pos = 0;
+        st->inv_beta = 0.0;
+        st->vscale = 1.0;
+    }
+}
+
+// alpha_{k+1}, plane rotations, norms, stopping rules
+__global__ void __launch_bounds__(1024) k_scalar_main(LsqrState* __restrict__ st,
+                                                      const double* __restrict__ part_v,
+                                                      const double* __restrict__ part_w, int64_t np) {
+    if (st->stop) return;
+    __shared__ double red[32];
+    double ssv = reduce_partials_1024(part_v, np, red);
+    double ssw = reduce_partials_1024(part_w, np, red);
+    if (threadIdx.x != 0) return;
+    double alpha = st->alpha;
+    const double beta = st->beta;
+    if (st->beta_pos) {
+        alpha = sqrt(ssv);
+        st->inv_alpha = alpha > 0.0 ? 1.0 / alpha : 1.0;
+    } else {
+        st->inv_alpha = 1.0;
+    }
+    st->alpha = alpha;
+    // plane rotation eliminating beta
+    const double rho = hyp(st->rhobar, beta);
+    const double cs = st->rhobar / rho, sn = beta / rho;
+    const double theta = sn * alpha;
+    st->rhobar = -cs * alpha;
+    const double phi = cs * st->phibar;
+    st->phibar = sn * st->phibar;
+    const double tau = sn * phi;
+    st->t1 = phi / rho;
+    st->t2 = -theta / rho;
+    st->ddnorm = st->ddnorm + ssw / (rho * rho);
+    // second rotation: ||x|| estimate
+    const double delta = st->sn2 * rho;
+    const double gambar = -st->cs2 * rho;
+    const double rhs = phi - delta * st->z;
+    const double zbar = rhs / gambar;
+    const double xnorm = sqrt(st->xxnorm + zbar * zbar);
+    const double gamma = hyp(gambar, theta);
+    st->cs2 = gambar / gamma;
+    st->sn2 = theta / gamma;
+    st->z = rhs / gamma;
+    st->xxnorm = st->xxnorm + st->z * st->z;
+    // norms and stopping tests
+    const double anorm = st->anorm, bnorm = st->bnorm;
+    const double acond = anorm * sqrt(st->ddnorm);
+    const double rnorm = st->phibar;
+    const double arnorm = alpha * fabs(tau);
+    st->acond = acond;
+    st->rnorm = rnorm;
+    st->arnorm = arnorm;
+    st->xnorm = xnorm;
+    const double test1 = rnorm / bnorm;
+    const double test2 = (anorm * rnorm > 0.0) ? arnorm / (anorm * rnorm) : INFINITY;
+    const double test3 = 1.0 / acond;
+    const double t1c = test1 / (1.0 + anorm * xnorm / bnorm);
+    const double rtol = st->btol + st->atol * anorm * xnorm / bnorm;
+    int nat = 0;
+    if (1.0 + test3 <= 1.0) nat = 6;
+    if (1.0 + test2 <= 1.0) nat = 5;
+    if (1.0 + t1c <= 1.0) nat = 4;
+    if (test3 <= st->ctol) nat = 3;
+    if (test2 <= st->atol) nat = 2;
+    if (test1 <= rtol) nat = 1;
+    if (nat != 0 && st->istop_nat == 0) {
+        st->istop_nat = nat;
+        st->itn_nat = st->itn;
+    }
+    int istop = 0;
+    if (st->itn >= st->itnlim) istop = 7;
+    if (!st->force && nat != 0) istop = nat;
+    st->istop = istop;
+    // coefficient of the next aprod1: u_hat <- A v - (alpha/beta) u_hat
+    st->ca = st->beta_pos ? -alpha / beta : 0.0;
+    // The update kernel of THIS iteration must still run; it checks `stop` first, so the
+    // flag is raised by k_raise_stop after it.
+}
+
+__global__ void k_raise_stop(LsqrState* __restrict__ st) {
+    if (st->istop != 0) st->stop = 1;
+}
+
+// ---- host side ----------------------------------------------------------------------------
+
+int ensure_workspace(gsr_matrix* A) {
+    Workspace& W = A->ws;
+    if (W.st) return GSR_OK;
+    const size_t n8 = (size_t)A->n_cols * 8;
+    int64_t npu = A->n_tiles > NB_N ? A->n_tiles : NB_N;
+    GSR_TRY(dev_alloc(A, (void**)&W.u, (size_t)A->m_pad * 8));
+    GSR_TRY(dev_alloc(A, (void**)&W.v, n8));
+    GSR_TRY(dev_alloc(A, (void**)&W.w, n8));
+    GSR_TRY(dev_alloc(A, (void**)&W.x, n8));
+    GSR_TRY(dev_alloc(A, (void**)&W.part_u, (size_t)npu * 8));
+    GSR_TRY(dev_alloc(A, (void**)&W.part_v, NB_N * 8));
+    GSR_TRY(dev_alloc(A, (void**)&W.part_w, NB_N * 8));
+    GSR_TRY(dev_alloc(A, (void**)&W.st, sizeof(LsqrState)));
+    GSR_CUDA_TRY(cudaMemset(W.u, 0, (size_t)A->m_pad * 8));
+    GSR_CUDA_TRY(cudaMemset(W.st, 0, sizeof(LsqrState)));
+    GSR_CUDA_TRY(cudaMallocHost((void**)&W.stop_host, 64));
+    return GSR_OK;
+}
+
+void free_workspace(gsr_matrix* A) {
+    Workspace& W = A->ws;
+    if (W.graph) cudaGraphExecDestroy(W.graph);
+    cudaFree(W.u); cudaFree(W.v); cudaFree(W.w); cudaFree(W.x);
+    cudaFree(W.part_u); cudaFree(W.part_v); cudaFree(W.part_w);
+    cudaFree(W.stage_m); cudaFree(W.stage_n); cudaFree(W.st);
+    if (W.stop_host) cudaFreeHost(W.stop_host);
+    cudaGetLastError();
+    W = Workspace();
+}
+
+constexpr int KERNELS_PER_ITERATION = 8;
+
+// One LSQR iteration as a fixed kernel sequence (row a11).  Every kernel reads its
+// coefficients from LsqrState and returns at once when st->stop is set.
+static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
+    Workspace& W = A->ws;
+    const int64_t n = A->n_cols;
+    // bidiagonalisation, first half: u_hat <- A v - (alpha/beta) u_hat ; partials of u_hat^2
+    GSR_TRY(launch_aprod1(A, W.v, W.u, &W.st->ca, W.part_u, &W.st->stop, s));
+    k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_tiles);
+    // second half: v <- A^T (u_hat/beta) - beta v
+    k_prescale<<<NB_N, TB_N, 0, s>>>(W.v, n, W.st);
+    GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, s));
+    k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop);
+    k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N);
+    k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w);
+    k_raise_stop<<<1, 1, 0, s>>>(W.st);
+    GSR_CUDA_TRY(cudaGetLastError());
+    return GSR_OK;
+}
+
+static int build_graph(gsr_matrix* A, cudaStream_t s) {
+    Workspace& W = A->ws;
+    if (W.graph_valid && W.graph_stream == s) return GSR_OK;
+    if (W.graph) {
+        cudaGraphExecDestroy(W.graph);
+        W.graph = nullptr;
+    }
+    cudaStream_t cs = s;
+    bool own = false;
+    if (s == nullptr || s == cudaStreamLegacy) {   // the legacy stream cannot be captured
+        GSR_CUDA_TRY(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+        own = true;
+    }
+    cudaGraph_t g = nullptr;
+    long long before = g_launches;
+    cudaError_t e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
+    int rc = GSR_OK;
+    if (e == cudaSuccess) {
+        rc = enqueue_iteration(A, cs);
+        e = cudaStreamEndCapture(cs, &g);
+    }
+    g_launches = before;   // capture issues no launches
+    if (own) cudaStreamDestroy(cs);
+    if (e != cudaSuccess || rc != GSR_OK || !g) {
+        cudaGetLastError();
+        if (g) cudaGraphDestroy(g);
+        return rc != GSR_OK ? rc : GSR_ECUDA;
+    }
+    e = cudaGraphInstantiate(&W.graph, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        W.graph = nullptr;
+        return GSR_ECUDA;
+    }
+    W.graph_valid = true;
+    W.graph_stream = s;
+    return GSR_OK;
+}
+
+}  // namespace gsr
+
+using namespace gsr;
+
+extern "C" {
+
+int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnlim, double atol,
+                   double btol, double conlim, gsr_lsqr_result* result, gsr_stream stream) {
+    if (!A || !x_hd || !result || (!b_hd && A->dims.n_rows > 0) || itnlim < 1) return GSR_EINVAL;
+    if (A->state != 1) return GSR_ESTATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    Workspace& W = A->ws;
+    GSR_TRY(ensure_workspace(A));
+    const int64_t m = A->dims.n_rows, n = A->n_cols;
+    memset(result, 0, sizeof(*result));
+
+    // b -> device
+    const double* b_dev = b_hd;
+    if (m > 0 && !is_device_ptr(b_hd)) {
+        if (!W.stage_m) GSR_TRY(dev_alloc(A, (void**)&W.stage_m, (size_t)m * 8));
+        GSR_CUDA_TRY(cudaMemcpyAsync(W.stage_m, b_hd, (size_t)m * 8, cudaMemcpyHostToDevice, s));
+        b_dev = W.stage_m;
+    }
+    // state
+    LsqrState h;
+    memset(&h, 0, sizeof(h));
+    h.cs2 = -1.0;
+    h.atol = atol;
+    h.btol = btol;
+    h.ctol = conlim > 0.0 ? 1.0 / conlim : 0.0;
+    h.itnlim = itnlim;
+    h.force = A->opt_force_itnlim;
+    h.inv_alpha = 1.0;
+    GSR_CUDA_TRY(cudaMemcpyAsync(W.st, &h, sizeof(h), cudaMemcpyHostToDevice, s));
+    GSR_CUDA_TRY(cudaMemsetAsync(W.v, 0, (size_t)n * 8, s));
+    GSR_CUDA_TRY(cudaMemsetAsync(W.x, 0, (size_t)n * 8, s));
+    // initialisation (row a2): u_hat = b, beta_1, v = A^T u, alpha_1, w = v
+    k_copy_sumsq<<<NB_N, TB_N, 0, s>>>(b_dev, W.u, m, A->m_pad, W.part_u);
+    k_scalar_init1<<<1, 1024, 0, s>>>(W.st, W.part_u, NB_N);
+    count_launch(2);
+    GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, s));
+    k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop);
+    k_scalar_init2<<<1, 1024, 0, s>>>(W.st, W.part_v, NB_N);
+    k_update<true><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w);
+    count_launch(3);
+    GSR_CUDA_TRY(cudaGetLastError());
+
+    // the loop: graph launches; the stop flag is polled from pinned memory between batches
+    GSR_TRY(build_graph(A, s));
+    const int64_t batch = A->opt_force_itnlim ? 256 : 32;
+    int64_t launched = 0;
+    while (launched < itnlim) {
+        int64_t nb = itnlim - launched < batch ? itnlim - launched : batch;
+        for (int64_t i = 0; i < nb; ++i) GSR_CUDA_TRY(cudaGraphLaunch(W.graph, s));
+        count_launch(nb * KERNELS_PER_ITERATION);
+        launched += nb;
+        GSR_CUDA_TRY(cudaMemcpyAsync(W.stop_host, &W.st->stop, sizeof(int), cudaMemcpyDeviceToHost, s));
+        GSR_CUDA_TRY(cudaStreamSynchronize(s));
+        if (*W.stop_host) break;
+    }
+    // finalisation (row a12)
+    const bool x_dev = is_device_ptr(x_hd);
+    double* xo = x_hd;
+    if (!x_dev) {
+        if (!W.stage_n) GSR_TRY(dev_alloc(A, (void**)&W.stage_n, (size_t)n * 8));
+        xo = W.stage_n;
+    }
+    k_finalize_x<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(W.x, A->p, xo, n);
+    count_launch();
+    GSR_CUDA_TRY(cudaGetLastError());
+    if (!x_dev) GSR_CUDA_TRY(cudaMemcpyAsync(x_hd, xo, (size_t)n * 8, cudaMemcpyDeviceToHost, s));
+    GSR_CUDA_TRY(cudaMemcpyAsync(&h, W.st, sizeof(h), cudaMemcpyDeviceToHost, s));
+    GSR_CUDA_TRY(cudaStreamSynchronize(s));
+    result->istop = h.istop;
+    result->istop_natural = h.istop_nat;
+    result->itn = h.itn;
+    result->itn_natural = h.itn_nat;
+    result->rnorm = h.rnorm;
+    result->arnorm = h.arnorm;
+    result->anorm = h.anorm;
+    result->acond = h.acond;
+    result->xnorm = h.xnorm;
+    result->bnorm = h.bnorm;
+    if (result->istop_natural == 0 && h.istop != 7) result->istop_natural = h.istop;
+    return GSR_OK;
+}
+
+int gsr_time_product(gsr_matrix* A, int which, int reps, float* ms_avg, gsr_stream stream) {
+    if (!A || !ms_avg || reps < 1 || (which != 1 && which != 2)) return GSR_EINVAL;
+    if (A->state != 1) return GSR_ESTATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    Workspace& W = A->ws;
+    GSR_TRY(ensure_workspace(A));
+    cudaEvent_t e0, e1;
+    GSR_CUDA_TRY(cudaEventCreate(&e0));
+    GSR_CUDA_TRY(cudaEventCreate(&e1));
+    int rc = GSR_OK;
+    for (int pass = 0; pass < 2 && rc == GSR_OK; ++pass) {   // pass 0: warm-up
+        int nrep = pass == 0 ? 1 : reps;
+        cudaEventRecord(e0, s);
+        for (int i = 0; i < nrep && rc == GSR_OK; ++i) {
+            if (which == 1) rc = launch_aprod1(A, W.v, W.u, A->coef_one, W.part_u, nullptr, s);
+            else rc = launch_aprod2(A, W.u, W.v, A->coef_one, nullptr, s);
+        }
+        cudaEventRecord(e1, s);
+        if (cudaEventSynchronize(e1) != cudaSuccess) rc = GSR_ECUDA;
+    }
+    float ms = 0.f;
+    if (rc == GSR_OK && cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess) rc = GSR_ECUDA;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaGetLastError();
+    *ms_avg = ms / reps;
+    return rc;
+}
+
+}  // extern "C"

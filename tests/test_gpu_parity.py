@@ -1,0 +1,236 @@
+"""GPU parity tests: the CUDA path (through the C ABI binding) against the CPU oracle on the
+same seeded inputs.  Bars: index construction bit-exact; aprod
+outputs within 1e-12 of the component-wise scale (reading A13); LSQR x within 1e-9 relative
+2-norm after a fixed iteration count, identical istop."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2212_11675_b200 import inputs
+from tests.helpers import make_oracle
+
+pytestmark = pytest.mark.gpu
+
+APROD_TOL = 1e-12
+X_TOL = 1e-9
+
+
+def _binding():
+    from paper_2212_11675_b200 import binding
+    return binding
+
+
+def _cases():
+    mc = inputs.micro_config
+    return {
+        "cfg1": inputs.named_config("cfg1"),
+        "one_row": mc("one_row", 21, [1], 4, 1),
+        "one_star_many_tiles": mc("one_star", 22, [1000], 9, 7),
+        "single_obs_stars": mc("single_obs", 23, [1] * 300 + [0] * 5 + [2] * 17, 12, 6),
+        "ragged_empty_stars": mc("ragged", 24, [0, 37, 1, 250, 0, 64, 3, 0, 700, 0], 40, 17),
+        "one_instr_col": mc("one_instr", 25, [130, 129, 300], 16, 1),
+        "skew_hot": inputs.GsrConfig("cfg4s", 3, 400, 400, 60, n_rows_total=50_000,
+                                     powerlaw=(10, 10_000, 1.36), att_hot=(0.9, 0.40, 0.45),
+                                     col_scales=True),
+    }
+
+
+CASES = _cases()
+
+
+class Sys:
+    def __init__(self, cfg, edge_att=False):
+        self.cfg = cfg
+        star, att, instr, vals = inputs.gen_all(cfg)
+        if edge_att and cfg.n_rows >= 2:      # attitude start at both ends of the range
+            att[0] = 0
+            att[-1] = cfg.n_dfa - 4
+        self.host = (star, att, instr, vals)
+        self.o = make_oracle(cfg, star.numpy(), att.numpy(), instr.numpy(), vals.numpy())
+        b = _binding()
+        dev = [t.cuda() for t in self.host]
+        self.A = b.GsrMatrix.create(cfg, *dev)
+        self.m, self.n = cfg.n_rows, cfg.n_cols
+
+
+@pytest.fixture(scope="module", params=list(CASES))
+def sysm(request):
+    s = Sys(CASES[request.param], edge_att=True)
+    yield s
+    s.A.close()
+
+
+def test_index_construction_bit_exact(sysm):
+    b = _binding()
+    cols, vals = b.gsr_debug_expand_rows(sysm.A.h, 0, sysm.m)
+    oc, ov = sysm.o.expand_rows()
+    assert np.array_equal(cols, oc)
+    assert np.array_equal(vals, ov)
+    d, n = b.gsr_matrix_dims(sysm.A.h)
+    assert (d.n_rows, n) == (sysm.m, sysm.n)
+
+
+def test_aprod1_parity(sysm):
+    b = _binding()
+    x = inputs.random_vector(sysm.cfg, 1, sysm.n)
+    y0 = inputs.random_vector(sysm.cfg, 2, sysm.m)
+    y_ref, scale = sysm.o.aprod1(x.numpy(), y0.numpy(), want_scale=True)
+    yd = y0.cuda()
+    b.gsr_aprod1(sysm.A.h, x.cuda(), yd)
+    err = np.abs(yd.cpu().numpy() - y_ref)
+    assert np.all(err <= APROD_TOL * scale), float((err / scale).max())
+
+
+def test_aprod2_parity(sysm):
+    b = _binding()
+    y = inputs.random_vector(sysm.cfg, 3, sysm.m)
+    x0 = inputs.random_vector(sysm.cfg, 4, sysm.n)
+    x_ref, scale = sysm.o.aprod2(y.numpy(), x0.numpy(), want_scale=True)
+    xd = x0.cuda()
+    b.gsr_aprod2(sysm.A.h, y.cuda(), xd)
+    err = np.abs(xd.cpu().numpy() - x_ref)
+    assert np.all(err <= APROD_TOL * np.maximum(scale, 1e-300)), float((err / scale).max())
+    # untouched columns (empty stars, unused instrumental columns) keep x0 exactly
+    untouched = scale == np.abs(x0.numpy())
+    assert np.array_equal(xd.cpu().numpy()[untouched], x0.numpy()[untouched])
+
+
+def test_adjoint_identity_on_gpu(sysm):
+    b = _binding()
+    x = inputs.random_vector(sysm.cfg, 5, sysm.n).cuda()
+    y = inputs.random_vector(sysm.cfg, 6, sysm.m).cuda()
+    Ax = torch.zeros(sysm.m, dtype=torch.float64, device="cuda")
+    ATy = torch.zeros(sysm.n, dtype=torch.float64, device="cuda")
+    b.gsr_aprod1(sysm.A.h, x, Ax)
+    b.gsr_aprod2(sysm.A.h, y, ATy)
+    lhs, rhs = float(Ax @ y), float(x @ ATy)
+    assert abs(lhs - rhs) <= 1e-12 * max(float(Ax.norm() * y.norm()), 1e-300)
+
+
+def _rhs(s):
+    xt = inputs.x_true(s.cfg).numpy()
+    return s.o.aprod1(xt, inputs.noise(s.cfg, 0, s.m).numpy())
+
+
+@pytest.mark.parametrize("name", ["cfg1", "ragged_empty_stars", "skew_hot", "one_instr_col"])
+def test_precondition_and_lsqr_parity(name):
+    """Column scaling then fixed-count and standard-mode PC-LSQR."""
+    b = _binding()
+    s = Sys(CASES[name])
+    try:
+        rhs = _rhs(s)                       # b formed with the oracle's aprod1 on the unscaled A
+        p_ref = s.o.precondition()
+        p = torch.empty(s.n, dtype=torch.float64, device="cuda")
+        b.gsr_precondition(s.A.h, p)
+        assert np.allclose(p.cpu().numpy(), p_ref, rtol=1e-13, atol=0)
+        with pytest.raises(b.GsrError) as ei:
+            b.gsr_precondition(s.A.h, p)
+        assert ei.value.code == b.GSR_ESTATE
+        _, vals = b.gsr_debug_expand_rows(s.A.h, 0, s.m)
+        assert np.allclose(vals, s.o.values, rtol=1e-13, atol=0)
+        bd = torch.from_numpy(rhs).cuda()
+        x = torch.empty(s.n, dtype=torch.float64, device="cuda")
+        # fixed-count mode (reading A9): exactly itnlim iterations, istop 7
+        iters = s.cfg.iterations or 60
+        b.gsr_set_option(s.A.h, b.GSR_OPT_FORCE_ITNLIM, 1)
+        for k in (1, 3, iters):
+            r = b.gsr_lsqr_solve(s.A.h, bd, x, k)
+            ro = s.o.lsqr(rhs, k, force_itnlim=True)
+            assert (r.istop, r.itn) == (ro.istop, ro.itn) == (7, k)
+            xg = x.cpu().numpy()
+            assert np.linalg.norm(xg - ro.x) <= X_TOL * np.linalg.norm(ro.x), (name, k)
+            assert abs(r.rnorm - ro.rnorm) <= 1e-9 * ro.rnorm
+            assert abs(r.xnorm - ro.xnorm) <= 1e-9 * ro.xnorm
+            assert abs(r.bnorm - ro.bnorm) <= 1e-12 * ro.bnorm
+            if ro.itn_natural == 0 or k < ro.itn_natural:      # reading A18
+                assert abs(r.anorm - ro.anorm) <= 1e-9 * ro.anorm
+                assert abs(r.acond - ro.acond) <= 1e-9 * ro.acond
+            else:   # past convergence alpha_k, beta_k are rounding noise: anorm loosely, acond not at all
+                assert abs(r.anorm - ro.anorm) <= 1e-2 * ro.anorm
+            if ro.itn_natural:
+                assert abs(r.itn_natural - ro.itn_natural) <= 1 and r.itn_natural > 0
+        # standard mode
+        b.gsr_set_option(s.A.h, b.GSR_OPT_FORCE_ITNLIM, 0)
+        r = b.gsr_lsqr_solve(s.A.h, bd, x, 500, 1e-10, 1e-10, 1e8)
+        ro = s.o.lsqr(rhs, 500, 1e-10, 1e-10, 1e8)
+        assert r.istop == ro.istop and abs(r.itn - ro.itn) <= 1
+        assert np.linalg.norm(x.cpu().numpy() - ro.x) <= X_TOL * np.linalg.norm(ro.x)
+    finally:
+        s.A.close()
+
+
+def test_lsqr_unpreconditioned_host_buffers_and_determinism():
+    """Host b / x buffers go through the same C call; two runs are bit-identical in x when the
+    deterministic option is on."""
+    b = _binding()
+    cfg = inputs.scaled(inputs.named_config("cfg1"), 10, "cfg1/10")
+    s = Sys(cfg)
+    try:
+        rhs = _rhs(s)
+        xh = np.empty(s.n)
+        b.gsr_set_option(s.A.h, b.GSR_OPT_FORCE_ITNLIM, 1)
+        r = b.gsr_lsqr_solve(s.A.h, rhs, xh, 4)           # numpy host arrays
+        ro = s.o.lsqr(rhs, 4, force_itnlim=True)
+        assert r.itn == 4 and np.linalg.norm(xh - ro.x) <= 1e-11 * np.linalg.norm(ro.x)
+        bp = torch.from_numpy(rhs).pin_memory()
+        xp = torch.empty(s.n, dtype=torch.float64).pin_memory()
+        b.gsr_lsqr_solve(s.A.h, bp, xp, 4)                # pinned host tensors
+        assert np.allclose(xp.numpy(), xh, rtol=1e-12, atol=1e-14)
+    finally:
+        s.A.close()
+
+
+def test_stop_rule_zero_and_errors():
+    b = _binding()
+    s = Sys(CASES["ragged_empty_stars"])
+    try:
+        x = torch.full((s.n,), 7.0, dtype=torch.float64, device="cuda")
+        r = b.gsr_lsqr_solve(s.A.h, torch.zeros(s.m, dtype=torch.float64, device="cuda"), x, 10,
+                             1e-8, 1e-8, 1e8)
+        assert (r.istop, r.itn) == (0, 0) and float(x.abs().max()) == 0.0
+        with pytest.raises(b.GsrError) as ei:
+            b.gsr_lsqr_solve(s.A.h, x, x, 0)
+        assert ei.value.code == b.GSR_EINVAL
+    finally:
+        s.A.close()
+    cfg = CASES["ragged_empty_stars"]
+    star, att, instr, vals = inputs.gen_all(cfg)
+    for mutate, what in ((lambda: star.__setitem__(5, 0), "star decreasing"),
+                         (lambda: att.__setitem__(3, cfg.n_dfa - 3), "att out of range"),
+                         (lambda: instr.__setitem__((4, 2), cfg.n_instr), "instr out of range"),
+                         (lambda: star.__setitem__(-1, cfg.n_stars), "star out of range")):
+        st, at, ic = star.clone(), att.clone(), instr.clone()
+        star_, att_, instr_ = star, att, instr
+        mutate()
+        with pytest.raises(b.GsrError) as ei:
+            b.GsrMatrix.create(cfg, star.cuda(), att.cuda(), instr.cuda(), vals.cuda())
+        assert ei.value.code == b.GSR_EINVAL, what
+        star.copy_(st); att.copy_(at); instr.copy_(ic)
+    with pytest.raises(b.GsrError):
+        b.gsr_matrix_begin(10, 1, 3, 1)          # D < 4
+
+
+def test_host_arrays_and_chunked_builder_equal_one_shot():
+    b = _binding()
+    cfg = CASES["ragged_empty_stars"]
+    star, att, instr, vals = inputs.gen_all(cfg)
+    A1 = b.GsrMatrix.create(cfg, star.cuda(), att.cuda(), instr.cuda(), vals.cuda())
+    A2 = b.GsrMatrix.create(cfg, star.numpy(), att.numpy(), instr.numpy(), vals.numpy())
+    h = b.gsr_matrix_begin(cfg.n_rows, cfg.n_stars, cfg.n_dfa, cfg.n_instr)
+    cuts = [0, 1, 300, 301, 777, cfg.n_rows]
+    for r0, r1 in zip(cuts[:-1], cuts[1:]):
+        b.gsr_matrix_append_rows(h, r0, r1 - r0, star[r0:r1].cuda(), att[r0:r1].cuda(),
+                                 instr[r0:r1].contiguous().cuda(), vals[r0:r1].contiguous().cuda())
+    b.gsr_matrix_finalize(h)
+    A3 = b.GsrMatrix(h)
+    x = inputs.random_vector(cfg, 1, cfg.n_cols).cuda()
+    outs = []
+    for A in (A1, A2, A3):
+        c, v = b.gsr_debug_expand_rows(A.h, 0, cfg.n_rows)
+        y = torch.zeros(cfg.n_rows, dtype=torch.float64, device="cuda")
+        b.gsr_aprod1(A.h, x, y)
+        outs.append((c, v, y.cpu().numpy()))
+        A.close()
+    for c, v, y in outs[1:]:
+        assert np.array_equal(c, outs[0][0]) and np.array_equal(v, outs[0][1])
+        assert np.array_equal(y, outs[0][2])
