@@ -39,7 +39,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="cfg3")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--oracle-rows", type=int, default=1 << 20)
+    ap.add_argument("--oracle-rows", type=int, default=1 << 21)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -202,9 +202,12 @@ def main():
     barrier()
     l0 = g.gsr_launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.profiler.start()      # cudaProfilerStart: ncu --profile-from-start off sees only this
     e0.record()
     res = g.gsr_lsqr_solve(h, b, x, K)
     e1.record()
+    torch.cuda.synchronize()
+    torch.cuda.profiler.stop()
     barrier()
     launches = g.gsr_launch_count() - l0
     ms = e0.elapsed_time(e1)
@@ -271,7 +274,7 @@ def main():
         if world == 1 and not args.no_cpu_baseline:
             from oracle import gsr_oracle
             gsr_oracle.build()
-            line["cpu_baseline"] = oracle_sample(cfg0, args.oracle_rows, 10)
+            line["cpu_baseline"] = oracle_sample(cfg0, args.oracle_rows, 12)
         print(json.dumps(line), flush=True)
     g.gsr_matrix_destroy(h)
     if world > 1:

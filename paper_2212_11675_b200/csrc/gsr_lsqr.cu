@@ -49,14 +49,16 @@ __device__ double reduce_partials_1024(const double* __restrict__ part, int64_t 
 
 __device__ __forceinline__ double hyp(double a, double b) { return sqrt(a * a + b * b); }
 
-// u_hat = b (pad rows zero), per-CTA partial sums of b^2
-__global__ void __launch_bounds__(TB_N) k_copy_sumsq(const double* __restrict__ src,
-                                                     double* __restrict__ dst, int64_t len,
-                                                     int64_t len_pad, double* __restrict__ part) {
+// u_hat = b gathered into the internal row order (padding rows zero), partial sums of b^2
+__global__ void __launch_bounds__(TB_N) k_gather_sumsq(const double* __restrict__ src,
+                                                       const uint32_t* __restrict__ perm,
+                                                       double* __restrict__ dst, int64_t len_int,
+                                                       double* __restrict__ part) {
     __shared__ double red[TB_N / 32];
     double q = 0.0;
-    for (int64_t i = (int64_t)blockIdx.x * TB_N + threadIdx.x; i < len_pad; i += (int64_t)gridDim.x * TB_N) {
-        double t = i < len ? src[i] : 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * TB_N + threadIdx.x; i < len_int; i += (int64_t)gridDim.x * TB_N) {
+        const uint32_t pe = perm[i];
+        double t = pe != PERM_PAD ? src[pe] : 0.0;
         dst[i] = t;
         q = fma(t, t, q);
     }
@@ -275,8 +277,8 @@ int ensure_workspace(gsr_matrix* A) {
     Workspace& W = A->ws;
     if (W.st) return GSR_OK;
     const size_t n8 = (size_t)A->n_cols * 8;
-    int64_t npu = A->n_tiles > NB_N ? A->n_tiles : NB_N;
-    GSR_TRY(dev_alloc(A, (void**)&W.u, (size_t)A->m_pad * 8));
+    int64_t npu = A->n_jobs > NB_N ? A->n_jobs : NB_N;
+    GSR_TRY(dev_alloc(A, (void**)&W.u, (size_t)A->m_int * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.v, n8));
     GSR_TRY(dev_alloc(A, (void**)&W.w, n8));
     GSR_TRY(dev_alloc(A, (void**)&W.x, n8));
@@ -284,7 +286,7 @@ int ensure_workspace(gsr_matrix* A) {
     GSR_TRY(dev_alloc(A, (void**)&W.part_v, NB_N * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.part_w, NB_N * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.st, sizeof(LsqrState)));
-    GSR_CUDA_TRY(cudaMemset(W.u, 0, (size_t)A->m_pad * 8));
+    GSR_CUDA_TRY(cudaMemset(W.u, 0, (size_t)A->m_int * 8));
     GSR_CUDA_TRY(cudaMemset(W.st, 0, sizeof(LsqrState)));
     GSR_CUDA_TRY(cudaMallocHost((void**)&W.stop_host, 64));
     return GSR_OK;
@@ -309,11 +311,11 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
     Workspace& W = A->ws;
     const int64_t n = A->n_cols;
     // bidiagonalisation, first half: u_hat <- A v - (alpha/beta) u_hat ; partials of u_hat^2
-    GSR_TRY(launch_aprod1(A, W.v, W.u, &W.st->ca, W.part_u, &W.st->stop, s));
-    k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_tiles);
+    GSR_TRY(launch_aprod1(A, W.v, W.u, &W.st->ca, W.part_u, &W.st->stop, nullptr, s));
+    k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_jobs);
     // second half: v <- A^T (u_hat/beta) - beta v
     k_prescale<<<NB_N, TB_N, 0, s>>>(W.v, n, W.st);
-    GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, s));
+    GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s));
     k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop);
     k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N);
     k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w);
@@ -399,10 +401,10 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     GSR_CUDA_TRY(cudaMemsetAsync(W.v, 0, (size_t)n * 8, s));
     GSR_CUDA_TRY(cudaMemsetAsync(W.x, 0, (size_t)n * 8, s));
     // initialisation (row a2): u_hat = b, beta_1, v = A^T u, alpha_1, w = v
-    k_copy_sumsq<<<NB_N, TB_N, 0, s>>>(b_dev, W.u, m, A->m_pad, W.part_u);
+    k_gather_sumsq<<<NB_N, TB_N, 0, s>>>(b_dev, A->perm, W.u, A->m_int, W.part_u);
     k_scalar_init1<<<1, 1024, 0, s>>>(W.st, W.part_u, NB_N);
     count_launch(2);
-    GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, s));
+    GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s));
     k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop);
     k_scalar_init2<<<1, 1024, 0, s>>>(W.st, W.part_v, NB_N);
     k_update<true><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w);
@@ -463,8 +465,8 @@ int gsr_time_product(gsr_matrix* A, int which, int reps, float* ms_avg, gsr_stre
         int nrep = pass == 0 ? 1 : reps;
         cudaEventRecord(e0, s);
         for (int i = 0; i < nrep && rc == GSR_OK; ++i) {
-            if (which == 1) rc = launch_aprod1(A, W.v, W.u, A->coef_one, W.part_u, nullptr, s);
-            else rc = launch_aprod2(A, W.u, W.v, A->coef_one, nullptr, s);
+            if (which == 1) rc = launch_aprod1(A, W.v, W.u, A->coef_one, W.part_u, nullptr, nullptr, s);
+            else rc = launch_aprod2(A, W.u, W.v, A->coef_one, nullptr, nullptr, s);
         }
         cudaEventRecord(e1, s);
         if (cudaEventSynchronize(e1) != cudaSuccess) rc = GSR_ECUDA;

@@ -20,15 +20,6 @@ bool is_device_ptr(const void* p) {
     return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
 }
 
-bool is_pinned_host_ptr(const void* p) {
-    cudaPointerAttributes a;
-    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
-        cudaGetLastError();
-        return false;
-    }
-    return a.type == cudaMemoryTypeHost;
-}
-
 int dev_alloc(gsr_matrix* A, void** p, size_t bytes) {
     *p = nullptr;
     if (bytes == 0) bytes = 8;
@@ -42,51 +33,165 @@ int dev_alloc(gsr_matrix* A, void** p, size_t bytes) {
     return GSR_OK;
 }
 
-// AoS caller form -> tile records.  One thread per row.  Validation sets bits in *err:
-// 1 star out of range, 2 star decreasing, 4 att_start out of range, 8 instr_col out of range.
-__global__ void k_layout_rows(unsigned char* __restrict__ tiles, int64_t row0, int64_t nrows,
-                              const int32_t* __restrict__ star, const int32_t* __restrict__ att,
-                              const int32_t* __restrict__ instr, const double* __restrict__ vals,
-                              int64_t S, int64_t D, int64_t I, int* __restrict__ err) {
-    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (r >= nrows) return;
-    int64_t row = row0 + r;
-    unsigned char* T = tiles + (row / R) * (int64_t)TILE_BYTES;
-    int lr = (int)(row % R);
-    int e = 0;
-    int32_t s = star[r], a = att[r];
-    if (s < 0 || s >= S) e |= 1;
-    int32_t sprev;
-    if (r > 0) sprev = star[r - 1];
-    else if (row > 0) {
-        const unsigned char* Tp = tiles + ((row - 1) / R) * (int64_t)TILE_BYTES;
-        sprev = ((const int32_t*)(Tp + OFF_STAR))[(row - 1) % R];
-    } else sprev = 0;
-    if (s < sprev) e |= 2;
-    if (a < 0 || a > D - 4) e |= 4;
-    ((int32_t*)(T + OFF_STAR))[lr] = s;
-    ((int32_t*)(T + OFF_ATT))[lr] = a;
-#pragma unroll
-    for (int j = 0; j < 6; ++j) {
-        int32_t c = instr[6 * r + j];
-        if (c < 0 || c >= I) e |= 8;
-        ((int32_t*)(T + OFF_INSTR + j * R * 4))[lr] = c;
-    }
-#pragma unroll
-    for (int k = 0; k < NPAR; ++k) ((double*)(T + k * R * 8))[lr] = vals[NPAR * r + k];
-    if (e) atomicOr(err, e);
+void dev_free(gsr_matrix* A, void* p, size_t bytes) {
+    if (!p) return;
+    cudaFree(p);
+    A->device_bytes -= (int64_t)(bytes == 0 ? 8 : bytes);
 }
 
-__global__ void k_expand_rows(const unsigned char* __restrict__ tiles, int64_t row0, int64_t nrows,
-                              int64_t S, int64_t D, int64_t I, int64_t* __restrict__ cols,
-                              double* __restrict__ vals) {
-    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (r >= nrows) return;
-    int64_t row = row0 + r;
-    const unsigned char* T = tiles + (row / R) * (int64_t)TILE_BYTES;
-    int lr = (int)(row % R);
-    int64_t s = ((const int32_t*)(T + OFF_STAR))[lr];
-    int64_t a = ((const int32_t*)(T + OFF_ATT))[lr];
+// ---- segment partition: stable counting sort of the staged rows by attitude bin ----------
+// Pass 1: per block of 256 staged rows, rows per bin -> counts[bin * nblk + blk]; validation.
+// Error bits: 1 star out of range, 2 star decreasing, 4 att_start out of range, 8 instr_col.
+__global__ void __launch_bounds__(256) k_seg_count(const int32_t* __restrict__ star,
+                                                   const int32_t* __restrict__ att,
+                                                   const int32_t* __restrict__ instr, int64_t ns,
+                                                   int64_t S, int64_t D, int64_t I, int bin_width,
+                                                   int nbins, int nblk, int* __restrict__ counts,
+                                                   const int* __restrict__ last_star,
+                                                   int* __restrict__ err) {
+    __shared__ int hist[NBIN_MAX];
+    for (int b = threadIdx.x; b < nbins; b += 256) hist[b] = 0;
+    __syncthreads();
+    const int64_t r = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (r < ns) {
+        int e = 0;
+        const int32_t s = star[r], a = att[r];
+        if (s < 0 || s >= S) e |= 1;
+        const int32_t sprev = r > 0 ? star[r - 1] : *last_star;
+        if (s < sprev) e |= 2;
+        int bin = 0;
+        if (a < 0 || a > D - 4) e |= 4;
+        else bin = a / bin_width;
+#pragma unroll
+        for (int j = 0; j < 6; ++j) {
+            const int32_t c = instr[6 * r + j];
+            if (c < 0 || c >= I) e |= 8;
+        }
+        if (e) atomicOr(err, e);
+        atomicAdd(&hist[bin], 1);
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < nbins; b += 256) counts[(int64_t)b * nblk + blockIdx.x] = hist[b];
+}
+
+// Pass 2 (one CTA): exclusive scan of counts in (bin, block) order; every bin starts on a tile
+// boundary.  counts[] becomes the destination offset (rows from the segment's first tile);
+// bin_info[b] = rows in bin b, bin_info[nbins + b] = padded start row of bin b,
+// bin_info[2*nbins] = padded rows of the whole segment.
+__global__ void __launch_bounds__(1024) k_seg_scan(int* __restrict__ counts, int nbins, int nblk,
+                                                   int* __restrict__ bin_info) {
+    __shared__ int part[1024];
+    __shared__ int base_s;
+    int base = 0;
+    for (int b = 0; b < nbins; ++b) {
+        int* c = counts + (int64_t)b * nblk;
+        const int per = (nblk + 1023) / 1024;
+        const int i0 = threadIdx.x * per, i1 = min(i0 + per, nblk);
+        int s = 0;
+        for (int i = i0; i < i1; ++i) s += c[i];
+        part[threadIdx.x] = s;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int run = 0;
+            for (int t = 0; t < 1024; ++t) {
+                int v = part[t];
+                part[t] = run;
+                run += v;
+            }
+            bin_info[b] = run;
+            bin_info[nbins + b] = base;
+            base_s = base + ((run + R - 1) / R) * R;
+        }
+        __syncthreads();
+        int off = base + part[threadIdx.x];
+        for (int i = i0; i < i1; ++i) {
+            int v = c[i];
+            c[i] = off;
+            off += v;
+        }
+        base = base_s;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) bin_info[2 * nbins] = base;
+}
+
+// Pass 3: stable scatter of the staged rows into tile records (internal order) + perm.
+__global__ void __launch_bounds__(256) k_seg_scatter(
+    unsigned char* __restrict__ tiles, uint32_t* __restrict__ perm, int64_t row_base_int,
+    int64_t row_base_ext, const int32_t* __restrict__ star, const int32_t* __restrict__ att,
+    const int32_t* __restrict__ instr, const double* __restrict__ vals, int64_t ns, int64_t D,
+    int bin_width, int nbins, int nblk, const int* __restrict__ offs) {
+    __shared__ int wcnt[8][NBIN_MAX + 1];
+    for (int i = threadIdx.x; i < 8 * (NBIN_MAX + 1); i += 256) (&wcnt[0][0])[i] = 0;
+    __syncthreads();
+    const int64_t r = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int bin = NBIN_MAX;   // inactive lanes share an extra bucket
+    int32_t a = 0;
+    if (r < ns) {
+        a = att[r];
+        bin = (a >= 0 && a <= D - 4) ? a / bin_width : 0;
+    }
+    const unsigned peers = __match_any_sync(0xffffffffu, bin);
+    const int rank_w = __popc(peers & ((1u << lane) - 1u));
+    if (rank_w == 0) wcnt[warp][bin] = __popc(peers);
+    __syncthreads();
+    if (r >= ns) return;
+    int rank = rank_w;
+    for (int w = 0; w < warp; ++w) rank += wcnt[w][bin];
+    const int64_t dst = row_base_int + offs[(int64_t)bin * nblk + blockIdx.x] + rank;
+    unsigned char* T = tiles + (dst / R) * (int64_t)TILE_BYTES;
+    const int lr = (int)(dst % R);
+    perm[dst] = (uint32_t)(row_base_ext + r);
+    ((int32_t*)(T + OFF_STAR))[lr] = star[r];
+    ((int32_t*)(T + OFF_ATT))[lr] = a;
+#pragma unroll
+    for (int j = 0; j < 6; ++j) ((int32_t*)(T + OFF_INSTR + j * R * 4))[lr] = instr[6 * r + j];
+#pragma unroll
+    for (int k = 0; k < NPAR; ++k) ((double*)(T + k * R * 8))[lr] = vals[NPAR * r + k];
+}
+
+__global__ void k_save_last_star(const int32_t* __restrict__ star, int64_t ns, int* last_star) {
+    if (ns > 0) *last_star = star[ns - 1];
+}
+
+// Padding rows (they round every bin up to whole tiles and trail the bin's real rows): zero
+// coefficients (tiles are memset to 0); att = the window's first knot and star = the star of
+// the last real row of the tile, so that they open no new window and no new star segment.
+__global__ void __launch_bounds__(R) k_fix_padding(unsigned char* __restrict__ tiles,
+                                                   const uint32_t* __restrict__ perm,
+                                                   const Job* __restrict__ jobs, int n_jobs) {
+    const int j = blockIdx.x;
+    if (j >= n_jobs) return;
+    const Job job = jobs[j];
+    for (int t = 0; t < job.ntiles; ++t) {
+        unsigned char* T = tiles + (int64_t)(job.tile0 + t) * TILE_BYTES;
+        const int64_t row = (int64_t)(job.tile0 + t) * R + threadIdx.x;
+        const bool real = perm[row] != PERM_PAD;
+        const int nreal = __syncthreads_count(real);
+        if (!real) {
+            ((int32_t*)(T + OFF_ATT))[threadIdx.x] = job.a0;
+            ((int32_t*)(T + OFF_STAR))[threadIdx.x] = nreal > 0 ? ((const int32_t*)(T + OFF_STAR))[nreal - 1] : 0;
+        }
+        __syncthreads();
+    }
+}
+
+// Caller-order dump of rows [row0, row0+nrows): every internal row whose caller row falls in
+// the range writes its 24 (column, value) pairs.
+__global__ void k_expand_rows(const unsigned char* __restrict__ tiles, const uint32_t* __restrict__ perm,
+                              int64_t m_int, int64_t row0, int64_t nrows, int64_t S, int64_t D,
+                              int64_t I, int64_t* __restrict__ cols, double* __restrict__ vals) {
+    const int64_t ri = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (ri >= m_int) return;
+    const uint32_t pe = perm[ri];
+    if (pe == PERM_PAD) return;
+    const int64_t r = (int64_t)pe - row0;
+    if (r < 0 || r >= nrows) return;
+    const unsigned char* T = tiles + (ri / R) * (int64_t)TILE_BYTES;
+    const int lr = (int)(ri % R);
+    const int64_t s = ((const int32_t*)(T + OFF_STAR))[lr];
+    const int64_t a = ((const int32_t*)(T + OFF_ATT))[lr];
     const int64_t off_att = 5 * S, off_instr = off_att + 3 * D, off_glob = off_instr + I;
     for (int k = 0; k < NPAR; ++k) {
         int64_t c;
@@ -136,6 +241,63 @@ __global__ void __launch_bounds__(R) k_scale_values(unsigned char* __restrict__ 
 
 using namespace gsr;
 
+static int flush_segment(gsr_matrix* A) {
+    const int64_t ns = A->seg_fill;
+    if (ns == 0) return GSR_OK;
+    const int nblk = (int)((ns + 255) / 256);
+    cudaStream_t s = A->stream;
+    k_seg_count<<<nblk, 256, 0, s>>>(A->st_star, A->st_att, A->st_instr, ns, A->dims.n_stars,
+                                     A->dims.n_dfa, A->dims.n_instr, A->bin_width, A->nbins, nblk,
+                                     A->seg_counts, A->last_star, A->err);
+    k_seg_scan<<<1, 1024, 0, s>>>(A->seg_counts, A->nbins, nblk, A->seg_bin_rows);
+    k_seg_scatter<<<nblk, 256, 0, s>>>(A->tiles, A->perm, A->n_tiles * R, A->rows_appended - ns,
+                                       A->st_star, A->st_att, A->st_instr, A->st_vals, ns,
+                                       A->dims.n_dfa, A->bin_width, A->nbins, nblk, A->seg_counts);
+    k_save_last_star<<<1, 1, 0, s>>>(A->st_star, ns, A->last_star);
+    count_launch(4);
+    GSR_CUDA_TRY(cudaGetLastError());
+    std::vector<int> info(2 * A->nbins + 1);
+    GSR_CUDA_TRY(cudaMemcpyAsync(info.data(), A->seg_bin_rows, info.size() * sizeof(int),
+                                 cudaMemcpyDeviceToHost, s));
+    GSR_CUDA_TRY(cudaStreamSynchronize(s));
+    // job table: runs of at most job_tiles tiles inside one (segment, bin)
+    const int64_t est_tiles = (A->dims.n_rows + R - 1) / R;
+    int64_t job_tiles = (est_tiles + (int64_t)A->sm_count * 16 - 1) / ((int64_t)A->sm_count * 16);
+    if (job_tiles < 1) job_tiles = 1;
+    if (job_tiles > JOB_TILES_MAX) job_tiles = JOB_TILES_MAX;
+    for (int b = 0; b < A->nbins; ++b) {
+        const int rows = info[b];
+        if (rows == 0) continue;
+        const int64_t t0 = A->n_tiles + info[A->nbins + b] / R;
+        const int64_t nt = (rows + R - 1) / R;
+        for (int64_t t = 0; t < nt; t += job_tiles) {
+            Job j;
+            j.tile0 = (int32_t)(t0 + t);
+            j.ntiles = (int32_t)(nt - t < job_tiles ? nt - t : job_tiles);
+            j.a0 = b * A->bin_width;
+            j.pad_ = 0;
+            A->jobs_host->push_back(j);
+        }
+    }
+    A->n_tiles += info[2 * A->nbins] / R;
+    if (A->n_tiles > A->tiles_cap) return GSR_ECUDA;   // cannot happen: capacity is an upper bound
+    A->seg_fill = 0;
+    return GSR_OK;
+}
+
+static void free_staging(gsr_matrix* A) {
+    const size_t c = (size_t)A->seg_cap;
+    dev_free(A, A->st_star, c * 4); A->st_star = nullptr;
+    dev_free(A, A->st_att, c * 4); A->st_att = nullptr;
+    dev_free(A, A->st_instr, c * 24); A->st_instr = nullptr;
+    dev_free(A, A->st_vals, c * 192); A->st_vals = nullptr;
+    if (A->seg_counts) {
+        const size_t nblk = (c + 255) / 256;
+        dev_free(A, A->seg_counts, (size_t)A->nbins * nblk * 4);
+        A->seg_counts = nullptr;
+    }
+}
+
 extern "C" {
 
 const char* gsr_strerror(int code) {
@@ -145,7 +307,7 @@ const char* gsr_strerror(int code) {
         case GSR_ENOMEM: return "out of device memory";
         case GSR_ECUDA: return "CUDA runtime error";
         case GSR_ESTATE: return "call not legal in this state";
-        case GSR_EUNSUPPORTED: return "unsupported device (needs sm_100) or option";
+        case GSR_EUNSUPPORTED: return "unsupported device (needs sm_100), size or option";
         default: return "unknown gsr status";
     }
 }
@@ -158,8 +320,22 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
     if (!d) return GSR_EINVAL;
     if (d->n_rows < 0 || d->n_stars < 1 || d->n_dfa < 4 || d->n_instr < 1 || d->n_glob != 1)
         return GSR_EINVAL;
-    int64_t n = 5 * d->n_stars + 3 * d->n_dfa + d->n_instr + 1;
-    if (n >= (int64_t)1 << 31) return GSR_EINVAL;
+    const int64_t n = 5 * d->n_stars + 3 * d->n_dfa + d->n_instr + 1;
+    if (n >= (int64_t)1 << 31 || d->n_rows >= (int64_t)0xFFFFFFF0) return GSR_EINVAL;
+    // shared-memory plan of the product kernels: whole instrumental block + one attitude window
+    const int64_t instr_bytes = d->n_instr * 8;
+    if (instr_bytes > SMEM_BUDGET - 24 * 1024) return GSR_EUNSUPPORTED;
+    int64_t att_budget = ATT_WIN_BYTES;
+    const int64_t half = 110 * 1024;   // two CTAs per SM when everything fits in 110 KB
+    if (instr_bytes + 16 * 1024 <= half) att_budget = att_budget < half - instr_bytes ? att_budget : half - instr_bytes;
+    else if (SMEM_BUDGET - instr_bytes < att_budget) att_budget = SMEM_BUDGET - instr_bytes;
+    const int64_t n_start = d->n_dfa - 3;
+    int64_t bw_max = att_budget / 24 - 3;
+    if (bw_max < 1) return GSR_EUNSUPPORTED;
+    const int64_t nbins = (n_start + bw_max - 1) / bw_max;
+    if (nbins > NBIN_MAX) return GSR_EUNSUPPORTED;
+    const int64_t bw = (n_start + nbins - 1) / nbins;
+
     int dev = 0;
     cudaDeviceProp prop;
     GSR_CUDA_TRY(cudaGetDevice(&dev));
@@ -169,25 +345,42 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
     if (!A) return GSR_ENOMEM;
     memset((void*)A, 0, sizeof(*A));
     new (&A->ws) Workspace();
+    A->jobs_host = new (std::nothrow) std::vector<Job>();
     A->dims = *d;
     A->n_cols = n;
     A->off_att = 5 * d->n_stars;
     A->off_instr = A->off_att + 3 * d->n_dfa;
     A->off_glob = A->off_instr + d->n_instr;
-    A->n_tiles = (d->n_rows + R - 1) / R;
-    A->m_pad = A->n_tiles * R;
+    A->nbins = (int)nbins;
+    A->bin_width = (int)bw;
+    A->win = (int)bw + 3;
+    A->smem_bytes = (int)((3 * (bw + 3) + d->n_instr + 2) * 8);
     A->stream = (cudaStream_t)stream;
     A->sm_count = prop.multiProcessorCount;
-    int rc = dev_alloc(A, (void**)&A->tiles, (size_t)A->n_tiles * TILE_BYTES);
+    A->seg_cap = d->n_rows < SEG ? (d->n_rows > 0 ? d->n_rows : 1) : SEG;
+    const int64_t n_seg = (d->n_rows + SEG - 1) / SEG;
+    A->tiles_cap = (d->n_rows + R - 1) / R + n_seg * nbins + 1;
+    const size_t c = (size_t)A->seg_cap, nblk = (c + 255) / 256;
+    int rc = dev_alloc(A, (void**)&A->tiles, (size_t)A->tiles_cap * TILE_BYTES);
+    if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->perm, (size_t)A->tiles_cap * R * 4);
+    if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->st_star, c * 4);
+    if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->st_att, c * 4);
+    if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->st_instr, c * 24);
+    if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->st_vals, c * 192);
+    if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->seg_counts, (size_t)nbins * nblk * 4);
+    if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->seg_bin_rows, (2 * nbins + 1) * 4);
+    if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->last_star, 4);
     if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->err, sizeof(int));
     if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->coef_one, 2 * sizeof(double));
-    if (rc != GSR_OK) {
+    if (rc != GSR_OK || !A->jobs_host) {
         gsr_matrix_destroy(A);
-        return rc;
+        return rc != GSR_OK ? rc : GSR_ENOMEM;
     }
     const double ones[2] = {1.0, 1.0};
-    cudaError_t e = cudaMemsetAsync(A->tiles, 0, (size_t)A->n_tiles * TILE_BYTES, A->stream);
+    cudaError_t e = cudaMemsetAsync(A->tiles, 0, (size_t)A->tiles_cap * TILE_BYTES, A->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(A->perm, 0xFF, (size_t)A->tiles_cap * R * 4, A->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(A->err, 0, sizeof(int), A->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(A->last_star, 0, 4, A->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(A->coef_one, ones, sizeof(ones), cudaMemcpyHostToDevice, A->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(A->stream);
     if (e != cudaSuccess) {
@@ -199,19 +392,6 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
     return GSR_OK;
 }
 
-static int append_device(gsr_matrix* A, int64_t row0, int64_t nrows, const int32_t* star,
-                         const int32_t* att, const int32_t* instr, const double* vals) {
-    if (nrows == 0) return GSR_OK;
-    const int threads = 256;
-    const int64_t blocks = (nrows + threads - 1) / threads;
-    k_layout_rows<<<(unsigned)blocks, threads, 0, A->stream>>>(A->tiles, row0, nrows, star, att, instr, vals,
-                                                               A->dims.n_stars, A->dims.n_dfa,
-                                                               A->dims.n_instr, A->err);
-    count_launch();
-    GSR_CUDA_TRY(cudaGetLastError());
-    return GSR_OK;
-}
-
 int gsr_matrix_append_rows(gsr_matrix* A, int64_t row0, int64_t nrows, const int32_t* star,
                            const int32_t* att, const int32_t* instr, const double* vals) {
     if (!A) return GSR_EINVAL;
@@ -219,42 +399,22 @@ int gsr_matrix_append_rows(gsr_matrix* A, int64_t row0, int64_t nrows, const int
     if (nrows < 0 || row0 != A->rows_appended || row0 + nrows > A->dims.n_rows) return GSR_EINVAL;
     if (nrows == 0) return GSR_OK;
     if (!star || !att || !instr || !vals) return GSR_EINVAL;
-    const bool dev = is_device_ptr(star);
-    if (dev != is_device_ptr(att) || dev != is_device_ptr(instr) || dev != is_device_ptr(vals))
-        return GSR_EINVAL;
-    if (dev) {
-        GSR_TRY(append_device(A, row0, nrows, star, att, instr, vals));
-    } else {
-        // host arrays: stage through a bounded device buffer (224 B per row)
-        const int64_t chunk = 1 << 20;
-        const size_t need = (size_t)(nrows < chunk ? nrows : chunk) * 224;
-        if (A->stage_bytes < need) {
-            if (A->stage) {
-                cudaFree(A->stage);
-                A->device_bytes -= (int64_t)A->stage_bytes;
-                A->stage = nullptr;
-                A->stage_bytes = 0;
-            }
-            GSR_TRY(dev_alloc(A, &A->stage, need));
-            A->stage_bytes = need;
-        }
-        for (int64_t r0 = 0; r0 < nrows; r0 += chunk) {
-            int64_t nr = nrows - r0 < chunk ? nrows - r0 : chunk;
-            unsigned char* sb = (unsigned char*)A->stage;
-            double* dv = (double*)sb;
-            int32_t* ds = (int32_t*)(sb + (size_t)nr * 192);
-            int32_t* da = ds + nr;
-            int32_t* di = da + nr;
-            GSR_CUDA_TRY(cudaMemcpyAsync(dv, vals + 24 * r0, (size_t)nr * 192, cudaMemcpyHostToDevice, A->stream));
-            GSR_CUDA_TRY(cudaMemcpyAsync(ds, star + r0, (size_t)nr * 4, cudaMemcpyHostToDevice, A->stream));
-            GSR_CUDA_TRY(cudaMemcpyAsync(da, att + r0, (size_t)nr * 4, cudaMemcpyHostToDevice, A->stream));
-            GSR_CUDA_TRY(cudaMemcpyAsync(di, instr + 6 * r0, (size_t)nr * 24, cudaMemcpyHostToDevice, A->stream));
-            GSR_TRY(append_device(A, row0 + r0, nr, ds, da, di, dv));
-            // the staging buffer is reused by the next chunk
-            GSR_CUDA_TRY(cudaStreamSynchronize(A->stream));
-        }
+    // host or device arrays: cudaMemcpyDefault resolves the direction per pointer
+    for (int64_t r0 = 0; r0 < nrows;) {
+        int64_t nr = A->seg_cap - A->seg_fill;
+        if (nr > nrows - r0) nr = nrows - r0;
+        const int64_t f = A->seg_fill;
+        GSR_CUDA_TRY(cudaMemcpyAsync(A->st_star + f, star + r0, (size_t)nr * 4, cudaMemcpyDefault, A->stream));
+        GSR_CUDA_TRY(cudaMemcpyAsync(A->st_att + f, att + r0, (size_t)nr * 4, cudaMemcpyDefault, A->stream));
+        GSR_CUDA_TRY(cudaMemcpyAsync(A->st_instr + 6 * f, instr + 6 * r0, (size_t)nr * 24, cudaMemcpyDefault, A->stream));
+        GSR_CUDA_TRY(cudaMemcpyAsync(A->st_vals + 24 * f, vals + 24 * r0, (size_t)nr * 192, cudaMemcpyDefault, A->stream));
+        A->seg_fill += nr;
+        A->rows_appended += nr;
+        r0 += nr;
+        if (A->seg_fill == A->seg_cap || A->rows_appended == A->dims.n_rows) GSR_TRY(flush_segment(A));
     }
-    A->rows_appended += nrows;
+    // the caller may free or overwrite its arrays once this returns
+    GSR_CUDA_TRY(cudaStreamSynchronize(A->stream));
     return GSR_OK;
 }
 
@@ -262,16 +422,24 @@ int gsr_matrix_finalize(gsr_matrix* A) {
     if (!A) return GSR_EINVAL;
     if (A->state != 0) return GSR_ESTATE;
     if (A->rows_appended != A->dims.n_rows) return GSR_ESTATE;
+    GSR_TRY(flush_segment(A));
     int err = 0;
     GSR_CUDA_TRY(cudaMemcpyAsync(&err, A->err, sizeof(int), cudaMemcpyDeviceToHost, A->stream));
     GSR_CUDA_TRY(cudaStreamSynchronize(A->stream));
-    if (A->stage) {
-        cudaFree(A->stage);
-        A->device_bytes -= (int64_t)A->stage_bytes;
-        A->stage = nullptr;
-        A->stage_bytes = 0;
-    }
+    free_staging(A);
     if (err != 0) return GSR_EINVAL;
+    A->n_jobs = (int)A->jobs_host->size();
+    A->m_int = A->n_tiles * R;
+    GSR_TRY(dev_alloc(A, (void**)&A->jobs, (size_t)(A->n_jobs > 0 ? A->n_jobs : 1) * sizeof(Job)));
+    if (A->n_jobs > 0) {
+        GSR_CUDA_TRY(cudaMemcpyAsync(A->jobs, A->jobs_host->data(), (size_t)A->n_jobs * sizeof(Job),
+                                     cudaMemcpyHostToDevice, A->stream));
+        k_fix_padding<<<A->n_jobs, R, 0, A->stream>>>(A->tiles, A->perm, A->jobs, A->n_jobs);
+        count_launch();
+        GSR_CUDA_TRY(cudaGetLastError());
+    }
+    GSR_CUDA_TRY(cudaStreamSynchronize(A->stream));
+    GSR_TRY(configure_product_kernels(A));
     A->state = 1;
     return GSR_OK;
 }
@@ -298,12 +466,17 @@ int gsr_matrix_create(gsr_matrix** out, const gsr_dims* dims, const int32_t* sta
 int gsr_matrix_destroy(gsr_matrix* A) {
     if (!A) return GSR_OK;
     free_workspace(A);
+    free_staging(A);
     cudaFree(A->tiles);
+    cudaFree(A->perm);
+    cudaFree(A->jobs);
+    cudaFree(A->seg_bin_rows);
+    cudaFree(A->last_star);
     cudaFree(A->p);
     cudaFree(A->err);
     cudaFree(A->coef_one);
-    cudaFree(A->stage);
     cudaGetLastError();
+    delete A->jobs_host;
     delete A;
     return GSR_OK;
 }
@@ -321,7 +494,7 @@ int gsr_set_option(gsr_matrix* A, int key, int64_t value) {
     if (!A) return GSR_EINVAL;
     switch (key) {
         case GSR_OPT_FORCE_ITNLIM: A->opt_force_itnlim = value != 0; return GSR_OK;
-        case GSR_OPT_DETERMINISTIC: A->opt_deterministic = value != 0; return GSR_OK;
+        case GSR_OPT_DETERMINISTIC: return value == 0 ? GSR_OK : GSR_EUNSUPPORTED;
         default: return GSR_EINVAL;
     }
 }
@@ -341,8 +514,8 @@ int gsr_debug_expand_rows(const gsr_matrix* A, int64_t row0, int64_t nrows, int6
         cudaGetLastError();
         return GSR_ENOMEM;
     }
-    k_expand_rows<<<(unsigned)((nrows + 255) / 256), 256, 0, A->stream>>>(
-        A->tiles, row0, nrows, A->dims.n_stars, A->dims.n_dfa, A->dims.n_instr, dc, dv);
+    k_expand_rows<<<(unsigned)((A->m_int + 255) / 256), 256, 0, A->stream>>>(
+        A->tiles, A->perm, A->m_int, row0, nrows, A->dims.n_stars, A->dims.n_dfa, A->dims.n_instr, dc, dv);
     count_launch();
     e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpyAsync(cols_host, dc, (size_t)nrows * NPAR * 8, cudaMemcpyDeviceToHost, A->stream);
@@ -373,14 +546,9 @@ int gsr_precondition(gsr_matrix* A, double* p_out, gsr_stream stream) {
     }
     GSR_CUDA_TRY(cudaGetLastError());
     if (p_out) {
-        if (is_device_ptr(p_out)) {
-            GSR_CUDA_TRY(cudaMemcpyAsync(p_out, A->p, (size_t)A->n_cols * 8, cudaMemcpyDeviceToDevice, s));
-        } else {
-            GSR_CUDA_TRY(cudaMemcpyAsync(p_out, A->p, (size_t)A->n_cols * 8, cudaMemcpyDeviceToHost, s));
-            GSR_CUDA_TRY(cudaStreamSynchronize(s));
-        }
+        GSR_CUDA_TRY(cudaMemcpyAsync(p_out, A->p, (size_t)A->n_cols * 8, cudaMemcpyDefault, s));
+        if (!is_device_ptr(p_out)) GSR_CUDA_TRY(cudaStreamSynchronize(s));
     }
-    A->ws.graph_valid = false;
     return GSR_OK;
 }
 
