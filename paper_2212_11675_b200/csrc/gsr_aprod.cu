@@ -12,8 +12,8 @@
 
 namespace gsr {
 
-constexpr int TPB = 512;                 // threads per product CTA: two tiles in flight
-constexpr int TILES_PER_STEP = TPB / R;
+constexpr int TPB1 = 1024;               // aprod1: four tiles in flight per CTA (latency-bound)
+constexpr int TPB2 = 512;                // aprod2: two tiles in flight (shared-memory-pipe-bound)
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
@@ -27,18 +27,30 @@ struct RowRegs {
     int32_t c[6];
 };
 
+// Streaming loads of one row, all 32 issued back to back (volatile asm keeps them together and
+// ahead of their first use, so every thread has 224 bytes in flight).
+__device__ __forceinline__ double ld_stream_f64(const double* p) {
+    double v;
+    asm volatile("ld.global.cs.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ int32_t ld_stream_s32(const int32_t* p) {
+    int32_t v;
+    asm volatile("ld.global.cs.s32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
 __device__ __forceinline__ void load_row(const unsigned char* __restrict__ T, int lr, RowRegs& r) {
+    r.s = ld_stream_s32((const int32_t*)(T + OFF_STAR) + lr);
+    r.a = ld_stream_s32((const int32_t*)(T + OFF_ATT) + lr);
 #pragma unroll
-    for (int k = 0; k < NPAR; ++k) r.v[k] = __ldcs((const double*)(T + k * R * 8) + lr);
-    r.s = __ldcs((const int32_t*)(T + OFF_STAR) + lr);
-    r.a = __ldcs((const int32_t*)(T + OFF_ATT) + lr);
+    for (int j = 0; j < 6; ++j) r.c[j] = ld_stream_s32((const int32_t*)(T + OFF_INSTR + j * R * 4) + lr);
 #pragma unroll
-    for (int j = 0; j < 6; ++j) r.c[j] = __ldcs((const int32_t*)(T + OFF_INSTR + j * R * 4) + lr);
+    for (int k = 0; k < NPAR; ++k) r.v[k] = ld_stream_f64((const double*)(T + k * R * 8) + lr);
 }
 
 // ---- aprod1: y[i] = ca*y[i] + sum_k A[i,k] x[col(i,k)]  (Algorithm 1) --------------------
 template <bool NORM, bool PERM>
-__global__ void __launch_bounds__(TPB) k_aprod1(const unsigned char* __restrict__ tiles,
+__global__ void __launch_bounds__(TPB1) k_aprod1(const unsigned char* __restrict__ tiles,
                                                 const Job* __restrict__ jobs,
                                                 const double* __restrict__ x, double* __restrict__ y,
                                                 const double* __restrict__ ca_p,
@@ -48,25 +60,25 @@ __global__ void __launch_bounds__(TPB) k_aprod1(const unsigned char* __restrict_
                                                 const int* __restrict__ stop) {
     if (stop && *stop) return;
     extern __shared__ double xw[];
-    __shared__ double red[TPB / 32];
+    __shared__ double red[TPB1 / 32];
     const Job job = jobs[blockIdx.x];
     const double* xatt = x + 5 * S;
     const double* xins = x + 5 * S + 3 * D;
     // stage the attitude window (three axes) and the instrumental block
-    for (int i = threadIdx.x; i < 3 * win; i += TPB) {
+    for (int i = threadIdx.x; i < 3 * win; i += TPB1) {
         const int ax = i / win, j = i - ax * win;
         const int64_t knot = (int64_t)job.a0 + j;
         xw[i] = knot < D ? __ldg(xatt + ax * D + knot) : 0.0;
     }
     double* xi = xw + 3 * win;
-    for (int i = threadIdx.x; i < I; i += TPB) xi[i] = __ldg(xins + i);
+    for (int i = threadIdx.x; i < I; i += TPB1) xi[i] = __ldg(xins + i);
     const double xg = __ldg(xins + I);
     const double ca = *ca_p;
     __syncthreads();
 
     const int sub = threadIdx.x / R, lr = threadIdx.x % R;
     double q = 0.0;
-    for (int t = sub; t < job.ntiles; t += TILES_PER_STEP) {
+    for (int t = sub; t < job.ntiles; t += (TPB1 / R)) {
         const int64_t tile = (int64_t)job.tile0 + t;
         const unsigned char* T = tiles + tile * TILE_BYTES;
         RowRegs r;
@@ -103,7 +115,7 @@ __global__ void __launch_bounds__(TPB) k_aprod1(const unsigned char* __restrict_
         if (threadIdx.x == 0) {
             double tsum = 0.0;
 #pragma unroll
-            for (int w = 0; w < TPB / 32; ++w) tsum += red[w];
+            for (int w = 0; w < TPB1 / 32; ++w) tsum += red[w];
             partials[blockIdx.x] = tsum;
         }
     }
@@ -116,7 +128,7 @@ __global__ void __launch_bounds__(TPB) k_aprod1(const unsigned char* __restrict_
 // column: register accumulation over the whole job, one atomic per job.
 // SQUARE: accumulate A[i,k]^2 instead (column sums of squares for the preconditioner).
 template <bool SQUARE, bool PERM>
-__global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict__ tiles,
+__global__ void __launch_bounds__(TPB2) k_aprod2(const unsigned char* __restrict__ tiles,
                                                 const Job* __restrict__ jobs,
                                                 const double* __restrict__ y, double* __restrict__ x,
                                                 const double* __restrict__ sy_p,
@@ -125,17 +137,17 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
                                                 const int* __restrict__ stop) {
     if (stop && *stop) return;
     extern __shared__ double xw[];
-    __shared__ double red[TPB / 32];
+    __shared__ double red[TPB2 / 32];
     const Job job = jobs[blockIdx.x];
     const int nacc = 3 * win + I;
-    for (int i = threadIdx.x; i < nacc; i += TPB) xw[i] = 0.0;
+    for (int i = threadIdx.x; i < nacc; i += TPB2) xw[i] = 0.0;
     double* xi = xw + 3 * win;
     const double sy = SQUARE ? 1.0 : *sy_p;
     __syncthreads();
 
     const int sub = threadIdx.x / R, lr = threadIdx.x % R, lane = threadIdx.x & 31;
     double g = 0.0;
-    for (int t = sub; t < job.ntiles; t += TILES_PER_STEP) {
+    for (int t = sub; t < job.ntiles; t += (TPB2 / R)) {
         const int64_t tile = (int64_t)job.tile0 + t;
         const unsigned char* T = tiles + tile * TILE_BYTES;
         RowRegs r;
@@ -198,12 +210,12 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
     if (threadIdx.x == 0) {
         double tsum = 0.0;
 #pragma unroll
-        for (int w = 0; w < TPB / 32; ++w) tsum += red[w];
+        for (int w = 0; w < TPB2 / 32; ++w) tsum += red[w];
         if (tsum != 0.0) atomicAdd(x + 5 * S + 3 * D + I, tsum);
     }
     // flush the privatised accumulators
     double* xatt = x + 5 * S;
-    for (int i = threadIdx.x; i < 3 * win; i += TPB) {
+    for (int i = threadIdx.x; i < 3 * win; i += TPB2) {
         const double vacc = xw[i];
         if (vacc != 0.0) {
             const int ax = i / win, j = i - ax * win;
@@ -211,7 +223,7 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
         }
     }
     double* xins = x + 5 * S + 3 * D;
-    for (int i = threadIdx.x; i < I; i += TPB) {
+    for (int i = threadIdx.x; i < I; i += TPB2) {
         const double vacc = xi[i];
         if (vacc != 0.0) atomicAdd(xins + i, vacc);
     }
@@ -223,11 +235,17 @@ static int set_smem(K kernel, int bytes) {
     return GSR_OK;
 }
 
-int configure_product_kernels(const gsr_matrix* A) {
+static int aprod1_smem(const gsr_matrix* A) {
     const int b = A->smem_bytes;
+    return b;   // measured: 2 CTAs x 1024 threads (64 warps) beat 1 CTA with a larger L1
+}
+
+int configure_product_kernels(const gsr_matrix* A) {
+    int b = aprod1_smem(A);
     GSR_TRY(set_smem(k_aprod1<true, false>, b));
     GSR_TRY(set_smem(k_aprod1<false, false>, b));
     GSR_TRY(set_smem(k_aprod1<false, true>, b));
+    b = A->smem_bytes;
     GSR_TRY(set_smem(k_aprod2<false, false>, b));
     GSR_TRY(set_smem(k_aprod2<false, true>, b));
     GSR_TRY(set_smem(k_aprod2<true, false>, b));
@@ -240,13 +258,13 @@ int launch_aprod1(const gsr_matrix* A, const double* x, double* y, const double*
     const int64_t S = A->dims.n_stars, D = A->dims.n_dfa;
     const int I = (int)A->dims.n_instr;
     if (perm)
-        k_aprod1<false, true><<<A->n_jobs, TPB, A->smem_bytes, s>>>(A->tiles, A->jobs, x, y, ca, nullptr,
+        k_aprod1<false, true><<<A->n_jobs, TPB1, aprod1_smem(A), s>>>(A->tiles, A->jobs, x, y, ca, nullptr,
                                                                     perm, S, D, I, A->win, stop);
     else if (partials)
-        k_aprod1<true, false><<<A->n_jobs, TPB, A->smem_bytes, s>>>(A->tiles, A->jobs, x, y, ca, partials,
+        k_aprod1<true, false><<<A->n_jobs, TPB1, aprod1_smem(A), s>>>(A->tiles, A->jobs, x, y, ca, partials,
                                                                     nullptr, S, D, I, A->win, stop);
     else
-        k_aprod1<false, false><<<A->n_jobs, TPB, A->smem_bytes, s>>>(A->tiles, A->jobs, x, y, ca, nullptr,
+        k_aprod1<false, false><<<A->n_jobs, TPB1, aprod1_smem(A), s>>>(A->tiles, A->jobs, x, y, ca, nullptr,
                                                                      nullptr, S, D, I, A->win, stop);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
@@ -259,10 +277,10 @@ int launch_aprod2(const gsr_matrix* A, const double* y, double* x, const double*
     const int64_t S = A->dims.n_stars, D = A->dims.n_dfa;
     const int I = (int)A->dims.n_instr;
     if (perm)
-        k_aprod2<false, true><<<A->n_jobs, TPB, A->smem_bytes, s>>>(A->tiles, A->jobs, y, x, sy, perm, S, D,
+        k_aprod2<false, true><<<A->n_jobs, TPB2, A->smem_bytes, s>>>(A->tiles, A->jobs, y, x, sy, perm, S, D,
                                                                     I, A->win, stop);
     else
-        k_aprod2<false, false><<<A->n_jobs, TPB, A->smem_bytes, s>>>(A->tiles, A->jobs, y, x, sy, nullptr, S,
+        k_aprod2<false, false><<<A->n_jobs, TPB2, A->smem_bytes, s>>>(A->tiles, A->jobs, y, x, sy, nullptr, S,
                                                                      D, I, A->win, stop);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
@@ -271,7 +289,7 @@ int launch_aprod2(const gsr_matrix* A, const double* y, double* x, const double*
 
 int launch_colsumsq(const gsr_matrix* A, double* q, cudaStream_t s) {
     if (A->n_jobs == 0) return GSR_OK;
-    k_aprod2<true, false><<<A->n_jobs, TPB, A->smem_bytes, s>>>(A->tiles, A->jobs, nullptr, q, nullptr,
+    k_aprod2<true, false><<<A->n_jobs, TPB2, A->smem_bytes, s>>>(A->tiles, A->jobs, nullptr, q, nullptr,
                                                                 nullptr, A->dims.n_stars, A->dims.n_dfa,
                                                                 (int)A->dims.n_instr, A->win, nullptr);
     count_launch();

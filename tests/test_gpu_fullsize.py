@@ -1,0 +1,151 @@
+"""Full-size GPU checks at BASELINE.json's sizes, in the configuration bench.py times
+(chunked device-side ingest, preconditioned, fixed-count solve).  The oracle cannot run 1e8
+to 3e8 rows, so it computes SAMPLED outputs one by one:
+  * aprod1: sampled rows (the oracle gets exactly those rows of the generator's arrays);
+  * aprod2: every column touched only by a row set that can be collected during ingest --
+    the 5 astrometric columns of sampled stars, one attitude column (rows whose 4-knot window
+    covers it) and one instrumental column -- for which the oracle sums the collected rows;
+plus properties that hold at any size: the adjoint identity (covers the global column) and
+LSQR's residual estimate against the directly computed ||b - A x||."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2212_11675_b200 import inputs
+from oracle.gsr_oracle import OracleSystem
+
+pytestmark = pytest.mark.gpu
+GEN_ROWS = 1 << 23
+
+
+def _need_gb(gb):
+    free, _ = torch.cuda.mem_get_info()
+    if free < gb * 1e9:
+        pytest.skip(f"needs {gb} GB of free device memory")
+
+
+def _build_and_collect(cfg, g, probe_knot, probe_instr, probe_rows):
+    """Ingest cfg chunk by chunk; keep host copies of the rows the probes need."""
+    dev = "cuda"
+    sptr = inputs.star_ptr(cfg)
+    scales = inputs.col_scales(cfg, dev)
+    h = g.gsr_matrix_begin(cfg.n_rows, cfg.n_stars, cfg.n_dfa, cfg.n_instr)
+    keep = {"rows": [], "knot": [], "instr": []}
+    probe_rows_t = torch.as_tensor(probe_rows, device=dev)
+    for r0 in range(0, cfg.n_rows, GEN_ROWS):
+        nr = min(GEN_ROWS, cfg.n_rows - r0)
+        star, att, instr, vals = inputs.gen_rows(cfg, r0, nr, dev, sptr=sptr, scales=scales)
+        g.gsr_matrix_append_rows(h, r0, nr, star, att, instr, vals)
+        sel = probe_rows_t[(probe_rows_t >= r0) & (probe_rows_t < r0 + nr)] - r0
+        mk = (att <= probe_knot) & (att >= probe_knot - 3)
+        mi = (instr == probe_instr).any(dim=1)
+        for key, idx in (("rows", sel), ("knot", mk.nonzero().squeeze(1)), ("instr", mi.nonzero().squeeze(1))):
+            keep[key].append((idx.cpu() + r0, star[idx].cpu(), att[idx].cpu(), instr[idx].cpu(), vals[idx].cpu()))
+        del star, att, instr, vals
+    g.gsr_matrix_finalize(h)
+    out = {}
+    for key, parts in keep.items():
+        out[key] = tuple(torch.cat([p[i] for p in parts]).numpy() for i in range(5))
+    return h, sptr, out
+
+
+def _oracle_rows(cfg, part):
+    _, star, att, instr, vals = part
+    return OracleSystem(cfg.n_stars, cfg.n_dfa, cfg.n_instr, star, att, instr, vals)
+
+
+@pytest.mark.parametrize("name,gb", [("cfg2", 40), ("cfg4", 40), ("cfg3", 110)])
+def test_fullsize_sampled_parity_and_properties(name, gb):
+    from paper_2212_11675_b200 import binding as g
+    _need_gb(gb)
+    cfg = inputs.named_config(name)
+    m, n = cfg.n_rows, cfg.n_cols
+    rng = np.random.default_rng(cfg.seed)
+    probe_rows = np.unique(rng.integers(0, m, 4000))
+    probe_knot = int(0.42 * (cfg.n_dfa - 3)) + 5       # inside config 4's hot window
+    probe_instr = int(rng.integers(0, cfg.n_instr))
+    h, sptr, kept = _build_and_collect(cfg, g, probe_knot, probe_instr, probe_rows)
+    try:
+        x = inputs.random_vector(cfg, 1, n, "cuda")
+        y = inputs.random_vector(cfg, 2, m, "cuda")
+        # ---- aprod1 on sampled rows
+        y0 = inputs.random_vector(cfg, 3, m, "cuda")
+        yd = y0.clone()
+        g.gsr_aprod1(h, x, yd)
+        rows = kept["rows"][0]
+        o = _oracle_rows(cfg, kept["rows"])
+        ref, scale = o.aprod1(x.cpu().numpy(), y0[rows].cpu().numpy(), want_scale=True)
+        err = np.abs(yd[rows].cpu().numpy() - ref)
+        assert np.all(err <= 1e-12 * scale), float((err / scale).max())
+        # index construction of the sampled rows, bit-exact, through the device layout
+        for r in rows[:50]:
+            c, v = g.gsr_debug_expand_rows(h, int(r), 1)
+            i = int(np.searchsorted(rows, r))
+            oc, ov = o.expand_rows(i, 1)
+            assert np.array_equal(c, oc) and np.array_equal(v, ov)
+        # ---- aprod2
+        x0 = inputs.random_vector(cfg, 4, n, "cuda")
+        xd = x0.clone()
+        g.gsr_aprod2(h, y, xd)
+        xh, x0h = xd.cpu().numpy(), x0.cpu().numpy()
+        # attitude column probe_knot of every axis, and one instrumental column
+        for key, cols in (("knot", [cfg.off_att + ax * cfg.n_dfa + probe_knot for ax in range(3)]),
+                          ("instr", [cfg.off_instr + probe_instr])):
+            o2 = _oracle_rows(cfg, kept[key])
+            ysub = y[kept[key][0]].cpu().numpy()
+            ref, scale = o2.aprod2(ysub, x0h, want_scale=True)
+            for c in cols:
+                assert abs(xh[c] - ref[c]) <= 1e-12 * scale[c], (key, c, abs(xh[c] - ref[c]) / scale[c])
+        # astrometric columns of sampled stars: their rows are one contiguous run
+        stars = rng.integers(0, cfg.n_stars, 6)
+        for s in stars:
+            r0, r1 = int(sptr[s]), int(sptr[s + 1])
+            if r1 == r0:
+                assert np.array_equal(xh[5 * s:5 * s + 5], x0h[5 * s:5 * s + 5])
+                continue
+            c0 = (r0 // inputs.CHUNK) * inputs.CHUNK
+            st, at, ic, va = inputs.gen_rows(cfg, c0, r1 - c0, "cuda", sptr=sptr)
+            sl = slice(r0 - c0, r1 - c0)
+            o3 = OracleSystem(cfg.n_stars, cfg.n_dfa, cfg.n_instr, st[sl].cpu().numpy(), at[sl].cpu().numpy(),
+                              ic[sl].cpu().numpy(), va[sl].cpu().numpy())
+            ref, scale = o3.aprod2(y[r0:r1].cpu().numpy(), x0h, want_scale=True)
+            seg = slice(5 * int(s), 5 * int(s) + 5)
+            assert np.all(np.abs(xh[seg] - ref[seg]) <= 1e-12 * scale[seg])
+        # ---- adjoint identity <A x, y> = <x, A^T y> at full size (covers the global column)
+        Ax = torch.zeros(m, dtype=torch.float64, device="cuda")
+        ATy = torch.zeros(n, dtype=torch.float64, device="cuda")
+        g.gsr_aprod1(h, x, Ax)
+        g.gsr_aprod2(h, y, ATy)
+        lhs, rhs = float(Ax @ y), float(x @ ATy)
+        assert abs(lhs - rhs) <= 1e-11 * float(Ax.norm() * y.norm())
+        del Ax, ATy, yd, y0, xd, x0
+        # ---- LSQR in bench.py's configuration: estimates against directly computed norms
+        xt = inputs.x_true(cfg, "cuda")
+        b = torch.empty(m, dtype=torch.float64, device="cuda")
+        for r0 in range(0, m, GEN_ROWS):
+            nr = min(GEN_ROWS, m - r0)
+            b[r0:r0 + nr] = inputs.noise(cfg, r0, nr, "cuda")
+        g.gsr_aprod1(h, xt, b)                       # b = A x_true + noise, before scaling
+        res0 = b.clone()
+        p = torch.empty(n, dtype=torch.float64, device="cuda")
+        g.gsr_precondition(h, p)
+        g.gsr_set_option(h, g.GSR_OPT_FORCE_ITNLIM, 1)
+        xs = torch.empty(n, dtype=torch.float64, device="cuda")
+        K = 12
+        r = g.gsr_lsqr_solve(h, b, xs, K)
+        assert (r.istop, r.itn) == (7, K)
+        z = xs / p                                   # iterate of the scaled system
+        neg = -z
+        g.gsr_aprod1(h, neg, res0)                   # res0 = b - A' z
+        rn = float(res0.norm())
+        assert abs(r.rnorm - rn) <= 1e-8 * rn
+        assert abs(r.xnorm - float(z.norm())) <= 1e-8 * float(z.norm())
+        assert abs(r.bnorm - float(b.norm())) <= 1e-12 * float(b.norm())
+        at_r = torch.zeros(n, dtype=torch.float64, device="cuda")
+        g.gsr_aprod2(h, res0, at_r)
+        assert abs(r.arnorm - float(at_r.norm())) <= 1e-6 * r.anorm * r.rnorm
+        r2 = g.gsr_lsqr_solve(h, b, xs, K + 6)
+        assert r2.rnorm <= r.rnorm * (1 + 1e-12)
+    finally:
+        g.gsr_matrix_destroy(h)
+        torch.cuda.empty_cache()

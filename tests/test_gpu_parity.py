@@ -187,7 +187,7 @@ def test_lsqr_unpreconditioned_host_buffers():
         bp = torch.from_numpy(rhs).pin_memory()
         xp = torch.empty(s.n, dtype=torch.float64).pin_memory()
         b.gsr_lsqr_solve(s.A.h, bp, xp, 4)                # pinned host tensors
-        assert np.allclose(xp.numpy(), xh, rtol=1e-12, atol=1e-14)
+        assert np.linalg.norm(xp.numpy() - xh) <= 1e-11 * np.linalg.norm(xh)   # atomics: order varies
     finally:
         s.A.close()
 
