@@ -1,19 +1,25 @@
 // aprod mode 1 and mode 2 (rows a3, a5-a8): Algorithms 1 and 2 of the paper
-// on the tiled, attitude-binned layout of gsr_internal.h.
+// on the warp-tiled, attitude-binned layout of gsr_internal.h.
 //
-// One CTA runs one job = a run of tiles whose rows all start their attitude block inside one
-// window of `win` knots per axis.  The CTA keeps in shared memory
-//     xw[0 .. 3*win)          the attitude window of x (aprod1) or its accumulator (aprod2)
-//     xw[3*win .. 3*win+I)    the whole instrumental block
+// Warps are autonomous.  A persistent grid (one or two CTAs of 16 warps per SM) fetches UNITS
+// (runs of 32-row tiles whose attitude blocks start inside one window of `win` knots per axis)
+// from a global counter, one unit per warp at a time.  In shared memory
+//     xi[0 .. I)                      the whole instrumental block, shared by the CTA's warps
+//     xw[warp][0 .. 3*win)            the unit's attitude window, PRIVATE to the warp
 // so the 18 irregular column accesses of a row never leave the SM; only the
-// astrometric columns (5 per star, rows star-sorted inside a job) and the global column go
-// to L1/L2.  The matrix itself is streamed once, coalesced, plane by plane.
+// astrometric columns (5 per star, rows star-sorted inside a unit) and the global column go
+// to L1/L2.  The matrix is streamed exactly once, every request coalesced.
+//
+// Attitude block.  Lane j < 12 of each half-warp owns COEFFICIENT j of 16 rows (the tile stores
+// the 32x12 attitude block row-major, see gsr_internal.h), so for one row the 12 lanes touch
+// 12 distinct, conflict-free window addresses:
+//   aprod2: plain shared-memory read-modify-write, row after row, no atomics (the window is
+//           private to the warp, and rows of the same warp are serialised);
+//   aprod1: 12 products per row, transposed back to "lane r owns row r" by a 15-shuffle
+//           butterfly inside each half-warp.
 #include "gsr_internal.h"
 
 namespace gsr {
-
-constexpr int TPB1 = 1024;               // aprod1: four tiles in flight per CTA (latency-bound)
-constexpr int TPB2 = 512;                // aprod2: two tiles in flight (shared-memory-pipe-bound)
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
@@ -21,209 +27,257 @@ __device__ __forceinline__ double warp_sum(double v) {
     return v;
 }
 
-struct RowRegs {
-    double v[NPAR];
-    int32_t s, a;
-    int32_t c[6];
+struct TileRegs {
+    double as[5], in[6], gl;   // lane r: coefficients of row r
+    double at[16];             // lane (h, j): attitude coefficient min(j, 11) of rows 16h .. 16h+15
+    int32_t s;
+    uint32_t aoff;
+    uint32_t c[6];
 };
 
-// Streaming loads of one row, all 32 issued back to back (volatile asm keeps them together and
-// ahead of their first use, so every thread has 224 bytes in flight).
-__device__ __forceinline__ double ld_stream_f64(const double* p) {
+// Streaming loads of one tile, all issued back to back (volatile asm keeps them together and
+// ahead of their first use, so every lane has ~340 bytes in flight).
+__device__ __forceinline__ double ld_stream_f64(const void* p) {
     double v;
     asm volatile("ld.global.cs.f64 %0, [%1];" : "=d"(v) : "l"(p));
     return v;
 }
-__device__ __forceinline__ int32_t ld_stream_s32(const int32_t* p) {
+__device__ __forceinline__ int32_t ld_stream_s32(const void* p) {
     int32_t v;
     asm volatile("ld.global.cs.s32 %0, [%1];" : "=r"(v) : "l"(p));
     return v;
 }
-__device__ __forceinline__ void load_row(const unsigned char* __restrict__ T, int lr, RowRegs& r) {
-    r.s = ld_stream_s32((const int32_t*)(T + OFF_STAR) + lr);
-    r.a = ld_stream_s32((const int32_t*)(T + OFF_ATT) + lr);
+__device__ __forceinline__ uint32_t ld_stream_u16(const void* p) {
+    uint16_t v;
+    asm volatile("ld.global.cs.u16 %0, [%1];" : "=h"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void load_tile(const unsigned char* __restrict__ T, int lane, TileRegs& r) {
+    r.s = ld_stream_s32(T + OFF_STAR + lane * 4);
+    r.aoff = ld_stream_u16(T + OFF_AOFF + lane * 2);
 #pragma unroll
-    for (int j = 0; j < 6; ++j) r.c[j] = ld_stream_s32((const int32_t*)(T + OFF_INSTR + j * R * 4) + lr);
+    for (int j = 0; j < 6; ++j) r.c[j] = ld_stream_u16(T + OFF_ICOL + (j * R + lane) * 2);
 #pragma unroll
-    for (int k = 0; k < NPAR; ++k) r.v[k] = ld_stream_f64((const double*)(T + k * R * 8) + lr);
+    for (int k = 0; k < 5; ++k) r.as[k] = ld_stream_f64(T + OFF_ASTRO + (k * R + lane) * 8);
+    const int h = lane >> 4, jj = min(lane & 15, 11);
+#pragma unroll
+    for (int q = 0; q < 16; ++q) r.at[q] = ld_stream_f64(T + OFF_ATTV + ((q * 2 + h) * 12 + jj) * 8);
+#pragma unroll
+    for (int j = 0; j < 6; ++j) r.in[j] = ld_stream_f64(T + OFF_INSTRV + (j * R + lane) * 8);
+    r.gl = ld_stream_f64(T + OFF_GLOBV + lane * 8);
+}
+
+__device__ __forceinline__ int fetch_unit(int* counter, int lane) {
+    int u = 0;
+    if (lane == 0) u = atomicAdd(counter, 1);
+    return __shfl_sync(0xffffffffu, u, 0);
 }
 
 // ---- aprod1: y[i] = ca*y[i] + sum_k A[i,k] x[col(i,k)]  (Algorithm 1) --------------------
 template <bool NORM, bool PERM>
-__global__ void __launch_bounds__(TPB1) k_aprod1(const unsigned char* __restrict__ tiles,
-                                                const Job* __restrict__ jobs,
-                                                const double* __restrict__ x, double* __restrict__ y,
-                                                const double* __restrict__ ca_p,
-                                                double* __restrict__ partials,
-                                                const uint32_t* __restrict__ perm, int64_t S,
-                                                int64_t D, int I, int win,
-                                                const int* __restrict__ stop) {
+__global__ void __launch_bounds__(TPB) k_aprod1(const unsigned char* __restrict__ tiles,
+                                               const Unit* __restrict__ units, int n_units,
+                                               int* __restrict__ counter,
+                                               const double* __restrict__ x, double* __restrict__ y,
+                                               const double* __restrict__ ca_p,
+                                               double* __restrict__ partials,
+                                               const uint32_t* __restrict__ perm, int64_t S,
+                                               int64_t D, int I, int win,
+                                               const int* __restrict__ stop) {
     if (stop && *stop) return;
-    extern __shared__ double xw[];
-    __shared__ double red[TPB1 / 32];
-    const Job job = jobs[blockIdx.x];
+    extern __shared__ double sm[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double* xi = sm;
+    double* xw = sm + ((I + 1) & ~1) + warp * 3 * win;
     const double* xatt = x + 5 * S;
     const double* xins = x + 5 * S + 3 * D;
-    // stage the attitude window (three axes) and the instrumental block
-    for (int i = threadIdx.x; i < 3 * win; i += TPB1) {
-        const int ax = i / win, j = i - ax * win;
-        const int64_t knot = (int64_t)job.a0 + j;
-        xw[i] = knot < D ? __ldg(xatt + ax * D + knot) : 0.0;
-    }
-    double* xi = xw + 3 * win;
-    for (int i = threadIdx.x; i < I; i += TPB1) xi[i] = __ldg(xins + i);
+    for (int i = threadIdx.x; i < I; i += TPB) xi[i] = __ldg(xins + i);
     const double xg = __ldg(xins + I);
     const double ca = *ca_p;
     __syncthreads();
 
-    const int sub = threadIdx.x / R, lr = threadIdx.x % R;
-    double q = 0.0;
-    for (int t = sub; t < job.ntiles; t += (TPB1 / R)) {
-        const int64_t tile = (int64_t)job.tile0 + t;
-        const unsigned char* T = tiles + tile * TILE_BYTES;
-        RowRegs r;
-        load_row(T, lr, r);
-        const int64_t ri = tile * R + lr;
-        int64_t ry = ri;
-        bool live = true;
-        if (PERM) {
-            const uint32_t pe = __ldcs(perm + ri);
-            live = pe != PERM_PAD;
-            ry = pe;
+    const int h = lane >> 4, j = lane & 15, jj = min(j, 11);
+    const int axo = (jj >> 2) * win + (jj & 3);   // my coefficient's column, relative to aoff
+    const bool att_lane = j < 12;
+    for (;;) {
+        const int u = fetch_unit(counter, lane);
+        if (u >= n_units) break;
+        const Unit un = units[u];
+        __syncwarp();
+        for (int i = lane; i < 3 * win; i += 32) {
+            const int ax = i / win, k = i - ax * win;
+            const int64_t knot = (int64_t)un.a0 + k;
+            xw[i] = knot < D ? __ldg(xatt + ax * D + knot) : 0.0;
         }
-        const double yold = live ? y[ry] : 0.0;
-        const double* xa = x + 5 * (int64_t)r.s;
-        double sum = 0.0;
+        __syncwarp();
+        double q = 0.0;
+        for (int t = 0; t < un.ntiles; ++t) {
+            const int64_t tile = (int64_t)un.tile0 + t;
+            TileRegs r;
+            load_tile(tiles + tile * TILE_BYTES, lane, r);
+            const int64_t ri = tile * R + lane;
+            int64_t ry = ri;
+            bool live = true;
+            if (PERM) {
+                const uint32_t pe = __ldcs(perm + ri);
+                live = pe != PERM_PAD;
+                ry = pe;
+            }
+            const double yold = live ? y[ry] : 0.0;
+            // attitude: 12 lanes per row, products transposed back by a butterfly
+            double p[16];
 #pragma unroll
-        for (int k = 0; k < 5; ++k) sum = fma(r.v[k], __ldg(xa + k), sum);
-        const double* wa = xw + (r.a - job.a0);
+            for (int qq = 0; qq < 16; ++qq) {
+                const uint32_t a = __shfl_sync(0xffffffffu, r.aoff, h * 16 + qq);
+                const double pv = r.at[qq] * xw[a + axo];
+                p[qq] = att_lane ? pv : 0.0;
+            }
 #pragma unroll
-        for (int ax = 0; ax < 3; ++ax)
+            for (int o = 8; o > 0; o >>= 1) {
+                const bool up = (j & o) != 0;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) sum = fma(r.v[5 + 4 * ax + j], wa[ax * win + j], sum);
+                for (int i = 0; i < o; ++i) {
+                    const double send = up ? p[i] : p[i + o];
+                    const double keep = up ? p[i + o] : p[i];
+                    p[i] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+                }
+            }
+            double sum = p[0];   // lane (h, j) now holds the attitude part of row 16h + j
+            const double* xa = x + 5 * (int64_t)r.s;
 #pragma unroll
-        for (int j = 0; j < 6; ++j) sum = fma(r.v[17 + j], xi[r.c[j]], sum);
-        sum = fma(r.v[23], xg, sum);
-        const double ynew = fma(ca, yold, sum);
-        if (live) y[ry] = ynew;
-        if (NORM) q = fma(ynew, ynew, q);   // padding rows: y stays 0
-    }
-    if (NORM) {
-        q = warp_sum(q);
-        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = q;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            double tsum = 0.0;
+            for (int k = 0; k < 5; ++k) sum = fma(r.as[k], __ldg(xa + k), sum);
 #pragma unroll
-            for (int w = 0; w < TPB1 / 32; ++w) tsum += red[w];
-            partials[blockIdx.x] = tsum;
+            for (int k = 0; k < 6; ++k) sum = fma(r.in[k], xi[r.c[k]], sum);
+            sum = fma(r.gl, xg, sum);
+            const double ynew = fma(ca, yold, sum);
+            if (live) y[ry] = ynew;
+            if (NORM) q = fma(ynew, ynew, q);   // padding rows: y stays 0
+        }
+        if (NORM) {
+            q = warp_sum(q);
+            if (lane == 0) partials[u] = q;
         }
     }
 }
 
 // ---- aprod2: x[col(i,k)] += A[i,k] * (y[i]*sy)  (Algorithm 2) ----------------------------
-// attitude and instrumental blocks: shared-memory accumulators (privatised per job), flushed
-// once per job with one global atomic per touched column; astrometric block: segmented warp
-// reduction over the star-sorted rows, one global atomic per (warp, star, column); global
-// column: register accumulation over the whole job, one atomic per job.
+// attitude block: warp-private shared-memory window, plain read-modify-write (see above),
+// flushed once per unit with one global atomic per touched column; instrumental block: CTA-
+// shared shared-memory accumulators (fp64 atomicAdd = CAS loop on sm_100a), flushed once per
+// CTA; astrometric block: segmented warp reduction over the star-sorted rows, one global atomic
+// per (warp, star, column); global column: register accumulation, one atomic per warp.
 // SQUARE: accumulate A[i,k]^2 instead (column sums of squares for the preconditioner).
 template <bool SQUARE, bool PERM>
-__global__ void __launch_bounds__(TPB2) k_aprod2(const unsigned char* __restrict__ tiles,
-                                                const Job* __restrict__ jobs,
-                                                const double* __restrict__ y, double* __restrict__ x,
-                                                const double* __restrict__ sy_p,
-                                                const uint32_t* __restrict__ perm, int64_t S,
-                                                int64_t D, int I, int win,
-                                                const int* __restrict__ stop) {
+__global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict__ tiles,
+                                               const Unit* __restrict__ units, int n_units,
+                                               int* __restrict__ counter,
+                                               const double* __restrict__ y, double* __restrict__ x,
+                                               const double* __restrict__ sy_p,
+                                               const uint32_t* __restrict__ perm, int64_t S,
+                                               int64_t D, int I, int win,
+                                               const int* __restrict__ stop) {
     if (stop && *stop) return;
-    extern __shared__ double xw[];
-    __shared__ double red[TPB2 / 32];
-    const Job job = jobs[blockIdx.x];
-    const int nacc = 3 * win + I;
-    for (int i = threadIdx.x; i < nacc; i += TPB2) xw[i] = 0.0;
-    double* xi = xw + 3 * win;
+    extern __shared__ double sm[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double* xi = sm;
+    double* xw = sm + ((I + 1) & ~1) + warp * 3 * win;
+    for (int i = threadIdx.x; i < I; i += TPB) xi[i] = 0.0;
     const double sy = SQUARE ? 1.0 : *sy_p;
     __syncthreads();
 
-    const int sub = threadIdx.x / R, lr = threadIdx.x % R, lane = threadIdx.x & 31;
-    double g = 0.0;
-    for (int t = sub; t < job.ntiles; t += (TPB2 / R)) {
-        const int64_t tile = (int64_t)job.tile0 + t;
-        const unsigned char* T = tiles + tile * TILE_BYTES;
-        RowRegs r;
-        load_row(T, lr, r);
-        const int64_t ri = tile * R + lr;
-        double yv = 1.0;
-        if (!SQUARE) {
-            if (PERM) {
-                const uint32_t pe = __ldcs(perm + ri);
-                yv = pe != PERM_PAD ? y[pe] * sy : 0.0;
-            } else {
-                yv = __ldcs(y + ri) * sy;
-            }
-        }
-#pragma unroll
-        for (int k = 0; k < NPAR; ++k) r.v[k] = SQUARE ? r.v[k] * r.v[k] : r.v[k] * yv;
-
-        // attitude: shared-memory accumulators
-        double* wa = xw + (r.a - job.a0);
-#pragma unroll
-        for (int ax = 0; ax < 3; ++ax)
-#pragma unroll
-            for (int j = 0; j < 4; ++j) atomicAdd(wa + ax * win + j, r.v[5 + 4 * ax + j]);
-        // instrumental
-#pragma unroll
-        for (int j = 0; j < 6; ++j) atomicAdd(xi + r.c[j], r.v[17 + j]);
-        // global
-        g += r.v[23];
-        // astrometric: segmented reduction, rows are star-sorted
-        const int32_t s_up = __shfl_up_sync(0xffffffffu, r.s, 1);
-        const bool head = lane == 0 || s_up != r.s;
-        const unsigned heads = __ballot_sync(0xffffffffu, head);
-        if (heads == 1u) {   // the whole warp lies inside one star
-#pragma unroll
-            for (int k = 0; k < 5; ++k) {
-                const double tsum = warp_sum(r.v[k]);
-                if (lane == 0 && tsum != 0.0) atomicAdd(x + 5 * (int64_t)r.s + k, tsum);
-            }
-        } else {
-            // segmented inclusive scan; the last lane of each segment holds its sum
-            const unsigned below = heads & ((2u << lane) - 1u);        // heads at or below me
-            const int seg_start = 31 - __clz(below);
-            const bool tail = lane == 31 || ((heads >> (lane + 1)) & 1u);
-#pragma unroll
-            for (int k = 0; k < 5; ++k) {
-                double vsum = r.v[k];
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const double up = __shfl_up_sync(0xffffffffu, vsum, o);
-                    if (lane - o >= seg_start) vsum += up;
-                }
-                if (tail && vsum != 0.0) atomicAdd(x + 5 * (int64_t)r.s + k, vsum);
-            }
-        }
-    }
-    // global column: one atomic per job
-    g = warp_sum(g);
-    if (lane == 0) red[threadIdx.x >> 5] = g;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double tsum = 0.0;
-#pragma unroll
-        for (int w = 0; w < TPB2 / 32; ++w) tsum += red[w];
-        if (tsum != 0.0) atomicAdd(x + 5 * S + 3 * D + I, tsum);
-    }
-    // flush the privatised accumulators
+    const int h = lane >> 4, j = lane & 15, jj = min(j, 11);
+    const int axo = (jj >> 2) * win + (jj & 3);
+    const bool lo12 = lane < 12, hi12 = lane >= 16 && lane < 28;
     double* xatt = x + 5 * S;
-    for (int i = threadIdx.x; i < 3 * win; i += TPB2) {
-        const double vacc = xw[i];
-        if (vacc != 0.0) {
-            const int ax = i / win, j = i - ax * win;
-            atomicAdd(xatt + ax * D + job.a0 + j, vacc);   // knot < D whenever vacc != 0
+    double g = 0.0;
+    for (;;) {
+        const int u = fetch_unit(counter, lane);
+        if (u >= n_units) break;
+        const Unit un = units[u];
+        __syncwarp();
+        for (int i = lane; i < 3 * win; i += 32) xw[i] = 0.0;
+        __syncwarp();
+        for (int t = 0; t < un.ntiles; ++t) {
+            const int64_t tile = (int64_t)un.tile0 + t;
+            TileRegs r;
+            load_tile(tiles + tile * TILE_BYTES, lane, r);
+            const int64_t ri = tile * R + lane;
+            double yv = 1.0;
+            if (!SQUARE) {
+                if (PERM) {
+                    const uint32_t pe = __ldcs(perm + ri);
+                    yv = pe != PERM_PAD ? y[pe] * sy : 0.0;
+                } else {
+                    yv = __ldcs(y + ri) * sy;
+                }
+            }
+            // attitude: rows 0-15 through lanes 0-11, rows 16-31 through
+            // lanes 16-27, one row at a time per half
+#pragma unroll
+            for (int qq = 0; qq < 16; ++qq) {
+                const int src = h * 16 + qq;
+                const uint32_t a = __shfl_sync(0xffffffffu, r.aoff, src);
+                const double yy = __shfl_sync(0xffffffffu, yv, src);
+                const double add = SQUARE ? r.at[qq] * r.at[qq] : r.at[qq] * yy;
+                double* pa = xw + a + axo;
+                if (lo12) *pa += add;
+                __syncwarp();
+                if (hi12) *pa += add;
+                __syncwarp();
+            }
+#pragma unroll
+            for (int k = 0; k < 5; ++k) r.as[k] = SQUARE ? r.as[k] * r.as[k] : r.as[k] * yv;
+#pragma unroll
+            for (int k = 0; k < 6; ++k) r.in[k] = SQUARE ? r.in[k] * r.in[k] : r.in[k] * yv;
+            // instrumental
+#pragma unroll
+            for (int k = 0; k < 6; ++k) atomicAdd(xi + r.c[k], r.in[k]);
+            // global
+            g += SQUARE ? r.gl * r.gl : r.gl * yv;
+            // astrometric: segmented reduction, rows are star-sorted
+            const int32_t s_up = __shfl_up_sync(0xffffffffu, r.s, 1);
+            const bool head = lane == 0 || s_up != r.s;
+            const unsigned heads = __ballot_sync(0xffffffffu, head);
+            if (heads == 1u) {   // the whole warp lies inside one star
+#pragma unroll
+                for (int k = 0; k < 5; ++k) {
+                    const double tsum = warp_sum(r.as[k]);
+                    if (lane == 0 && tsum != 0.0) atomicAdd(x + 5 * (int64_t)r.s + k, tsum);
+                }
+            } else {
+                // segmented inclusive scan; the last lane of each segment holds its sum
+                const unsigned below = heads & ((2u << lane) - 1u);        // heads at or below me
+                const int seg_start = 31 - __clz(below);
+                const bool tail = lane == 31 || ((heads >> (lane + 1)) & 1u);
+#pragma unroll
+                for (int k = 0; k < 5; ++k) {
+                    double vsum = r.as[k];
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const double up = __shfl_up_sync(0xffffffffu, vsum, o);
+                        if (lane - o >= seg_start) vsum += up;
+                    }
+                    if (tail && vsum != 0.0) atomicAdd(x + 5 * (int64_t)r.s + k, vsum);
+                }
+            }
+        }
+        // flush the unit's window
+        __syncwarp();
+        for (int i = lane; i < 3 * win; i += 32) {
+            const double vacc = xw[i];
+            if (vacc != 0.0) {
+                const int ax = i / win, k = i - ax * win;
+                atomicAdd(xatt + ax * D + un.a0 + k, vacc);   // knot < D whenever vacc != 0
+            }
         }
     }
+    // global column: one atomic per warp
+    g = warp_sum(g);
+    if (lane == 0 && g != 0.0) atomicAdd(x + 5 * S + 3 * D + I, g);
+    // flush the CTA's instrumental accumulators
+    __syncthreads();
     double* xins = x + 5 * S + 3 * D;
-    for (int i = threadIdx.x; i < I; i += TPB2) {
+    for (int i = threadIdx.x; i < I; i += TPB) {
         const double vacc = xi[i];
         if (vacc != 0.0) atomicAdd(xins + i, vacc);
     }
@@ -235,37 +289,52 @@ static int set_smem(K kernel, int bytes) {
     return GSR_OK;
 }
 
-static int aprod1_smem(const gsr_matrix* A) {
-    const int b = A->smem_bytes;
-    return b;   // measured: 2 CTAs x 1024 threads (64 warps) beat 1 CTA with a larger L1
+template <typename K>
+static int resident_ctas(K kernel, const gsr_matrix* A) {
+    int nb = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, TPB, A->smem_bytes) != cudaSuccess) {
+        cudaGetLastError();
+        nb = 1;
+    }
+    return nb < 1 ? 1 : nb;
 }
 
-int configure_product_kernels(const gsr_matrix* A) {
-    int b = aprod1_smem(A);
+int configure_product_kernels(gsr_matrix* A) {
+    const int b = A->smem_bytes;
     GSR_TRY(set_smem(k_aprod1<true, false>, b));
     GSR_TRY(set_smem(k_aprod1<false, false>, b));
     GSR_TRY(set_smem(k_aprod1<false, true>, b));
-    b = A->smem_bytes;
     GSR_TRY(set_smem(k_aprod2<false, false>, b));
     GSR_TRY(set_smem(k_aprod2<false, true>, b));
     GSR_TRY(set_smem(k_aprod2<true, false>, b));
+    A->grid1 = A->sm_count * resident_ctas(k_aprod1<true, false>, A);
+    A->grid2 = A->sm_count * resident_ctas(k_aprod2<false, false>, A);
+    const int need = (A->n_units + NWARP - 1) / NWARP;
+    if (A->grid1 > need) A->grid1 = need;
+    if (A->grid2 > need) A->grid2 = need;
+    return GSR_OK;
+}
+
+static int reset_counter(const gsr_matrix* A, cudaStream_t s) {
+    GSR_CUDA_TRY(cudaMemsetAsync(A->unit_counter, 0, sizeof(int), s));
     return GSR_OK;
 }
 
 int launch_aprod1(const gsr_matrix* A, const double* x, double* y, const double* ca,
                   double* partials, const int* stop, const uint32_t* perm, cudaStream_t s) {
-    if (A->n_jobs == 0) return GSR_OK;
+    if (A->n_units == 0) return GSR_OK;
     const int64_t S = A->dims.n_stars, D = A->dims.n_dfa;
     const int I = (int)A->dims.n_instr;
+    GSR_TRY(reset_counter(A, s));
     if (perm)
-        k_aprod1<false, true><<<A->n_jobs, TPB1, aprod1_smem(A), s>>>(A->tiles, A->jobs, x, y, ca, nullptr,
-                                                                    perm, S, D, I, A->win, stop);
+        k_aprod1<false, true><<<A->grid1, TPB, A->smem_bytes, s>>>(
+            A->tiles, A->units, A->n_units, A->unit_counter, x, y, ca, nullptr, perm, S, D, I, A->win, stop);
     else if (partials)
-        k_aprod1<true, false><<<A->n_jobs, TPB1, aprod1_smem(A), s>>>(A->tiles, A->jobs, x, y, ca, partials,
-                                                                    nullptr, S, D, I, A->win, stop);
+        k_aprod1<true, false><<<A->grid1, TPB, A->smem_bytes, s>>>(
+            A->tiles, A->units, A->n_units, A->unit_counter, x, y, ca, partials, nullptr, S, D, I, A->win, stop);
     else
-        k_aprod1<false, false><<<A->n_jobs, TPB1, aprod1_smem(A), s>>>(A->tiles, A->jobs, x, y, ca, nullptr,
-                                                                     nullptr, S, D, I, A->win, stop);
+        k_aprod1<false, false><<<A->grid1, TPB, A->smem_bytes, s>>>(
+            A->tiles, A->units, A->n_units, A->unit_counter, x, y, ca, nullptr, nullptr, S, D, I, A->win, stop);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;
@@ -273,25 +342,27 @@ int launch_aprod1(const gsr_matrix* A, const double* x, double* y, const double*
 
 int launch_aprod2(const gsr_matrix* A, const double* y, double* x, const double* sy,
                   const int* stop, const uint32_t* perm, cudaStream_t s) {
-    if (A->n_jobs == 0) return GSR_OK;
+    if (A->n_units == 0) return GSR_OK;
     const int64_t S = A->dims.n_stars, D = A->dims.n_dfa;
     const int I = (int)A->dims.n_instr;
+    GSR_TRY(reset_counter(A, s));
     if (perm)
-        k_aprod2<false, true><<<A->n_jobs, TPB2, A->smem_bytes, s>>>(A->tiles, A->jobs, y, x, sy, perm, S, D,
-                                                                    I, A->win, stop);
+        k_aprod2<false, true><<<A->grid2, TPB, A->smem_bytes, s>>>(
+            A->tiles, A->units, A->n_units, A->unit_counter, y, x, sy, perm, S, D, I, A->win, stop);
     else
-        k_aprod2<false, false><<<A->n_jobs, TPB2, A->smem_bytes, s>>>(A->tiles, A->jobs, y, x, sy, nullptr, S,
-                                                                     D, I, A->win, stop);
+        k_aprod2<false, false><<<A->grid2, TPB, A->smem_bytes, s>>>(
+            A->tiles, A->units, A->n_units, A->unit_counter, y, x, sy, nullptr, S, D, I, A->win, stop);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;
 }
 
 int launch_colsumsq(const gsr_matrix* A, double* q, cudaStream_t s) {
-    if (A->n_jobs == 0) return GSR_OK;
-    k_aprod2<true, false><<<A->n_jobs, TPB2, A->smem_bytes, s>>>(A->tiles, A->jobs, nullptr, q, nullptr,
-                                                                nullptr, A->dims.n_stars, A->dims.n_dfa,
-                                                                (int)A->dims.n_instr, A->win, nullptr);
+    if (A->n_units == 0) return GSR_OK;
+    GSR_TRY(reset_counter(A, s));
+    k_aprod2<true, false><<<A->grid2, TPB, A->smem_bytes, s>>>(
+        A->tiles, A->units, A->n_units, A->unit_counter, nullptr, q, nullptr, nullptr, A->dims.n_stars,
+        A->dims.n_dfa, (int)A->dims.n_instr, A->win, nullptr);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;

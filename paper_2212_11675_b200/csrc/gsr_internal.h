@@ -10,38 +10,66 @@
 namespace gsr {
 
 // ---- device layout ------------------------------------
-// Rows are stored in tiles of R rows; a tile is one contiguous record, plane-major:
-//   val[24][R] f64 | att[R] i32 | star[R] i32 | instr[6][R] i32     = 224*R bytes
-// so that lane r of a warp reads consecutive addresses in every plane (coalesced 256 B per
-// warp request) and a whole tile is one contiguous stream for the memory system.
+// Rows are stored in WARP TILES of R = 32 rows; a tile is one contiguous, 128-byte-aligned
+// record that one warp streams (lane r <-> row r of the tile):
+//   astro [5][32] f64   plane-major: lane r reads consecutive addresses, 256 B per request
+//   att   [16][2][12] f64  ROW-major and half-interleaved: record q holds the 12 attitude
+//         coefficients of row q and then those of row 16+q, so that lanes 0-11 (rows 0-15) and
+//         lanes 16-27 (rows 16-31) each fetch one coefficient of one row per request (192
+//         contiguous bytes) and end up owning a COLUMN of the 32x12 block: lane j holds
+//         coefficient j of 16 rows.  aprod2 then adds row after row into the window with 12
+//         lanes at 12 distinct addresses (plain read-modify-write, no atomics); aprod1 forms
+//         the 12 products per row the same way and transposes them back with 15 shuffles.
+//   instr [6][32] f64, glob [32] f64   plane-major
+//   star  [32] i32
+//   icol  [6][32] u16   instrumental columns (I <= 65535 is implied by the shared-memory plan)
+//   aoff  [32] u16      att_start - a0 of the unit (offset inside the warp's window)
+//   a0    i32           first knot of the window (same for every tile of a unit)
+//   60 bytes of padding                                                = 6784 B = 212 B/row
 //
 // INTERNAL ROW ORDER.  LSQR only ever touches the m-sized vectors through A and A^T, so the
 // solver is free to keep them in any row order.  Rows are ingested in segments of SEG rows;
-// inside a segment they are stably partitioned by ATTITUDE BIN (att_start / bin_width), which
-// keeps the star grouping inside every bin.  A "job" is a run of tiles of one (segment, bin):
-// every attitude column its rows touch lies in a window of bin_width+3 knots per axis, small
-// enough to live in shared memory together with the whole instrumental block.  perm[] maps
-// an internal row to the caller's row (0xFFFFFFFF for the zero padding rows that round every
-// bin up to whole tiles).
-constexpr int R = 256;                       // rows per tile
+// inside a segment they are stably partitioned by FINE ATTITUDE BIN (att_start / fw), which
+// keeps the star grouping inside every bin.  A "unit" is a run of tiles of one (segment, bin):
+// every attitude column its rows touch lies in a window of fw+3 knots per axis, a few KB that
+// ONE WARP keeps privately in shared memory.  Warps are autonomous: a persistent grid of CTAs
+// fetches units from a global counter, one unit per warp at a time; only the instrumental
+// block (I doubles) is shared by the warps of a CTA.  perm[] maps an internal row to the
+// caller's row (0xFFFFFFFF for the zero padding rows that round every bin up to whole tiles).
+constexpr int R = 32;                        // rows per tile (one warp)
 constexpr int NPAR = 24;
-constexpr int OFF_ATT = NPAR * R * 8;        // byte offsets inside a tile record
-constexpr int OFF_STAR = OFF_ATT + R * 4;
-constexpr int OFF_INSTR = OFF_STAR + R * 4;
-constexpr int TILE_BYTES = OFF_INSTR + 6 * R * 4;  // 57344
-static_assert(TILE_BYTES == 224 * R, "tile record is 224 bytes per row");
+constexpr int OFF_ASTRO = 0;                 // byte offsets inside a tile record
+constexpr int OFF_ATTV = 5 * R * 8;          // 1280
+constexpr int OFF_INSTRV = OFF_ATTV + 12 * R * 8;   // 4352
+constexpr int OFF_GLOBV = OFF_INSTRV + 6 * R * 8;   // 5888
+constexpr int OFF_STAR = OFF_GLOBV + R * 8;         // 6144
+constexpr int OFF_ICOL = OFF_STAR + R * 4;          // 6272
+constexpr int OFF_AOFF = OFF_ICOL + 6 * R * 2;      // 6656
+constexpr int OFF_A0 = OFF_AOFF + R * 2;            // 6720: i32 first knot of the tile's window
+constexpr int TILE_BYTES = 6784;                    // 53 * 128
+static_assert(OFF_A0 + 4 <= TILE_BYTES && TILE_BYTES % 128 == 0, "tile record");
+// byte offset of coefficient k (paper order) of row lr inside a tile record
+__host__ __device__ inline int val_offset(int k, int lr) {
+    if (k < 5) return OFF_ASTRO + (k * R + lr) * 8;
+    if (k < 17) return OFF_ATTV + (((lr & 15) * 2 + (lr >> 4)) * 12 + (k - 5)) * 8;
+    if (k < 23) return OFF_INSTRV + ((k - 17) * R + lr) * 8;
+    return OFF_GLOBV + lr * 8;
+}
 
 constexpr int64_t SEG = 1 << 22;             // rows per ingest segment
-constexpr int NBIN_MAX = 256;                // attitude bins
-constexpr int SMEM_BUDGET = 220 * 1024;      // bytes of shared memory a product CTA may use
-constexpr int ATT_WIN_BYTES = 64 * 1024;     // target size of the attitude window (3 axes)
-constexpr int JOB_TILES_MAX = 128;           // tiles per job (upper bound)
+constexpr int NBIN_MAX = 4096;               // fine attitude bins
+constexpr int NWARP = 16;                    // warps per product CTA
+constexpr int TPB = NWARP * 32;
+constexpr int SMEM_BUDGET = 224 * 1024;      // dynamic shared memory a product CTA may use
+constexpr int WIN_BYTES_MAX = 6 * 1024;      // per-warp attitude window, 3 axes
+constexpr int STAGE_BYTES = 0;               // per-warp scratch besides the window
+constexpr int UNIT_TILES_MAX = 128;          // tiles per unit (upper bound)
 constexpr uint32_t PERM_PAD = 0xFFFFFFFFu;
 
-struct Job {
-    int32_t tile0;    // first tile of the job
-    int32_t ntiles;   // tiles in the job
-    int32_t a0;       // first knot of the attitude window
+struct Unit {
+    int32_t tile0;    // first tile of the unit
+    int32_t ntiles;   // tiles in the unit
+    int32_t a0;       // first knot of the unit's attitude window
     int32_t pad_;
 };
 
@@ -68,7 +96,7 @@ struct Workspace {
     double* v = nullptr;        // [n]
     double* w = nullptr;        // [n]
     double* x = nullptr;        // [n]  iterate z of the (scaled) system
-    double* part_u = nullptr;   // [max(n_jobs, NB_N)] per-CTA partial sums of u_hat^2
+    double* part_u = nullptr;   // [max(n_units, NB_N)] per-unit partial sums of u_hat^2
     double* part_v = nullptr;   // [NB_N]
     double* part_w = nullptr;   // [NB_N]
     double* stage_m = nullptr;  // [m] staging for a host b
@@ -86,15 +114,18 @@ struct gsr_matrix {
     gsr_dims dims;
     int64_t n_cols, off_att, off_instr, off_glob;
     // layout
-    int nbins, bin_width, win;      // attitude bins; win = bin_width + 3 knots per axis
+    int nbins, bin_width, win;      // fine attitude bins; win = bin_width + 3 knots per axis
     int smem_bytes;                 // dynamic shared memory of the product kernels
+    int ctas_per_sm;                // resident product CTAs per SM the shared-memory plan allows
+    int grid1, grid2;               // persistent grids of aprod1 / aprod2
     int64_t tiles_cap, n_tiles;     // allocated / used tiles
     int64_t m_int;                  // n_tiles * R, length of internal-order vectors
     unsigned char* tiles;           // tiles_cap * TILE_BYTES
     uint32_t* perm;                 // [tiles_cap * R]
-    gsr::Job* jobs;                 // device copy of the job table
-    int n_jobs;
-    std::vector<gsr::Job>* jobs_host;
+    gsr::Unit* units;               // device copy of the unit table
+    int n_units;
+    std::vector<gsr::Unit>* units_host;
+    int* unit_counter;              // device: next unit to fetch (reset before every product)
     // ingest
     int64_t rows_appended;
     int64_t seg_fill, seg_cap;
@@ -142,8 +173,8 @@ void free_workspace(gsr_matrix* A);
 
 // product launchers (gsr_aprod.cu).  coef points to device doubles.  `perm` selects the row
 // order of the m-sized vector: nullptr = internal order (the solver), A->perm = caller order.
-//   aprod1: y[i] = (*ca) * y[i] + sum_k A[i,k] x[col];  if partials != nullptr, per-job sums
-//           of y_new^2 are written to partials[0..n_jobs).
+//   aprod1: y[i] = (*ca) * y[i] + sum_k A[i,k] x[col];  if partials != nullptr, per-unit sums
+//           of y_new^2 are written to partials[0..n_units).
 int launch_aprod1(const gsr_matrix* A, const double* x, double* y, const double* ca,
                   double* partials, const int* stop, const uint32_t* perm, cudaStream_t s);
 //   aprod2: x[col] += A[i,k] * (y[i] * (*sy))
@@ -151,6 +182,6 @@ int launch_aprod2(const gsr_matrix* A, const double* y, double* x, const double*
                   const int* stop, const uint32_t* perm, cudaStream_t s);
 //   column sums of squares (preconditioner): q[col] += A[i,k]^2
 int launch_colsumsq(const gsr_matrix* A, double* q, cudaStream_t s);
-int configure_product_kernels(const gsr_matrix* A);
+int configure_product_kernels(gsr_matrix* A);
 
 }  // namespace gsr

@@ -277,7 +277,7 @@ int ensure_workspace(gsr_matrix* A) {
     Workspace& W = A->ws;
     if (W.st) return GSR_OK;
     const size_t n8 = (size_t)A->n_cols * 8;
-    int64_t npu = A->n_jobs > NB_N ? A->n_jobs : NB_N;
+    int64_t npu = A->n_units > NB_N ? A->n_units : NB_N;
     GSR_TRY(dev_alloc(A, (void**)&W.u, (size_t)A->m_int * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.v, n8));
     GSR_TRY(dev_alloc(A, (void**)&W.w, n8));
@@ -312,7 +312,7 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
     const int64_t n = A->n_cols;
     // bidiagonalisation, first half: u_hat <- A v - (alpha/beta) u_hat ; partials of u_hat^2
     GSR_TRY(launch_aprod1(A, W.v, W.u, &W.st->ca, W.part_u, &W.st->stop, nullptr, s));
-    k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_jobs);
+    k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_units);
     // second half: v <- A^T (u_hat/beta) - beta v
     k_prescale<<<NB_N, TB_N, 0, s>>>(W.v, n, W.st);
     GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s));

@@ -39,20 +39,22 @@ void dev_free(gsr_matrix* A, void* p, size_t bytes) {
     A->device_bytes -= (int64_t)(bytes == 0 ? 8 : bytes);
 }
 
-// ---- segment partition: stable counting sort of the staged rows by attitude bin ----------
-// Pass 1: per block of 256 staged rows, rows per bin -> counts[bin * nblk + blk]; validation.
+// ---- segment partition: stable counting sort of the staged rows by fine attitude bin ------
+constexpr int BLK = 1024;   // staged rows per block of the partition kernels
+
+// Pass 1: per block of BLK staged rows, rows per bin -> counts[bin * nblk + blk]; validation.
 // Error bits: 1 star out of range, 2 star decreasing, 4 att_start out of range, 8 instr_col.
-__global__ void __launch_bounds__(256) k_seg_count(const int32_t* __restrict__ star,
+__global__ void __launch_bounds__(BLK) k_seg_count(const int32_t* __restrict__ star,
                                                    const int32_t* __restrict__ att,
                                                    const int32_t* __restrict__ instr, int64_t ns,
                                                    int64_t S, int64_t D, int64_t I, int bin_width,
                                                    int nbins, int nblk, int* __restrict__ counts,
                                                    const int* __restrict__ last_star,
                                                    int* __restrict__ err) {
-    __shared__ int hist[NBIN_MAX];
-    for (int b = threadIdx.x; b < nbins; b += 256) hist[b] = 0;
+    extern __shared__ int hist[];
+    for (int b = threadIdx.x; b < nbins; b += BLK) hist[b] = 0;
     __syncthreads();
-    const int64_t r = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    const int64_t r = (int64_t)blockIdx.x * BLK + threadIdx.x;
     if (r < ns) {
         int e = 0;
         const int32_t s = star[r], a = att[r];
@@ -71,7 +73,7 @@ __global__ void __launch_bounds__(256) k_seg_count(const int32_t* __restrict__ s
         atomicAdd(&hist[bin], 1);
     }
     __syncthreads();
-    for (int b = threadIdx.x; b < nbins; b += 256) counts[(int64_t)b * nblk + blockIdx.x] = hist[b];
+    for (int b = threadIdx.x; b < nbins; b += BLK) counts[(int64_t)b * nblk + blockIdx.x] = hist[b];
 }
 
 // Pass 2 (one CTA): exclusive scan of counts in (bin, block) order; every bin starts on a tile
@@ -81,74 +83,83 @@ __global__ void __launch_bounds__(256) k_seg_count(const int32_t* __restrict__ s
 __global__ void __launch_bounds__(1024) k_seg_scan(int* __restrict__ counts, int nbins, int nblk,
                                                    int* __restrict__ bin_info) {
     __shared__ int part[1024];
-    __shared__ int base_s;
+    __shared__ int wsum[32];
     int base = 0;
+    const int per = (nblk + 1023) / 1024;
+    const int i0 = threadIdx.x * per, i1 = min(i0 + per, nblk);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int b = 0; b < nbins; ++b) {
         int* c = counts + (int64_t)b * nblk;
-        const int per = (nblk + 1023) / 1024;
-        const int i0 = threadIdx.x * per, i1 = min(i0 + per, nblk);
         int s = 0;
         for (int i = i0; i < i1; ++i) s += c[i];
-        part[threadIdx.x] = s;
+        // exclusive scan of the 1024 per-thread sums
+        int incl = s;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int up = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += up;
+        }
+        if (lane == 31) wsum[warp] = incl;
         __syncthreads();
-        if (threadIdx.x == 0) {
-            int run = 0;
-            for (int t = 0; t < 1024; ++t) {
-                int v = part[t];
-                part[t] = run;
-                run += v;
+        if (warp == 0) {
+            int w = wsum[lane], wi = w;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int up = __shfl_up_sync(0xffffffffu, wi, o);
+                if (lane >= o) wi += up;
             }
-            bin_info[b] = run;
-            bin_info[nbins + b] = base;
-            base_s = base + ((run + R - 1) / R) * R;
+            wsum[lane] = wi - w;           // exclusive warp offsets
+            if (lane == 31) part[0] = wi;  // total rows of the bin
         }
         __syncthreads();
-        int off = base + part[threadIdx.x];
+        const int run = part[0];
+        int off = base + wsum[warp] + incl - s;
         for (int i = i0; i < i1; ++i) {
-            int v = c[i];
+            const int v = c[i];
             c[i] = off;
             off += v;
         }
-        base = base_s;
+        if (threadIdx.x == 0) {
+            bin_info[b] = run;
+            bin_info[nbins + b] = base;
+        }
+        base += ((run + R - 1) / R) * R;
         __syncthreads();
     }
     if (threadIdx.x == 0) bin_info[2 * nbins] = base;
 }
 
 // Pass 3: stable scatter of the staged rows into tile records (internal order) + perm.
-__global__ void __launch_bounds__(256) k_seg_scatter(
+__global__ void __launch_bounds__(BLK) k_seg_scatter(
     unsigned char* __restrict__ tiles, uint32_t* __restrict__ perm, int64_t row_base_int,
     int64_t row_base_ext, const int32_t* __restrict__ star, const int32_t* __restrict__ att,
     const int32_t* __restrict__ instr, const double* __restrict__ vals, int64_t ns, int64_t D,
-    int bin_width, int nbins, int nblk, const int* __restrict__ offs) {
-    __shared__ int wcnt[8][NBIN_MAX + 1];
-    for (int i = threadIdx.x; i < 8 * (NBIN_MAX + 1); i += 256) (&wcnt[0][0])[i] = 0;
-    __syncthreads();
-    const int64_t r = (int64_t)blockIdx.x * 256 + threadIdx.x;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    int bin = NBIN_MAX;   // inactive lanes share an extra bucket
+    int bin_width, int nblk, const int* __restrict__ offs) {
+    __shared__ int sbin[BLK];
+    const int64_t r = (int64_t)blockIdx.x * BLK + threadIdx.x;
+    int bin = -1;
     int32_t a = 0;
     if (r < ns) {
         a = att[r];
         bin = (a >= 0 && a <= D - 4) ? a / bin_width : 0;
     }
-    const unsigned peers = __match_any_sync(0xffffffffu, bin);
-    const int rank_w = __popc(peers & ((1u << lane) - 1u));
-    if (rank_w == 0) wcnt[warp][bin] = __popc(peers);
+    sbin[threadIdx.x] = bin;
     __syncthreads();
     if (r >= ns) return;
-    int rank = rank_w;
-    for (int w = 0; w < warp; ++w) rank += wcnt[w][bin];
+    int rank = 0;   // rows of my bin that precede me in this block (stable)
+    for (int i = 0; i < (int)threadIdx.x; ++i) rank += sbin[i] == bin;
     const int64_t dst = row_base_int + offs[(int64_t)bin * nblk + blockIdx.x] + rank;
     unsigned char* T = tiles + (dst / R) * (int64_t)TILE_BYTES;
     const int lr = (int)(dst % R);
     perm[dst] = (uint32_t)(row_base_ext + r);
     ((int32_t*)(T + OFF_STAR))[lr] = star[r];
-    ((int32_t*)(T + OFF_ATT))[lr] = a;
+    const int a0 = bin * bin_width;
+    ((uint16_t*)(T + OFF_AOFF))[lr] = (uint16_t)(bin == 0 && (a < 0 || a > D - 4) ? 0 : a - a0);
+    *(int32_t*)(T + OFF_A0) = a0;   // same value from every row of the tile
 #pragma unroll
-    for (int j = 0; j < 6; ++j) ((int32_t*)(T + OFF_INSTR + j * R * 4))[lr] = instr[6 * r + j];
+    for (int j = 0; j < 6; ++j) ((uint16_t*)(T + OFF_ICOL))[j * R + lr] = (uint16_t)instr[6 * r + j];
 #pragma unroll
-    for (int k = 0; k < NPAR; ++k) ((double*)(T + k * R * 8))[lr] = vals[NPAR * r + k];
+    for (int k = 0; k < NPAR; ++k) *(double*)(T + val_offset(k, lr)) = vals[NPAR * r + k];
 }
 
 __global__ void k_save_last_star(const int32_t* __restrict__ star, int64_t ns, int* last_star) {
@@ -156,25 +167,19 @@ __global__ void k_save_last_star(const int32_t* __restrict__ star, int64_t ns, i
 }
 
 // Padding rows (they round every bin up to whole tiles and trail the bin's real rows): zero
-// coefficients (tiles are memset to 0); att = the window's first knot and star = the star of
-// the last real row of the tile, so that they open no new window and no new star segment.
-__global__ void __launch_bounds__(R) k_fix_padding(unsigned char* __restrict__ tiles,
-                                                   const uint32_t* __restrict__ perm,
-                                                   const Job* __restrict__ jobs, int n_jobs) {
-    const int j = blockIdx.x;
-    if (j >= n_jobs) return;
-    const Job job = jobs[j];
-    for (int t = 0; t < job.ntiles; ++t) {
-        unsigned char* T = tiles + (int64_t)(job.tile0 + t) * TILE_BYTES;
-        const int64_t row = (int64_t)(job.tile0 + t) * R + threadIdx.x;
-        const bool real = perm[row] != PERM_PAD;
-        const int nreal = __syncthreads_count(real);
-        if (!real) {
-            ((int32_t*)(T + OFF_ATT))[threadIdx.x] = job.a0;
-            ((int32_t*)(T + OFF_STAR))[threadIdx.x] = nreal > 0 ? ((const int32_t*)(T + OFF_STAR))[nreal - 1] : 0;
-        }
-        __syncthreads();
-    }
+// coefficients, window offset 0 and instrumental column 0 (tiles are memset to 0); star = the
+// star of the last real row of the tile, so that they open no new star segment.
+// One warp per tile.
+__global__ void __launch_bounds__(256) k_fix_padding(unsigned char* __restrict__ tiles,
+                                                     const uint32_t* __restrict__ perm,
+                                                     int64_t n_tiles) {
+    const int64_t t = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (t >= n_tiles) return;
+    const int lane = threadIdx.x & 31;
+    unsigned char* T = tiles + t * TILE_BYTES;
+    const bool real = perm[t * R + lane] != PERM_PAD;
+    const int nreal = __popc(__ballot_sync(0xffffffffu, real));
+    if (!real) ((int32_t*)(T + OFF_STAR))[lane] = nreal > 0 ? ((const int32_t*)(T + OFF_STAR))[nreal - 1] : 0;
 }
 
 // Caller-order dump of rows [row0, row0+nrows): every internal row whose caller row falls in
@@ -191,16 +196,16 @@ __global__ void k_expand_rows(const unsigned char* __restrict__ tiles, const uin
     const unsigned char* T = tiles + (ri / R) * (int64_t)TILE_BYTES;
     const int lr = (int)(ri % R);
     const int64_t s = ((const int32_t*)(T + OFF_STAR))[lr];
-    const int64_t a = ((const int32_t*)(T + OFF_ATT))[lr];
+    const int64_t a = (int64_t)(*(const int32_t*)(T + OFF_A0)) + ((const uint16_t*)(T + OFF_AOFF))[lr];
     const int64_t off_att = 5 * S, off_instr = off_att + 3 * D, off_glob = off_instr + I;
     for (int k = 0; k < NPAR; ++k) {
         int64_t c;
         if (k < 5) c = 5 * s + k;
         else if (k < 17) c = off_att + ((k - 5) / 4) * D + a + (k - 5) % 4;
-        else if (k < 23) c = off_instr + ((const int32_t*)(T + OFF_INSTR + (k - 17) * R * 4))[lr];
+        else if (k < 23) c = off_instr + ((const uint16_t*)(T + OFF_ICOL))[(k - 17) * R + lr];
         else c = off_glob;
         cols[NPAR * r + k] = c;
-        vals[NPAR * r + k] = ((const double*)(T + k * R * 8))[lr];
+        vals[NPAR * r + k] = *(const double*)(T + val_offset(k, lr));
     }
 }
 
@@ -212,29 +217,31 @@ __global__ void k_make_p(double* __restrict__ p, int64_t n) {
     p[j] = q > 0.0 ? 1.0 / sqrt(q) : 1.0;
 }
 
-// values[i,k] *= p[col(i,k)] in place, one thread per row of a tile.
-__global__ void __launch_bounds__(R) k_scale_values(unsigned char* __restrict__ tiles,
-                                                    const double* __restrict__ p, int64_t S,
-                                                    int64_t D, int64_t I) {
-    unsigned char* T = tiles + (int64_t)blockIdx.x * TILE_BYTES;
-    const int lr = threadIdx.x;
+// values[i,k] *= p[col(i,k)] in place, one thread per row (8 tiles per CTA).
+__global__ void __launch_bounds__(256) k_scale_values(unsigned char* __restrict__ tiles,
+                                                      int64_t n_tiles, const double* __restrict__ p,
+                                                      int64_t S, int64_t D, int64_t I) {
+    const int64_t t = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (t >= n_tiles) return;
+    unsigned char* T = tiles + t * TILE_BYTES;
+    const int lr = threadIdx.x & 31;
     const int64_t s = ((const int32_t*)(T + OFF_STAR))[lr];
-    const int64_t a = ((const int32_t*)(T + OFF_ATT))[lr];
+    const int64_t a = (int64_t)(*(const int32_t*)(T + OFF_A0)) + ((const uint16_t*)(T + OFF_AOFF))[lr];
     const double* pa = p + 5 * s;
     const double* pt = p + 5 * S + a;
     const double* pi = p + 5 * S + 3 * D;
 #pragma unroll
-    for (int k = 0; k < 5; ++k) ((double*)(T + k * R * 8))[lr] *= pa[k];
+    for (int k = 0; k < 5; ++k) *(double*)(T + val_offset(k, lr)) *= pa[k];
 #pragma unroll
     for (int ax = 0; ax < 3; ++ax)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) ((double*)(T + (5 + 4 * ax + j) * R * 8))[lr] *= pt[ax * D + j];
+        for (int j = 0; j < 4; ++j) *(double*)(T + val_offset(5 + 4 * ax + j, lr)) *= pt[ax * D + j];
 #pragma unroll
     for (int j = 0; j < 6; ++j) {
-        int32_t c = ((const int32_t*)(T + OFF_INSTR + j * R * 4))[lr];
-        ((double*)(T + (17 + j) * R * 8))[lr] *= pi[c];
+        const int c = ((const uint16_t*)(T + OFF_ICOL))[j * R + lr];
+        *(double*)(T + val_offset(17 + j, lr)) *= pi[c];
     }
-    ((double*)(T + 23 * R * 8))[lr] *= pi[I];
+    *(double*)(T + val_offset(23, lr)) *= pi[I];
 }
 
 }  // namespace gsr
@@ -244,15 +251,16 @@ using namespace gsr;
 static int flush_segment(gsr_matrix* A) {
     const int64_t ns = A->seg_fill;
     if (ns == 0) return GSR_OK;
-    const int nblk = (int)((ns + 255) / 256);
+    const int nblk = (int)((ns + BLK - 1) / BLK);
     cudaStream_t s = A->stream;
-    k_seg_count<<<nblk, 256, 0, s>>>(A->st_star, A->st_att, A->st_instr, ns, A->dims.n_stars,
-                                     A->dims.n_dfa, A->dims.n_instr, A->bin_width, A->nbins, nblk,
-                                     A->seg_counts, A->last_star, A->err);
+    k_seg_count<<<nblk, BLK, A->nbins * sizeof(int), s>>>(A->st_star, A->st_att, A->st_instr, ns,
+                                                        A->dims.n_stars, A->dims.n_dfa, A->dims.n_instr,
+                                                        A->bin_width, A->nbins, nblk, A->seg_counts,
+                                                        A->last_star, A->err);
     k_seg_scan<<<1, 1024, 0, s>>>(A->seg_counts, A->nbins, nblk, A->seg_bin_rows);
-    k_seg_scatter<<<nblk, 256, 0, s>>>(A->tiles, A->perm, A->n_tiles * R, A->rows_appended - ns,
+    k_seg_scatter<<<nblk, BLK, 0, s>>>(A->tiles, A->perm, A->n_tiles * R, A->rows_appended - ns,
                                        A->st_star, A->st_att, A->st_instr, A->st_vals, ns,
-                                       A->dims.n_dfa, A->bin_width, A->nbins, nblk, A->seg_counts);
+                                       A->dims.n_dfa, A->bin_width, nblk, A->seg_counts);
     k_save_last_star<<<1, 1, 0, s>>>(A->st_star, ns, A->last_star);
     count_launch(4);
     GSR_CUDA_TRY(cudaGetLastError());
@@ -260,23 +268,25 @@ static int flush_segment(gsr_matrix* A) {
     GSR_CUDA_TRY(cudaMemcpyAsync(info.data(), A->seg_bin_rows, info.size() * sizeof(int),
                                  cudaMemcpyDeviceToHost, s));
     GSR_CUDA_TRY(cudaStreamSynchronize(s));
-    // job table: runs of at most job_tiles tiles inside one (segment, bin)
+    // unit table: runs of at most unit_tiles tiles inside one (segment, bin); sized so that
+    // every resident warp gets several units (dynamic fetch balances the rest)
     const int64_t est_tiles = (A->dims.n_rows + R - 1) / R;
-    int64_t job_tiles = (est_tiles + (int64_t)A->sm_count * 16 - 1) / ((int64_t)A->sm_count * 16);
-    if (job_tiles < 1) job_tiles = 1;
-    if (job_tiles > JOB_TILES_MAX) job_tiles = JOB_TILES_MAX;
+    const int64_t warps = (int64_t)A->sm_count * A->ctas_per_sm * NWARP;
+    int64_t unit_tiles = est_tiles / (warps * 8);
+    if (unit_tiles < 4) unit_tiles = 4;
+    if (unit_tiles > UNIT_TILES_MAX) unit_tiles = UNIT_TILES_MAX;
     for (int b = 0; b < A->nbins; ++b) {
         const int rows = info[b];
         if (rows == 0) continue;
         const int64_t t0 = A->n_tiles + info[A->nbins + b] / R;
         const int64_t nt = (rows + R - 1) / R;
-        for (int64_t t = 0; t < nt; t += job_tiles) {
-            Job j;
-            j.tile0 = (int32_t)(t0 + t);
-            j.ntiles = (int32_t)(nt - t < job_tiles ? nt - t : job_tiles);
-            j.a0 = b * A->bin_width;
-            j.pad_ = 0;
-            A->jobs_host->push_back(j);
+        for (int64_t t = 0; t < nt; t += unit_tiles) {
+            Unit u;
+            u.tile0 = (int32_t)(t0 + t);
+            u.ntiles = (int32_t)(nt - t < unit_tiles ? nt - t : unit_tiles);
+            u.a0 = b * A->bin_width;
+            u.pad_ = 0;
+            A->units_host->push_back(u);
         }
     }
     A->n_tiles += info[2 * A->nbins] / R;
@@ -292,7 +302,7 @@ static void free_staging(gsr_matrix* A) {
     dev_free(A, A->st_instr, c * 24); A->st_instr = nullptr;
     dev_free(A, A->st_vals, c * 192); A->st_vals = nullptr;
     if (A->seg_counts) {
-        const size_t nblk = (c + 255) / 256;
+        const size_t nblk = (c + BLK - 1) / BLK;
         dev_free(A, A->seg_counts, (size_t)A->nbins * nblk * 4);
         A->seg_counts = nullptr;
     }
@@ -322,19 +332,19 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
         return GSR_EINVAL;
     const int64_t n = 5 * d->n_stars + 3 * d->n_dfa + d->n_instr + 1;
     if (n >= (int64_t)1 << 31 || d->n_rows >= (int64_t)0xFFFFFFF0) return GSR_EINVAL;
-    // shared-memory plan of the product kernels: whole instrumental block + one attitude window
-    const int64_t instr_bytes = d->n_instr * 8;
-    if (instr_bytes > SMEM_BUDGET - 24 * 1024) return GSR_EUNSUPPORTED;
-    int64_t att_budget = ATT_WIN_BYTES;
-    const int64_t half = 110 * 1024;   // two CTAs per SM when everything fits in 110 KB
-    if (instr_bytes + 16 * 1024 <= half) att_budget = att_budget < half - instr_bytes ? att_budget : half - instr_bytes;
-    else if (SMEM_BUDGET - instr_bytes < att_budget) att_budget = SMEM_BUDGET - instr_bytes;
+    // shared-memory plan of the product kernels: the whole instrumental block, shared by the
+    // warps of a CTA, + one private attitude window of `win` knots x 3 axes per warp
+    const int64_t instr_bytes = (d->n_instr + 1) / 2 * 16;
+    if (d->n_instr > 65535 || instr_bytes > SMEM_BUDGET - NWARP * 24 * 4) return GSR_EUNSUPPORTED;
+    int64_t win_bytes = (SMEM_BUDGET - instr_bytes) / NWARP;
+    if (win_bytes > WIN_BYTES_MAX) win_bytes = WIN_BYTES_MAX;
     const int64_t n_start = d->n_dfa - 3;
-    int64_t bw_max = att_budget / 24 - 3;
+    const int64_t bw_max = win_bytes / 24 - 3;
     if (bw_max < 1) return GSR_EUNSUPPORTED;
     const int64_t nbins = (n_start + bw_max - 1) / bw_max;
     if (nbins > NBIN_MAX) return GSR_EUNSUPPORTED;
     const int64_t bw = (n_start + nbins - 1) / nbins;
+    const int64_t smem_bytes = instr_bytes + NWARP * 3 * (bw + 3) * 8;
 
     int dev = 0;
     cudaDeviceProp prop;
@@ -345,7 +355,7 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
     if (!A) return GSR_ENOMEM;
     memset((void*)A, 0, sizeof(*A));
     new (&A->ws) Workspace();
-    A->jobs_host = new (std::nothrow) std::vector<Job>();
+    A->units_host = new (std::nothrow) std::vector<Unit>();
     A->dims = *d;
     A->n_cols = n;
     A->off_att = 5 * d->n_stars;
@@ -354,13 +364,14 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
     A->nbins = (int)nbins;
     A->bin_width = (int)bw;
     A->win = (int)bw + 3;
-    A->smem_bytes = (int)((3 * (bw + 3) + d->n_instr + 2) * 8);
+    A->smem_bytes = (int)smem_bytes;
+    A->ctas_per_sm = 2 * (smem_bytes + 2048) <= 227 * 1024 ? 2 : 1;
     A->stream = (cudaStream_t)stream;
     A->sm_count = prop.multiProcessorCount;
     A->seg_cap = d->n_rows < SEG ? (d->n_rows > 0 ? d->n_rows : 1) : SEG;
     const int64_t n_seg = (d->n_rows + SEG - 1) / SEG;
     A->tiles_cap = (d->n_rows + R - 1) / R + n_seg * nbins + 1;
-    const size_t c = (size_t)A->seg_cap, nblk = (c + 255) / 256;
+    const size_t c = (size_t)A->seg_cap, nblk = (c + BLK - 1) / BLK;
     int rc = dev_alloc(A, (void**)&A->tiles, (size_t)A->tiles_cap * TILE_BYTES);
     if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->perm, (size_t)A->tiles_cap * R * 4);
     if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->st_star, c * 4);
@@ -372,7 +383,8 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
     if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->last_star, 4);
     if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->err, sizeof(int));
     if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->coef_one, 2 * sizeof(double));
-    if (rc != GSR_OK || !A->jobs_host) {
+    if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->unit_counter, sizeof(int));
+    if (rc != GSR_OK || !A->units_host) {
         gsr_matrix_destroy(A);
         return rc != GSR_OK ? rc : GSR_ENOMEM;
     }
@@ -428,13 +440,13 @@ int gsr_matrix_finalize(gsr_matrix* A) {
     GSR_CUDA_TRY(cudaStreamSynchronize(A->stream));
     free_staging(A);
     if (err != 0) return GSR_EINVAL;
-    A->n_jobs = (int)A->jobs_host->size();
+    A->n_units = (int)A->units_host->size();
     A->m_int = A->n_tiles * R;
-    GSR_TRY(dev_alloc(A, (void**)&A->jobs, (size_t)(A->n_jobs > 0 ? A->n_jobs : 1) * sizeof(Job)));
-    if (A->n_jobs > 0) {
-        GSR_CUDA_TRY(cudaMemcpyAsync(A->jobs, A->jobs_host->data(), (size_t)A->n_jobs * sizeof(Job),
+    GSR_TRY(dev_alloc(A, (void**)&A->units, (size_t)(A->n_units > 0 ? A->n_units : 1) * sizeof(Unit)));
+    if (A->n_units > 0) {
+        GSR_CUDA_TRY(cudaMemcpyAsync(A->units, A->units_host->data(), (size_t)A->n_units * sizeof(Unit),
                                      cudaMemcpyHostToDevice, A->stream));
-        k_fix_padding<<<A->n_jobs, R, 0, A->stream>>>(A->tiles, A->perm, A->jobs, A->n_jobs);
+        k_fix_padding<<<(unsigned)((A->n_tiles + 7) / 8), 256, 0, A->stream>>>(A->tiles, A->perm, A->n_tiles);
         count_launch();
         GSR_CUDA_TRY(cudaGetLastError());
     }
@@ -469,14 +481,15 @@ int gsr_matrix_destroy(gsr_matrix* A) {
     free_staging(A);
     cudaFree(A->tiles);
     cudaFree(A->perm);
-    cudaFree(A->jobs);
+    cudaFree(A->units);
+    cudaFree(A->unit_counter);
     cudaFree(A->seg_bin_rows);
     cudaFree(A->last_star);
     cudaFree(A->p);
     cudaFree(A->err);
     cudaFree(A->coef_one);
     cudaGetLastError();
-    delete A->jobs_host;
+    delete A->units_host;
     delete A;
     return GSR_OK;
 }
@@ -540,8 +553,8 @@ int gsr_precondition(gsr_matrix* A, double* p_out, gsr_stream stream) {
     k_make_p<<<(unsigned)((A->n_cols + 255) / 256), 256, 0, s>>>(A->p, A->n_cols);
     count_launch();
     if (A->n_tiles > 0) {
-        k_scale_values<<<(unsigned)A->n_tiles, R, 0, s>>>(A->tiles, A->p, A->dims.n_stars,
-                                                          A->dims.n_dfa, A->dims.n_instr);
+        k_scale_values<<<(unsigned)((A->n_tiles + 7) / 8), 256, 0, s>>>(
+            A->tiles, A->n_tiles, A->p, A->dims.n_stars, A->dims.n_dfa, A->dims.n_instr);
         count_launch();
     }
     GSR_CUDA_TRY(cudaGetLastError());
