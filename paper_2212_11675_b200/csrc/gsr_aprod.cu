@@ -27,16 +27,22 @@ __device__ __forceinline__ double warp_sum(double v) {
     return v;
 }
 
-struct TileRegs {
-    double as[5], in[6], gl;   // lane r: coefficients of row r
+// A tile is consumed in two phases so that the loads of one phase are in flight while the
+// other phase computes (software pipeline, no extra registers):
+//   phase A: the attitude block (16 coefficients per lane) + window offsets
+//   phase B: astrometric, instrumental and global coefficients + star and column indices
+struct RegsA {
     double at[16];             // lane (h, j): attitude coefficient min(j, 11) of rows 16h .. 16h+15
+    uint32_t aoff;             // lane r: att_start - a0 of row r
+};
+struct RegsB {
+    double as[5], in[6], gl;   // lane r: coefficients of row r
     int32_t s;
-    uint32_t aoff;
     uint32_t c[6];
 };
 
-// Streaming loads of one tile, all issued back to back (volatile asm keeps them together and
-// ahead of their first use, so every lane has ~340 bytes in flight).
+// Streaming loads, all of a phase issued back to back (volatile asm keeps them together and
+// ahead of their first use).
 __device__ __forceinline__ double ld_stream_f64(const void* p) {
     double v;
     asm volatile("ld.global.cs.f64 %0, [%1];" : "=d"(v) : "l"(p));
@@ -47,21 +53,28 @@ __device__ __forceinline__ int32_t ld_stream_s32(const void* p) {
     asm volatile("ld.global.cs.s32 %0, [%1];" : "=r"(v) : "l"(p));
     return v;
 }
+__device__ __forceinline__ uint32_t ld_stream_u32(const void* p) {
+    uint32_t v;
+    asm volatile("ld.global.cs.u32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
 __device__ __forceinline__ uint32_t ld_stream_u16(const void* p) {
     uint16_t v;
     asm volatile("ld.global.cs.u16 %0, [%1];" : "=h"(v) : "l"(p));
     return v;
 }
-__device__ __forceinline__ void load_tile(const unsigned char* __restrict__ T, int lane, TileRegs& r) {
-    r.s = ld_stream_s32(T + OFF_STAR + lane * 4);
+__device__ __forceinline__ void load_A(const unsigned char* __restrict__ T, int lane, RegsA& r) {
     r.aoff = ld_stream_u16(T + OFF_AOFF + lane * 2);
+    const int h = lane >> 4, jj = min(lane & 15, 11);
+#pragma unroll
+    for (int q = 0; q < 16; ++q) r.at[q] = ld_stream_f64(T + OFF_ATTV + ((q * 2 + h) * 12 + jj) * 8);
+}
+__device__ __forceinline__ void load_B(const unsigned char* __restrict__ T, int lane, RegsB& r) {
+    r.s = ld_stream_s32(T + OFF_STAR + lane * 4);
 #pragma unroll
     for (int j = 0; j < 6; ++j) r.c[j] = ld_stream_u16(T + OFF_ICOL + (j * R + lane) * 2);
 #pragma unroll
     for (int k = 0; k < 5; ++k) r.as[k] = ld_stream_f64(T + OFF_ASTRO + (k * R + lane) * 8);
-    const int h = lane >> 4, jj = min(lane & 15, 11);
-#pragma unroll
-    for (int q = 0; q < 16; ++q) r.at[q] = ld_stream_f64(T + OFF_ATTV + ((q * 2 + h) * 12 + jj) * 8);
 #pragma unroll
     for (int j = 0; j < 6; ++j) r.in[j] = ld_stream_f64(T + OFF_INSTRV + (j * R + lane) * 8);
     r.gl = ld_stream_f64(T + OFF_GLOBV + lane * 8);
@@ -82,13 +95,13 @@ __global__ void __launch_bounds__(TPB) k_aprod1(const unsigned char* __restrict_
                                                const double* __restrict__ ca_p,
                                                double* __restrict__ partials,
                                                const uint32_t* __restrict__ perm, int64_t S,
-                                               int64_t D, int I, int win,
+                                               int64_t D, int I, int win, int ws,
                                                const int* __restrict__ stop) {
     if (stop && *stop) return;
     extern __shared__ double sm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double* xi = sm;
-    double* xw = sm + ((I + 1) & ~1) + warp * 3 * win;
+    double* xw = sm + ((I + 1) & ~1) + warp * 3 * ws;
     const double* xatt = x + 5 * S;
     const double* xins = x + 5 * S + 3 * D;
     for (int i = threadIdx.x; i < I; i += TPB) xi[i] = __ldg(xins + i);
@@ -97,7 +110,7 @@ __global__ void __launch_bounds__(TPB) k_aprod1(const unsigned char* __restrict_
     __syncthreads();
 
     const int h = lane >> 4, j = lane & 15, jj = min(j, 11);
-    const int axo = (jj >> 2) * win + (jj & 3);   // my coefficient's column, relative to aoff
+    const int axo = (jj >> 2) * ws + (jj & 3);   // my coefficient's column, relative to aoff
     const bool att_lane = j < 12;
     for (;;) {
         const int u = fetch_unit(counter, lane);
@@ -107,15 +120,17 @@ __global__ void __launch_bounds__(TPB) k_aprod1(const unsigned char* __restrict_
         for (int i = lane; i < 3 * win; i += 32) {
             const int ax = i / win, k = i - ax * win;
             const int64_t knot = (int64_t)un.a0 + k;
-            xw[i] = knot < D ? __ldg(xatt + ax * D + knot) : 0.0;
+            xw[ax * ws + k] = knot < D ? __ldg(xatt + ax * D + knot) : 0.0;
         }
         __syncwarp();
         double q = 0.0;
-        for (int t = 0; t < un.ntiles; ++t) {
-            const int64_t tile = (int64_t)un.tile0 + t;
-            TileRegs r;
-            load_tile(tiles + tile * TILE_BYTES, lane, r);
-            const int64_t ri = tile * R + lane;
+        const unsigned char* T = tiles + (int64_t)un.tile0 * TILE_BYTES;
+        RegsA ra;
+        load_A(T, lane, ra);
+        for (int t = 0; t < un.ntiles; ++t, T += TILE_BYTES) {
+            RegsB r;
+            load_B(T, lane, r);
+            const int64_t ri = ((int64_t)un.tile0 + t) * R + lane;
             int64_t ry = ri;
             bool live = true;
             if (PERM) {
@@ -123,13 +138,13 @@ __global__ void __launch_bounds__(TPB) k_aprod1(const unsigned char* __restrict_
                 live = pe != PERM_PAD;
                 ry = pe;
             }
-            const double yold = live ? y[ry] : 0.0;
-            // attitude: 12 lanes per row, products transposed back by a butterfly
+            const double yold = live ? __ldcs(y + ry) : 0.0;
+            // phase A -- attitude: 12 lanes per row, products transposed back by a butterfly
             double p[16];
 #pragma unroll
             for (int qq = 0; qq < 16; ++qq) {
-                const uint32_t a = __shfl_sync(0xffffffffu, r.aoff, h * 16 + qq);
-                const double pv = r.at[qq] * xw[a + axo];
+                const uint32_t a = __shfl_sync(0xffffffffu, ra.aoff, h * 16 + qq);
+                const double pv = ra.at[qq] * xw[a + axo];
                 p[qq] = att_lane ? pv : 0.0;
             }
 #pragma unroll
@@ -143,6 +158,8 @@ __global__ void __launch_bounds__(TPB) k_aprod1(const unsigned char* __restrict_
                 }
             }
             double sum = p[0];   // lane (h, j) now holds the attitude part of row 16h + j
+            if (t + 1 < un.ntiles) load_A(T + TILE_BYTES, lane, ra);   // in flight during phase B
+            // phase B
             const double* xa = x + 5 * (int64_t)r.s;
 #pragma unroll
             for (int k = 0; k < 5; ++k) sum = fma(r.as[k], __ldg(xa + k), sum);
@@ -174,19 +191,19 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
                                                const double* __restrict__ y, double* __restrict__ x,
                                                const double* __restrict__ sy_p,
                                                const uint32_t* __restrict__ perm, int64_t S,
-                                               int64_t D, int I, int win,
+                                               int64_t D, int I, int win, int ws,
                                                const int* __restrict__ stop) {
     if (stop && *stop) return;
     extern __shared__ double sm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double* xi = sm;
-    double* xw = sm + ((I + 1) & ~1) + warp * 3 * win;
+    double* xw = sm + ((I + 1) & ~1) + warp * 3 * ws;
     for (int i = threadIdx.x; i < I; i += TPB) xi[i] = 0.0;
     const double sy = SQUARE ? 1.0 : *sy_p;
     __syncthreads();
 
     const int h = lane >> 4, j = lane & 15, jj = min(j, 11);
-    const int axo = (jj >> 2) * win + (jj & 3);
+    const int axo = (jj >> 2) * ws + (jj & 3);
     const bool lo12 = lane < 12, hi12 = lane >= 16 && lane < 28;
     double* xatt = x + 5 * S;
     double g = 0.0;
@@ -195,13 +212,15 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
         if (u >= n_units) break;
         const Unit un = units[u];
         __syncwarp();
-        for (int i = lane; i < 3 * win; i += 32) xw[i] = 0.0;
+        for (int i = lane; i < 3 * ws; i += 32) xw[i] = 0.0;
         __syncwarp();
-        for (int t = 0; t < un.ntiles; ++t) {
-            const int64_t tile = (int64_t)un.tile0 + t;
-            TileRegs r;
-            load_tile(tiles + tile * TILE_BYTES, lane, r);
-            const int64_t ri = tile * R + lane;
+        const unsigned char* T = tiles + (int64_t)un.tile0 * TILE_BYTES;
+        RegsA ra;
+        load_A(T, lane, ra);
+        for (int t = 0; t < un.ntiles; ++t, T += TILE_BYTES) {
+            RegsB r;
+            load_B(T, lane, r);
+            const int64_t ri = ((int64_t)un.tile0 + t) * R + lane;
             double yv = 1.0;
             if (!SQUARE) {
                 if (PERM) {
@@ -211,20 +230,30 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
                     yv = __ldcs(y + ri) * sy;
                 }
             }
-            // attitude: rows 0-15 through lanes 0-11, rows 16-31 through
-            // lanes 16-27, one row at a time per half
+            // phase A -- attitude: rows 0-15 through lanes 0-11, rows 16-31
+            // through lanes 16-27, one row per half and step; the two rows of a step go in one
+            // instruction unless their windows overlap (then one after the other)
+            const uint32_t a_other = __shfl_xor_sync(0xffffffffu, ra.aoff, 16);
+            const int da = (int)ra.aoff - (int)a_other;
+            const unsigned cmask = __ballot_sync(0xffffffffu, da > -4 && da < 4);
 #pragma unroll
             for (int qq = 0; qq < 16; ++qq) {
                 const int src = h * 16 + qq;
-                const uint32_t a = __shfl_sync(0xffffffffu, r.aoff, src);
+                const uint32_t a = __shfl_sync(0xffffffffu, ra.aoff, src);
                 const double yy = __shfl_sync(0xffffffffu, yv, src);
-                const double add = SQUARE ? r.at[qq] * r.at[qq] : r.at[qq] * yy;
+                const double add = SQUARE ? ra.at[qq] * ra.at[qq] : ra.at[qq] * yy;
                 double* pa = xw + a + axo;
-                if (lo12) *pa += add;
-                __syncwarp();
-                if (hi12) *pa += add;
+                if ((cmask >> qq) & 1u) {
+                    if (lo12) *pa += add;
+                    __syncwarp();
+                    if (hi12) *pa += add;
+                } else {
+                    if (lo12 || hi12) *pa += add;
+                }
                 __syncwarp();
             }
+            if (t + 1 < un.ntiles) load_A(T + TILE_BYTES, lane, ra);   // in flight during phase B
+            // phase B
 #pragma unroll
             for (int k = 0; k < 5; ++k) r.as[k] = SQUARE ? r.as[k] * r.as[k] : r.as[k] * yv;
 #pragma unroll
@@ -245,28 +274,39 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
                     if (lane == 0 && tsum != 0.0) atomicAdd(x + 5 * (int64_t)r.s + k, tsum);
                 }
             } else {
-                // segmented inclusive scan; the last lane of each segment holds its sum
+                // segmented inclusive scan; the last lane of each segment holds its sum.  A step
+                // of distance o is needed only if some run is longer than o rows, i.e. if there
+                // are o consecutive non-head lanes (shuffles cost LSU data-pipe wavefronts).
                 const unsigned below = heads & ((2u << lane) - 1u);        // heads at or below me
                 const int seg_start = 31 - __clz(below);
                 const bool tail = lane == 31 || ((heads >> (lane + 1)) & 1u);
+                const unsigned n1 = ~heads, n2 = n1 & (n1 >> 1), n4 = n2 & (n2 >> 2),
+                               n8 = n4 & (n4 >> 4), n16 = n8 & (n8 >> 8);
+                const unsigned need = 1u | (n2 ? 2u : 0u) | (n4 ? 4u : 0u) | (n8 ? 8u : 0u) | (n16 ? 16u : 0u);
+                double vs[5];
 #pragma unroll
-                for (int k = 0; k < 5; ++k) {
-                    double vsum = r.as[k];
+                for (int k = 0; k < 5; ++k) vs[k] = r.as[k];
 #pragma unroll
-                    for (int o = 1; o < 32; o <<= 1) {
-                        const double up = __shfl_up_sync(0xffffffffu, vsum, o);
-                        if (lane - o >= seg_start) vsum += up;
+                for (int o = 1; o < 32; o <<= 1) {
+                    if (need & o) {
+#pragma unroll
+                        for (int k = 0; k < 5; ++k) {
+                            const double up = __shfl_up_sync(0xffffffffu, vs[k], o);
+                            if (lane - o >= seg_start) vs[k] += up;
+                        }
                     }
-                    if (tail && vsum != 0.0) atomicAdd(x + 5 * (int64_t)r.s + k, vsum);
                 }
+#pragma unroll
+                for (int k = 0; k < 5; ++k)
+                    if (tail && vs[k] != 0.0) atomicAdd(x + 5 * (int64_t)r.s + k, vs[k]);
             }
         }
         // flush the unit's window
         __syncwarp();
         for (int i = lane; i < 3 * win; i += 32) {
-            const double vacc = xw[i];
+            const int ax = i / win, k = i - ax * win;
+            const double vacc = xw[ax * ws + k];
             if (vacc != 0.0) {
-                const int ax = i / win, k = i - ax * win;
                 atomicAdd(xatt + ax * D + un.a0 + k, vacc);   // knot < D whenever vacc != 0
             }
         }
@@ -328,13 +368,13 @@ int launch_aprod1(const gsr_matrix* A, const double* x, double* y, const double*
     GSR_TRY(reset_counter(A, s));
     if (perm)
         k_aprod1<false, true><<<A->grid1, TPB, A->smem_bytes, s>>>(
-            A->tiles, A->units, A->n_units, A->unit_counter, x, y, ca, nullptr, perm, S, D, I, A->win, stop);
+            A->tiles, A->units, A->n_units, A->unit_counter, x, y, ca, nullptr, perm, S, D, I, A->win, A->wstride, stop);
     else if (partials)
         k_aprod1<true, false><<<A->grid1, TPB, A->smem_bytes, s>>>(
-            A->tiles, A->units, A->n_units, A->unit_counter, x, y, ca, partials, nullptr, S, D, I, A->win, stop);
+            A->tiles, A->units, A->n_units, A->unit_counter, x, y, ca, partials, nullptr, S, D, I, A->win, A->wstride, stop);
     else
         k_aprod1<false, false><<<A->grid1, TPB, A->smem_bytes, s>>>(
-            A->tiles, A->units, A->n_units, A->unit_counter, x, y, ca, nullptr, nullptr, S, D, I, A->win, stop);
+            A->tiles, A->units, A->n_units, A->unit_counter, x, y, ca, nullptr, nullptr, S, D, I, A->win, A->wstride, stop);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;
@@ -348,10 +388,10 @@ int launch_aprod2(const gsr_matrix* A, const double* y, double* x, const double*
     GSR_TRY(reset_counter(A, s));
     if (perm)
         k_aprod2<false, true><<<A->grid2, TPB, A->smem_bytes, s>>>(
-            A->tiles, A->units, A->n_units, A->unit_counter, y, x, sy, perm, S, D, I, A->win, stop);
+            A->tiles, A->units, A->n_units, A->unit_counter, y, x, sy, perm, S, D, I, A->win, A->wstride, stop);
     else
         k_aprod2<false, false><<<A->grid2, TPB, A->smem_bytes, s>>>(
-            A->tiles, A->units, A->n_units, A->unit_counter, y, x, sy, nullptr, S, D, I, A->win, stop);
+            A->tiles, A->units, A->n_units, A->unit_counter, y, x, sy, nullptr, S, D, I, A->win, A->wstride, stop);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;
@@ -362,7 +402,7 @@ int launch_colsumsq(const gsr_matrix* A, double* q, cudaStream_t s) {
     GSR_TRY(reset_counter(A, s));
     k_aprod2<true, false><<<A->grid2, TPB, A->smem_bytes, s>>>(
         A->tiles, A->units, A->n_units, A->unit_counter, nullptr, q, nullptr, nullptr, A->dims.n_stars,
-        A->dims.n_dfa, (int)A->dims.n_instr, A->win, nullptr);
+        A->dims.n_dfa, (int)A->dims.n_instr, A->win, A->wstride, nullptr);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;

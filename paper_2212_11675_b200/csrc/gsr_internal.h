@@ -115,6 +115,9 @@ struct gsr_matrix {
     int64_t n_cols, off_att, off_instr, off_glob;
     // layout
     int nbins, bin_width, win;      // fine attitude bins; win = bin_width + 3 knots per axis
+    int wstride;                    // doubles between the axes of a window in shared memory:
+                                    // win rounded up to 4 mod 16, so that the 3 x 4 addresses
+                                    // of a row fall into 12 distinct 8-byte banks
     int smem_bytes;                 // dynamic shared memory of the product kernels
     int ctas_per_sm;                // resident product CTAs per SM the shared-memory plan allows
     int grid1, grid2;               // persistent grids of aprod1 / aprod2

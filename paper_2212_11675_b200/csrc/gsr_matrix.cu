@@ -339,12 +339,15 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
     int64_t win_bytes = (SMEM_BUDGET - instr_bytes) / NWARP;
     if (win_bytes > WIN_BYTES_MAX) win_bytes = WIN_BYTES_MAX;
     const int64_t n_start = d->n_dfa - 3;
-    const int64_t bw_max = win_bytes / 24 - 3;
+    int64_t ws_max = win_bytes / 24;                       // doubles per axis
+    ws_max = ws_max - ((ws_max - 4) % 16 + 16) % 16;       // largest value = 4 (mod 16)
+    const int64_t bw_max = ws_max - 3;
     if (bw_max < 1) return GSR_EUNSUPPORTED;
     const int64_t nbins = (n_start + bw_max - 1) / bw_max;
     if (nbins > NBIN_MAX) return GSR_EUNSUPPORTED;
     const int64_t bw = (n_start + nbins - 1) / nbins;
-    const int64_t smem_bytes = instr_bytes + NWARP * 3 * (bw + 3) * 8;
+    const int64_t wstride = (bw + 3) + ((4 - (bw + 3)) % 16 + 16) % 16;   // >= bw+3, = 4 (mod 16)
+    const int64_t smem_bytes = instr_bytes + NWARP * 3 * wstride * 8;
 
     int dev = 0;
     cudaDeviceProp prop;
@@ -364,6 +367,7 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
     A->nbins = (int)nbins;
     A->bin_width = (int)bw;
     A->win = (int)bw + 3;
+    A->wstride = (int)wstride;
     A->smem_bytes = (int)smem_bytes;
     A->ctas_per_sm = 2 * (smem_bytes + 2048) <= 227 * 1024 ? 2 : 1;
     A->stream = (cudaStream_t)stream;
