@@ -28,7 +28,12 @@ if ROOT not in sys.path:
 
 METRIC = "lsqr_iterations_per_s"
 UNIT = "it/s"
-BYTES_APROD1, BYTES_APROD2 = 240, 232          # algorithmic HBM bytes per row (DESIGN.md)
+BYTES_APROD1, BYTES_APROD2 = 240, 232          # algorithmic HBM bytes per row (DESIGN.md 5)
+TRAFFIC_APROD1, TRAFFIC_APROD2 = 228, 220      # bytes per row the 212 B/row layout really moves
+# DRAM bytes per row measured by `ncu --set full` (dram__bytes_read.sum + dram__bytes_write.sum
+# over the rows of the launch; profiles/r1_v2_aprod_ncu_full.md); multiplied by the rows of the
+# timed launch to give roofline.traffic
+NCU_TRAFFIC_PER_ROW = {"aprod1": 228.9, "aprod2": 220.3}
 GEN_ROWS = 1 << 23                              # rows generated and appended per chunk
 
 
@@ -41,6 +46,8 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--oracle-rows", type=int, default=1 << 21)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true",
+                    help="BASELINE config 5: time aprod1/aprod2 alone from 1e6 to 3e8 rows")
     return ap.parse_args()
 
 
@@ -150,12 +157,58 @@ def build_system(cfg, g, inputs, torch, dev):
     return h
 
 
+def run_sweep(args):
+    """BASELINE.json config 5: the config-1 structure from 1e6 to 3e8 rows, each product timed
+    alone (internal row order = after the attitude-bin reordering, and through the caller-order
+    API = what a caller who keeps its own row order pays for the perm gather/scatter)."""
+    import torch
+    from paper_2212_11675_b200 import binding as g, inputs
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    peak, peak_src = peaks()
+    sizes = [1_000_000 * 2 ** k for k in range(9)] + [300_000_000]
+    for m in sizes:
+        cfg = inputs.named_config(f"cfg5_{m}")
+        h = build_system(cfg, g, inputs, torch, dev)
+        ms1 = g.gsr_time_product(h, 1, 20)
+        ms2 = g.gsr_time_product(h, 2, 20)
+        x = inputs.random_vector(cfg, 1, cfg.n_cols, dev)
+        y = inputs.random_vector(cfg, 2, cfg.n_rows, dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        api = []
+        for fn, a, b in ((g.gsr_aprod1, x, y), (g.gsr_aprod2, y, x)):
+            fn(h, a, b)
+            e0.record()
+            for _ in range(5):
+                fn(h, a, b)
+            e1.record()
+            torch.cuda.synchronize()
+            api.append(e0.elapsed_time(e1) / 5)
+        row = {"workload": cfg.name, "rows": m, "cols": cfg.n_cols,
+               "l2": "L2-assisted" if 224 * m < 1e9 else "HBM",
+               "aprod1_ms": ms1, "aprod2_ms": ms2,
+               "aprod1_gbs": BYTES_APROD1 * m / ms1 * 1e-6, "aprod2_gbs": BYTES_APROD2 * m / ms2 * 1e-6,
+               "aprod1_nnz_per_s": 24 * m / (ms1 * 1e-3), "aprod2_nnz_per_s": 24 * m / (ms2 * 1e-3),
+               "aprod1_frac_of_measured": BYTES_APROD1 * m / ms1 * 1e-6 / peak,
+               "aprod2_frac_of_measured": BYTES_APROD2 * m / ms2 * 1e-6 / peak,
+               "aprod1_caller_order_ms": api[0], "aprod2_caller_order_ms": api[1],
+               "aprod1_caller_order_gbs": BYTES_APROD1 * m / api[0] * 1e-6,
+               "aprod2_caller_order_gbs": BYTES_APROD2 * m / api[1] * 1e-6,
+               "peak": peak, "peak_source": peak_src}
+        print(json.dumps(row), flush=True)
+        g.gsr_matrix_destroy(h)
+        del x, y
+        torch.cuda.empty_cache()
+
+
 def main():
     args = parse()
     from paper_2212_11675_b200 import inputs
     cfg0 = inputs.named_config(args.config)
     if args.impl == "reference":
         return run_reference(args, cfg0)
+    if args.sweep:
+        return run_sweep(args)
 
     import torch
     import torch.distributed as dist
@@ -243,6 +296,7 @@ def main():
         gb1, gb2 = BYTES_APROD1 * m / ms1 * 1e-6, BYTES_APROD2 * m / ms2 * 1e-6
         gb12 = (BYTES_APROD1 + BYTES_APROD2) * m / (ms1 + ms2) * 1e-6
         dom = ("aprod2", gb2, ms2, BYTES_APROD2) if ms2 >= ms1 else ("aprod1", gb1, ms1, BYTES_APROD1)
+        traffic = NCU_TRAFFIC_PER_ROW[dom[0]] * m
         line = {
             "metric": METRIC, "value": world * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
             "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True,
@@ -259,10 +313,15 @@ def main():
             "gpu_launches": int(launches),
             "clocks": clocks,
             "roofline": {"bound": "hbm", "kernel": dom[0], "achieved": dom[1], "peak": peak,
-                         "unit": "GB/s", "frac": dom[1] / peak, "traffic": None,
+                         "unit": "GB/s", "frac": dom[1] / peak, "traffic": traffic,
+                         "traffic_note": "DRAM bytes per launch: ncu --set full bytes per row "
+                                         "(profiles/r1_v2_aprod_ncu_full.md) x rows of this launch; the "
+                                         "layout stores 212 B/row, so traffic < algorithmic bytes",
                          "peak_source": peak_src, "algorithmic_bytes_per_row": dom[3],
                          "ms_per_launch": dom[2]},
             "products": {"aprod1_gbs": gb1, "aprod2_gbs": gb2, "aprod1_ms": ms1, "aprod2_ms": ms2,
+                         "aprod1_actual_gbs": TRAFFIC_APROD1 * m / ms1 * 1e-6,
+                         "aprod2_actual_gbs": TRAFFIC_APROD2 * m / ms2 * 1e-6,
                          "combined_gbs": gb12, "combined_frac_of_measured": gb12 / peak,
                          "combined_frac_of_8tbs": gb12 / 8000.0,
                          "iteration_gbs": 472 * m / (ms / K) * 1e-6},
