@@ -33,7 +33,7 @@ TRAFFIC_APROD1, TRAFFIC_APROD2 = 228, 220      # bytes per row the 212 B/row lay
 # DRAM bytes per row measured by `ncu --set full` (dram__bytes_read.sum + dram__bytes_write.sum
 # over the rows of the launch; profiles/r1_v2_aprod_ncu_full.md); multiplied by the rows of the
 # timed launch to give roofline.traffic
-NCU_TRAFFIC_PER_ROW = {"aprod1": 228.9, "aprod2": 220.3}
+NCU_TRAFFIC_PER_ROW = {"aprod1": 228.1, "aprod2": 220.3}
 GEN_ROWS = 1 << 23                              # rows generated and appended per chunk
 
 
