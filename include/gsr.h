@@ -135,7 +135,12 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
 enum {
     GSR_OPT_FORCE_ITNLIM = 1, /* 1: rules 1-6 are evaluated and recorded in *_natural but only
                                  the iteration limit stops the loop (fixed-count mode, A9)    */
-    GSR_OPT_DETERMINISTIC = 2 /* 1: aprod2 uses no floating-point atomics (bit-reproducible)  */
+    GSR_OPT_DETERMINISTIC = 2, /* 1: aprod2 uses no floating-point atomics (bit-reproducible);
+                                 reserved: any value but 0 returns GSR_EUNSUPPORTED           */
+    GSR_OPT_FUSED = 3         /* 1 (default): one LSQR iteration reads the matrix ONCE -- u_hat =
+                                 A v - (alpha/beta) u_hat and A^T u_hat are formed in the same
+                                 pass, v = A^T u_hat / beta - beta v afterwards (same recurrences,
+                                 DESIGN.md 5.5); 0: aprod1 then aprod2, two reads per iteration  */
 };
 int gsr_set_option(gsr_matrix* A, int key, int64_t value);
 
@@ -151,7 +156,9 @@ int gsr_debug_expand_rows(const gsr_matrix* A, int64_t row0, int64_t nrows, int6
 
 /* Average device time (ms, CUDA events on `stream`) of `reps` back-to-back launches of the
  * product kernels as the solver runs them (internal row order, fused coefficients):
- * which = 1: aprod1 (u <- A v - c u, + norm partials), which = 2: aprod2 (v += A^T u/beta).
+ * which = 1: aprod1 (u <- A v - c u, + norm partials), which = 2: aprod2 (v += A^T u/beta),
+ * which = 3: the fused pass of GSR_OPT_FUSED (u <- A v - c u and t += A^T u without the
+ * instrumental block), which = 4: its instrumental pass.
  * Scratch vectors inside the handle are used; results are discarded.  Synchronous. */
 int gsr_time_product(gsr_matrix* A, int which, int reps, float* ms_avg, gsr_stream stream);
 

@@ -323,6 +323,190 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
     }
 }
 
+// ---- fused LSQR pass: u <- A v + ca u  and  t += A^T u_new  in ONE read of the matrix ------
+// The second half of the bidiagonalisation step needs A^T u_{k+1} = A^T u_hat / beta_{k+1}; by
+// linearity the unnormalised A^T u_hat can be accumulated while u_hat is being produced, row by
+// row, so the matrix is streamed once per iteration instead of twice (rows a3 + a5, a6, a8).
+// The instrumental block of A^T u_hat (a7) is left to k_aprod2_instr, because its CTA-shared
+// accumulator (I doubles) does not fit in shared memory beside x's instrumental block and the
+// two attitude windows per warp at I = 10 000.
+__global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__ tiles,
+                                              const Unit* __restrict__ units, int n_units,
+                                              int* __restrict__ counter,
+                                              const double* __restrict__ x, double* __restrict__ y,
+                                              const double* __restrict__ ca_p,
+                                              double* __restrict__ partials, double* __restrict__ tacc,
+                                              int64_t S, int64_t D, int I, int win, int ws,
+                                              const int* __restrict__ stop) {
+    if (stop && *stop) return;
+    extern __shared__ double sm[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double* xi = sm;
+    double* xw = sm + ((I + 1) & ~1) + warp * 6 * ws;   // window of v (read)
+    double* tw = xw + 3 * ws;                           // window of A^T u_hat (accumulate)
+    const double* xatt = x + 5 * S;
+    const double* xins = x + 5 * S + 3 * D;
+    double* tatt = tacc + 5 * S;
+    for (int i = threadIdx.x; i < I; i += TPB) xi[i] = __ldg(xins + i);
+    const double xg = __ldg(xins + I);
+    const double ca = *ca_p;
+    __syncthreads();
+
+    const int h = lane >> 4, j = lane & 15, jj = min(j, 11);
+    const int axo = (jj >> 2) * ws + (jj & 3);
+    const bool att_lane = j < 12;
+    const bool lo12 = lane < 12, hi12 = lane >= 16 && lane < 28;
+    double g = 0.0;
+    for (;;) {
+        const int u = fetch_unit(counter, lane);
+        if (u >= n_units) break;
+        const Unit un = units[u];
+        __syncwarp();
+        for (int i = lane; i < 3 * win; i += 32) {
+            const int ax = i / win, k = i - ax * win;
+            const int64_t knot = (int64_t)un.a0 + k;
+            xw[ax * ws + k] = knot < D ? __ldg(xatt + ax * D + knot) : 0.0;
+        }
+        for (int i = lane; i < 3 * ws; i += 32) tw[i] = 0.0;
+        __syncwarp();
+        double q = 0.0;
+        const unsigned char* T = tiles + (int64_t)un.tile0 * TILE_BYTES;
+        RegsA ra;
+        load_A(T, lane, ra);
+        for (int t = 0; t < un.ntiles; ++t, T += TILE_BYTES) {
+            RegsB r;
+            load_B(T, lane, r);
+            const int64_t ri = ((int64_t)un.tile0 + t) * R + lane;
+            const double yold = __ldcs(y + ri);
+            // ---- mode 1 for this tile
+            double p[16];
+#pragma unroll
+            for (int qq = 0; qq < 16; ++qq) {
+                const uint32_t a = __shfl_sync(0xffffffffu, ra.aoff, h * 16 + qq);
+                const double pv = ra.at[qq] * xw[a + axo];
+                p[qq] = att_lane ? pv : 0.0;
+            }
+#pragma unroll
+            for (int o = 8; o > 0; o >>= 1) {
+                const bool up = (j & o) != 0;
+#pragma unroll
+                for (int i = 0; i < o; ++i) {
+                    const double send = up ? p[i] : p[i + o];
+                    const double keep = up ? p[i + o] : p[i];
+                    p[i] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+                }
+            }
+            double sum = p[0];
+            const double* xa = x + 5 * (int64_t)r.s;
+#pragma unroll
+            for (int k = 0; k < 5; ++k) sum = fma(r.as[k], __ldg(xa + k), sum);
+#pragma unroll
+            for (int k = 0; k < 6; ++k) sum = fma(r.in[k], xi[r.c[k]], sum);
+            sum = fma(r.gl, xg, sum);
+            const double yv = fma(ca, yold, sum);   // u_hat of this row (padding rows: 0)
+            y[ri] = yv;
+            q = fma(yv, yv, q);
+            // ---- mode 2 for this tile, attitude
+            const uint32_t a_other = __shfl_xor_sync(0xffffffffu, ra.aoff, 16);
+            const int da = (int)ra.aoff - (int)a_other;
+            const unsigned cmask = __ballot_sync(0xffffffffu, da > -4 && da < 4);
+#pragma unroll
+            for (int qq = 0; qq < 16; ++qq) {
+                const int src = h * 16 + qq;
+                const uint32_t a = __shfl_sync(0xffffffffu, ra.aoff, src);
+                const double yy = __shfl_sync(0xffffffffu, yv, src);
+                const double add = ra.at[qq] * yy;
+                double* pa = tw + a + axo;
+                if ((cmask >> qq) & 1u) {
+                    if (lo12) *pa += add;
+                    __syncwarp();
+                    if (hi12) *pa += add;
+                } else {
+                    if (lo12 || hi12) *pa += add;
+                }
+                __syncwarp();
+            }
+            if (t + 1 < un.ntiles) load_A(T + TILE_BYTES, lane, ra);
+            // ---- mode 2, global and astrometric
+            g = fma(r.gl, yv, g);
+#pragma unroll
+            for (int k = 0; k < 5; ++k) r.as[k] *= yv;
+            const int32_t s_up = __shfl_up_sync(0xffffffffu, r.s, 1);
+            const bool head = lane == 0 || s_up != r.s;
+            const unsigned heads = __ballot_sync(0xffffffffu, head);
+            if (heads == 1u) {
+#pragma unroll
+                for (int k = 0; k < 5; ++k) {
+                    const double tsum = warp_sum(r.as[k]);
+                    if (lane == 0 && tsum != 0.0) atomicAdd(tacc + 5 * (int64_t)r.s + k, tsum);
+                }
+            } else {
+                const unsigned below = heads & ((2u << lane) - 1u);
+                const int seg_start = 31 - __clz(below);
+                const bool tail = lane == 31 || ((heads >> (lane + 1)) & 1u);
+                const unsigned n1 = ~heads, n2 = n1 & (n1 >> 1), n4 = n2 & (n2 >> 2),
+                               n8 = n4 & (n4 >> 4), n16 = n8 & (n8 >> 8);
+                const unsigned need = 1u | (n2 ? 2u : 0u) | (n4 ? 4u : 0u) | (n8 ? 8u : 0u) | (n16 ? 16u : 0u);
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    if (need & o) {
+#pragma unroll
+                        for (int k = 0; k < 5; ++k) {
+                            const double up = __shfl_up_sync(0xffffffffu, r.as[k], o);
+                            if (lane - o >= seg_start) r.as[k] += up;
+                        }
+                    }
+                }
+#pragma unroll
+                for (int k = 0; k < 5; ++k)
+                    if (tail && r.as[k] != 0.0) atomicAdd(tacc + 5 * (int64_t)r.s + k, r.as[k]);
+            }
+        }
+        q = warp_sum(q);
+        if (lane == 0) partials[u] = q;
+        __syncwarp();
+        for (int i = lane; i < 3 * win; i += 32) {
+            const int ax = i / win, k = i - ax * win;
+            const double vacc = tw[ax * ws + k];
+            if (vacc != 0.0) atomicAdd(tatt + ax * D + un.a0 + k, vacc);
+        }
+    }
+    g = warp_sum(g);
+    if (lane == 0 && g != 0.0) atomicAdd(tacc + 5 * S + 3 * D + I, g);
+}
+
+// Instrumental block of A^T u (row a7) over the instrumental planes only (1920 B per tile):
+// CTA-shared shared-memory accumulators, six fp64 shared atomicAdds per row.
+__global__ void __launch_bounds__(TPB) k_aprod2_instr(const unsigned char* __restrict__ tiles,
+                                                     int64_t n_tiles, const double* __restrict__ y,
+                                                     double* __restrict__ xins, int I,
+                                                     const int* __restrict__ stop) {
+    if (stop && *stop) return;
+    extern __shared__ double sm[];
+    for (int i = threadIdx.x; i < I; i += TPB) sm[i] = 0.0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31;
+    const int64_t w0 = (int64_t)blockIdx.x * NWARP + (threadIdx.x >> 5);
+    const int64_t nw = (int64_t)gridDim.x * NWARP;
+    for (int64_t tile = w0; tile < n_tiles; tile += nw) {
+        const unsigned char* T = tiles + tile * TILE_BYTES;
+        uint32_t c[6];
+        double v[6];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) c[k] = ld_stream_u16(T + OFF_ICOL + (k * R + lane) * 2);
+#pragma unroll
+        for (int k = 0; k < 6; ++k) v[k] = ld_stream_f64(T + OFF_INSTRV + (k * R + lane) * 8);
+        const double yv = __ldcs(y + tile * R + lane);
+#pragma unroll
+        for (int k = 0; k < 6; ++k) atomicAdd(sm + c[k], v[k] * yv);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < I; i += TPB) {
+        const double vacc = sm[i];
+        if (vacc != 0.0) atomicAdd(xins + i, vacc);
+    }
+}
+
 template <typename K>
 static int set_smem(K kernel, int bytes) {
     GSR_CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
@@ -347,11 +531,31 @@ int configure_product_kernels(gsr_matrix* A) {
     GSR_TRY(set_smem(k_aprod2<false, false>, b));
     GSR_TRY(set_smem(k_aprod2<false, true>, b));
     GSR_TRY(set_smem(k_aprod2<true, false>, b));
+    GSR_TRY(set_smem(k_fused, A->smem_fused));
+    GSR_TRY(set_smem(k_aprod2_instr, (int)((A->dims.n_instr + 1) / 2 * 16)));
+    {
+        int nb = 1;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_fused, TPB, A->smem_fused) != cudaSuccess || nb < 1) {
+            cudaGetLastError();
+            nb = 1;
+        }
+        A->grid_fused = A->sm_count * nb;
+        nb = 1;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_aprod2_instr, TPB,
+                                                          (size_t)((A->dims.n_instr + 1) / 2 * 16)) != cudaSuccess || nb < 1) {
+            cudaGetLastError();
+            nb = 1;
+        }
+        A->grid_instr = A->sm_count * nb;
+    }
     A->grid1 = A->sm_count * resident_ctas(k_aprod1<true, false>, A);
     A->grid2 = A->sm_count * resident_ctas(k_aprod2<false, false>, A);
     const int need = (A->n_units + NWARP - 1) / NWARP;
     if (A->grid1 > need) A->grid1 = need;
     if (A->grid2 > need) A->grid2 = need;
+    if (A->grid_fused > need) A->grid_fused = need;
+    const int64_t need_i = (A->n_tiles + NWARP - 1) / NWARP;
+    if (A->grid_instr > need_i) A->grid_instr = (int)(need_i > 0 ? need_i : 1);
     return GSR_OK;
 }
 
@@ -392,6 +596,28 @@ int launch_aprod2(const gsr_matrix* A, const double* y, double* x, const double*
     else
         k_aprod2<false, false><<<A->grid2, TPB, A->smem_bytes, s>>>(
             A->tiles, A->units, A->n_units, A->unit_counter, y, x, sy, nullptr, S, D, I, A->win, A->wstride, stop);
+    count_launch();
+    GSR_CUDA_TRY(cudaGetLastError());
+    return GSR_OK;
+}
+
+int launch_fused(const gsr_matrix* A, const double* v, double* u, const double* ca,
+                 double* partials, double* t, const int* stop, cudaStream_t s) {
+    if (A->n_units == 0) return GSR_OK;
+    GSR_TRY(reset_counter(A, s));
+    k_fused<<<A->grid_fused, TPB, A->smem_fused, s>>>(A->tiles, A->units, A->n_units, A->unit_counter, v, u,
+                                                     ca, partials, t, A->dims.n_stars, A->dims.n_dfa,
+                                                     (int)A->dims.n_instr, A->win, A->wstride, stop);
+    count_launch();
+    GSR_CUDA_TRY(cudaGetLastError());
+    return GSR_OK;
+}
+
+int launch_aprod2_instr(const gsr_matrix* A, const double* u, double* t, const int* stop,
+                        cudaStream_t s) {
+    if (A->n_tiles == 0) return GSR_OK;
+    k_aprod2_instr<<<A->grid_instr, TPB, (size_t)((A->dims.n_instr + 1) / 2 * 16), s>>>(
+        A->tiles, A->n_tiles, u, t + A->off_instr, (int)A->dims.n_instr, stop);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;

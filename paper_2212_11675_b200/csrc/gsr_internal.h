@@ -20,9 +20,10 @@ namespace gsr {
 //         coefficient j of 16 rows.  aprod2 then adds row after row into the window with 12
 //         lanes at 12 distinct addresses (plain read-modify-write, no atomics); aprod1 forms
 //         the 12 products per row the same way and transposes them back with 15 shuffles.
-//   instr [6][32] f64, glob [32] f64   plane-major
-//   star  [32] i32
+//   instr [6][32] f64   plane-major
 //   icol  [6][32] u16   instrumental columns (I <= 65535 is implied by the shared-memory plan)
+//   glob  [32] f64
+//   star  [32] i32
 //   aoff  [32] u16      att_start - a0 of the unit (offset inside the warp's window)
 //   a0    i32           first knot of the window (same for every tile of a unit)
 //   60 bytes of padding                                                = 6784 B = 212 B/row
@@ -41,10 +42,12 @@ constexpr int NPAR = 24;
 constexpr int OFF_ASTRO = 0;                 // byte offsets inside a tile record
 constexpr int OFF_ATTV = 5 * R * 8;          // 1280
 constexpr int OFF_INSTRV = OFF_ATTV + 12 * R * 8;   // 4352
-constexpr int OFF_GLOBV = OFF_INSTRV + 6 * R * 8;   // 5888
-constexpr int OFF_STAR = OFF_GLOBV + R * 8;         // 6144
-constexpr int OFF_ICOL = OFF_STAR + R * 4;          // 6272
-constexpr int OFF_AOFF = OFF_ICOL + 6 * R * 2;      // 6656
+constexpr int OFF_ICOL = OFF_INSTRV + 6 * R * 8;    // 5888 (instrumental values and columns are
+                                                    //       adjacent: the instrumental pass of the
+                                                    //       fused iteration reads only these 1920 B)
+constexpr int OFF_GLOBV = OFF_ICOL + 6 * R * 2;     // 6272
+constexpr int OFF_STAR = OFF_GLOBV + R * 8;         // 6528
+constexpr int OFF_AOFF = OFF_STAR + R * 4;          // 6656
 constexpr int OFF_A0 = OFF_AOFF + R * 2;            // 6720: i32 first knot of the tile's window
 constexpr int TILE_BYTES = 6784;                    // 53 * 128
 static_assert(OFF_A0 + 4 <= TILE_BYTES && TILE_BYTES % 128 == 0, "tile record");
@@ -61,7 +64,8 @@ constexpr int NBIN_MAX = 4096;               // fine attitude bins
 constexpr int NWARP = 16;                    // warps per product CTA
 constexpr int TPB = NWARP * 32;
 constexpr int SMEM_BUDGET = 224 * 1024;      // dynamic shared memory a product CTA may use
-constexpr int WIN_BYTES_MAX = 6 * 1024;      // per-warp attitude window, 3 axes
+constexpr int WIN_BYTES_MAX = 6 * 1024;      // per-warp attitude window, 3 axes (the fused
+                                             // iteration kernel keeps two of them per warp)
 constexpr int STAGE_BYTES = 0;               // per-warp scratch besides the window
 constexpr int UNIT_TILES_MAX = 128;          // tiles per unit (upper bound)
 constexpr uint32_t PERM_PAD = 0xFFFFFFFFu;
@@ -96,6 +100,7 @@ struct Workspace {
     double* v = nullptr;        // [n]
     double* w = nullptr;        // [n]
     double* x = nullptr;        // [n]  iterate z of the (scaled) system
+    double* t = nullptr;        // [n]  A^T u_hat of the fused pass (zero between iterations)
     double* part_u = nullptr;   // [max(n_units, NB_N)] per-unit partial sums of u_hat^2
     double* part_v = nullptr;   // [NB_N]
     double* part_w = nullptr;   // [NB_N]
@@ -106,6 +111,7 @@ struct Workspace {
     cudaGraphExec_t graph = nullptr;
     cudaStream_t graph_stream = nullptr;
     bool graph_valid = false;
+    int graph_two_pass = 0;
 };
 
 }  // namespace gsr
@@ -119,8 +125,10 @@ struct gsr_matrix {
                                     // win rounded up to 4 mod 16, so that the 3 x 4 addresses
                                     // of a row fall into 12 distinct 8-byte banks
     int smem_bytes;                 // dynamic shared memory of the product kernels
+    int smem_fused;                 // ... of the fused iteration kernel (two windows per warp)
     int ctas_per_sm;                // resident product CTAs per SM the shared-memory plan allows
     int grid1, grid2;               // persistent grids of aprod1 / aprod2
+    int grid_fused, grid_instr;     // ... of the fused iteration kernel / its instrumental pass
     int64_t tiles_cap, n_tiles;     // allocated / used tiles
     int64_t m_int;                  // n_tiles * R, length of internal-order vectors
     unsigned char* tiles;           // tiles_cap * TILE_BYTES
@@ -144,6 +152,7 @@ struct gsr_matrix {
     double* coef_one;               // device constants {1.0, 1.0}
     int64_t device_bytes;
     int opt_force_itnlim;
+    int opt_two_pass;               // 1: aprod1 + aprod2 per iteration instead of the fused pass
     int sm_count;
     gsr::Workspace ws;
 };
@@ -185,6 +194,15 @@ int launch_aprod2(const gsr_matrix* A, const double* y, double* x, const double*
                   const int* stop, const uint32_t* perm, cudaStream_t s);
 //   column sums of squares (preconditioner): q[col] += A[i,k]^2
 int launch_colsumsq(const gsr_matrix* A, double* q, cudaStream_t s);
+// fused LSQR pass (one read of the matrix per iteration):
+//   u[i] = (*ca) * u[i] + sum_k A[i,k] v[col]   (partials[unit] = sum of u_new^2)
+//   t[col] += A[i,k] * u_new[i]                  for the astrometric, attitude and global blocks
+// followed by the instrumental pass  t[off_instr + c] += A[i,17+j] * u[i]  over the
+// instrumental planes only.  t must hold zeros (or the value to accumulate onto) on entry.
+int launch_fused(const gsr_matrix* A, const double* v, double* u, const double* ca,
+                 double* partials, double* t, const int* stop, cudaStream_t s);
+int launch_aprod2_instr(const gsr_matrix* A, const double* u, double* t, const int* stop,
+                        cudaStream_t s);
 int configure_product_kernels(gsr_matrix* A);
 
 }  // namespace gsr

@@ -88,6 +88,24 @@ __global__ void __launch_bounds__(TB_N) k_prescale(double* __restrict__ v, int64
         v[i] = c * v[i];
 }
 
+// v <- t * inv_beta + vscale * v  (= A^T u - beta v with t = A^T u_hat from the fused pass) and
+// partial sums of the new v squared
+__global__ void __launch_bounds__(TB_N) k_vnew(double* __restrict__ v, const double* __restrict__ t,
+                                               int64_t len, const LsqrState* __restrict__ st,
+                                               double* __restrict__ part) {
+    if (st->stop) return;
+    __shared__ double red[TB_N / 32];
+    const double ib = st->inv_beta, c = st->vscale;
+    double q = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * TB_N + threadIdx.x; i < len; i += (int64_t)gridDim.x * TB_N) {
+        const double vn = fma(t[i], ib, c * v[i]);
+        v[i] = vn;
+        q = fma(vn, vn, q);
+    }
+    q = block_sum_256(q, red);
+    if (threadIdx.x == 0) part[blockIdx.x] = q;
+}
+
 // fused n-sized update (row a10): v <- v*inv_alpha ; x += t1 w ; w = v + t2 w ; partials of
 // the NEW w squared (used as ||w||^2 by the next iteration's ddnorm, reading A10).
 // INIT: w = v (first step), x untouched (already zero).
@@ -95,7 +113,7 @@ template <bool INIT>
 __global__ void __launch_bounds__(TB_N) k_update(double* __restrict__ v, double* __restrict__ w,
                                                  double* __restrict__ x, int64_t len,
                                                  const LsqrState* __restrict__ st,
-                                                 double* __restrict__ part_w) {
+                                                 double* __restrict__ part_w, double* __restrict__ tz) {
     if (st->stop) return;
     __shared__ double red[TB_N / 32];
     const double ia = st->inv_alpha, t1 = st->t1, t2 = st->t2;
@@ -112,6 +130,7 @@ __global__ void __launch_bounds__(TB_N) k_update(double* __restrict__ v, double*
             wn = fma(t2, wo, vn);
         }
         w[i] = wn;
+        if (tz) tz[i] = 0.0;   // clears the accumulator of the next fused pass
         q = fma(wn, wn, q);
     }
     q = block_sum_256(q, red);
@@ -282,6 +301,7 @@ int ensure_workspace(gsr_matrix* A) {
     GSR_TRY(dev_alloc(A, (void**)&W.v, n8));
     GSR_TRY(dev_alloc(A, (void**)&W.w, n8));
     GSR_TRY(dev_alloc(A, (void**)&W.x, n8));
+    GSR_TRY(dev_alloc(A, (void**)&W.t, n8));
     GSR_TRY(dev_alloc(A, (void**)&W.part_u, (size_t)npu * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.part_v, NB_N * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.part_w, NB_N * 8));
@@ -295,7 +315,7 @@ int ensure_workspace(gsr_matrix* A) {
 void free_workspace(gsr_matrix* A) {
     Workspace& W = A->ws;
     if (W.graph) cudaGraphExecDestroy(W.graph);
-    cudaFree(W.u); cudaFree(W.v); cudaFree(W.w); cudaFree(W.x);
+    cudaFree(W.u); cudaFree(W.v); cudaFree(W.w); cudaFree(W.x); cudaFree(W.t);
     cudaFree(W.part_u); cudaFree(W.part_v); cudaFree(W.part_w);
     cudaFree(W.stage_m); cudaFree(W.stage_n); cudaFree(W.st);
     if (W.stop_host) cudaFreeHost(W.stop_host);
@@ -303,22 +323,34 @@ void free_workspace(gsr_matrix* A) {
     W = Workspace();
 }
 
-constexpr int KERNELS_PER_ITERATION = 8;
-
 // One LSQR iteration as a fixed kernel sequence (row a11).  Every kernel reads its
 // coefficients from LsqrState and returns at once when st->stop is set.
+// Fused form (default): the matrix is read once -- k_fused produces u_hat and t = A^T u_hat
+// together, k_aprod2_instr adds the instrumental block of t, k_vnew forms v = t/beta - beta v.
+// Two-pass form (GSR_OPT_FUSED = 0): aprod1, then aprod2 on the pre-scaled v.
+static int kernels_per_iteration(const gsr_matrix* A) { return A->opt_two_pass ? 8 : 7; }
+
 static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
     Workspace& W = A->ws;
     const int64_t n = A->n_cols;
-    // bidiagonalisation, first half: u_hat <- A v - (alpha/beta) u_hat ; partials of u_hat^2
-    GSR_TRY(launch_aprod1(A, W.v, W.u, &W.st->ca, W.part_u, &W.st->stop, nullptr, s));
-    k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_units);
-    // second half: v <- A^T (u_hat/beta) - beta v
-    k_prescale<<<NB_N, TB_N, 0, s>>>(W.v, n, W.st);
-    GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s));
-    k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop);
-    k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N);
-    k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w);
+    if (A->opt_two_pass) {
+        // bidiagonalisation, first half: u_hat <- A v - (alpha/beta) u_hat ; partials of u_hat^2
+        GSR_TRY(launch_aprod1(A, W.v, W.u, &W.st->ca, W.part_u, &W.st->stop, nullptr, s));
+        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_units);
+        // second half: v <- A^T (u_hat/beta) - beta v
+        k_prescale<<<NB_N, TB_N, 0, s>>>(W.v, n, W.st);
+        GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s));
+        k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop);
+        k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N);
+        k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, nullptr);
+    } else {
+        GSR_TRY(launch_fused(A, W.v, W.u, &W.st->ca, W.part_u, W.t, &W.st->stop, s));
+        GSR_TRY(launch_aprod2_instr(A, W.u, W.t, &W.st->stop, s));
+        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_units);
+        k_vnew<<<NB_N, TB_N, 0, s>>>(W.v, W.t, n, W.st, W.part_v);
+        k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N);
+        k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, W.t);
+    }
     k_raise_stop<<<1, 1, 0, s>>>(W.st);
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;
@@ -326,7 +358,7 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
 
 static int build_graph(gsr_matrix* A, cudaStream_t s) {
     Workspace& W = A->ws;
-    if (W.graph_valid && W.graph_stream == s) return GSR_OK;
+    if (W.graph_valid && W.graph_stream == s && W.graph_two_pass == A->opt_two_pass) return GSR_OK;
     if (W.graph) {
         cudaGraphExecDestroy(W.graph);
         W.graph = nullptr;
@@ -361,6 +393,7 @@ static int build_graph(gsr_matrix* A, cudaStream_t s) {
     }
     W.graph_valid = true;
     W.graph_stream = s;
+    W.graph_two_pass = A->opt_two_pass;
     return GSR_OK;
 }
 
@@ -407,7 +440,8 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s));
     k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop);
     k_scalar_init2<<<1, 1024, 0, s>>>(W.st, W.part_v, NB_N);
-    k_update<true><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w);
+    k_update<true><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, nullptr);
+    GSR_CUDA_TRY(cudaMemsetAsync(W.t, 0, (size_t)n * 8, s));
     count_launch(3);
     GSR_CUDA_TRY(cudaGetLastError());
 
@@ -418,7 +452,7 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     while (launched < itnlim) {
         int64_t nb = itnlim - launched < batch ? itnlim - launched : batch;
         for (int64_t i = 0; i < nb; ++i) GSR_CUDA_TRY(cudaGraphLaunch(W.graph, s));
-        count_launch(nb * KERNELS_PER_ITERATION);
+        count_launch(nb * kernels_per_iteration(A));
         launched += nb;
         GSR_CUDA_TRY(cudaMemcpyAsync(W.stop_host, &W.st->stop, sizeof(int), cudaMemcpyDeviceToHost, s));
         GSR_CUDA_TRY(cudaStreamSynchronize(s));
@@ -452,7 +486,7 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
 }
 
 int gsr_time_product(gsr_matrix* A, int which, int reps, float* ms_avg, gsr_stream stream) {
-    if (!A || !ms_avg || reps < 1 || (which != 1 && which != 2)) return GSR_EINVAL;
+    if (!A || !ms_avg || reps < 1 || which < 1 || which > 4) return GSR_EINVAL;
     if (A->state != 1) return GSR_ESTATE;
     cudaStream_t s = (cudaStream_t)stream;
     Workspace& W = A->ws;
@@ -466,7 +500,9 @@ int gsr_time_product(gsr_matrix* A, int which, int reps, float* ms_avg, gsr_stre
         cudaEventRecord(e0, s);
         for (int i = 0; i < nrep && rc == GSR_OK; ++i) {
             if (which == 1) rc = launch_aprod1(A, W.v, W.u, A->coef_one, W.part_u, nullptr, nullptr, s);
-            else rc = launch_aprod2(A, W.u, W.v, A->coef_one, nullptr, nullptr, s);
+            else if (which == 2) rc = launch_aprod2(A, W.u, W.v, A->coef_one, nullptr, nullptr, s);
+            else if (which == 3) rc = launch_fused(A, W.v, W.u, A->coef_one, W.part_u, W.t, nullptr, s);
+            else rc = launch_aprod2_instr(A, W.u, W.t, nullptr, s);
         }
         cudaEventRecord(e1, s);
         if (cudaEventSynchronize(e1) != cudaSuccess) rc = GSR_ECUDA;

@@ -336,7 +336,8 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
     // warps of a CTA, + one private attitude window of `win` knots x 3 axes per warp
     const int64_t instr_bytes = (d->n_instr + 1) / 2 * 16;
     if (d->n_instr > 65535 || instr_bytes > SMEM_BUDGET - NWARP * 24 * 4) return GSR_EUNSUPPORTED;
-    int64_t win_bytes = (SMEM_BUDGET - instr_bytes) / NWARP;
+    // (the fused iteration kernel keeps two windows per warp: v to read, A^T u to accumulate)
+    int64_t win_bytes = (SMEM_BUDGET - instr_bytes) / NWARP / 2;
     if (win_bytes > WIN_BYTES_MAX) win_bytes = WIN_BYTES_MAX;
     const int64_t n_start = d->n_dfa - 3;
     int64_t ws_max = win_bytes / 24;                       // doubles per axis
@@ -369,6 +370,7 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
     A->win = (int)bw + 3;
     A->wstride = (int)wstride;
     A->smem_bytes = (int)smem_bytes;
+    A->smem_fused = (int)(instr_bytes + NWARP * 6 * wstride * 8);
     A->ctas_per_sm = 2 * (smem_bytes + 2048) <= 227 * 1024 ? 2 : 1;
     A->stream = (cudaStream_t)stream;
     A->sm_count = prop.multiProcessorCount;
@@ -512,6 +514,7 @@ int gsr_set_option(gsr_matrix* A, int key, int64_t value) {
     switch (key) {
         case GSR_OPT_FORCE_ITNLIM: A->opt_force_itnlim = value != 0; return GSR_OK;
         case GSR_OPT_DETERMINISTIC: return value == 0 ? GSR_OK : GSR_EUNSUPPORTED;
+        case GSR_OPT_FUSED: A->opt_two_pass = value == 0; return GSR_OK;
         default: return GSR_EINVAL;
     }
 }

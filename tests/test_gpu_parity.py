@@ -117,12 +117,15 @@ def _rhs(s):
     return s.o.aprod1(xt, inputs.noise(s.cfg, 0, s.m).numpy())
 
 
+@pytest.mark.parametrize("fused", [1, 0])
 @pytest.mark.parametrize("name", ["cfg1", "ragged_empty_stars", "skew_hot", "one_instr_col"])
-def test_precondition_and_lsqr_parity(name):
-    """Column scaling then fixed-count and standard-mode PC-LSQR."""
+def test_precondition_and_lsqr_parity(name, fused):
+    """Column scaling then fixed-count and standard-mode PC-LSQR, with the fused
+    one-pass iteration (GSR_OPT_FUSED = 1, default) and with aprod1 + aprod2 per iteration."""
     b = _binding()
     s = Sys(CASES[name])
     try:
+        b.gsr_set_option(s.A.h, b.GSR_OPT_FUSED, fused)
         rhs = _rhs(s)                       # b formed with the oracle's aprod1 on the unscaled A
         p_ref = s.o.precondition()
         p = torch.empty(s.n, dtype=torch.float64, device="cuda")
