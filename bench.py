@@ -30,10 +30,14 @@ METRIC = "lsqr_iterations_per_s"
 UNIT = "it/s"
 BYTES_APROD1, BYTES_APROD2 = 240, 232          # algorithmic HBM bytes per row
 TRAFFIC_APROD1, TRAFFIC_APROD2 = 228, 220      # bytes per row the 212 B/row layout really moves
+# fused iteration (GSR_OPT_FUSED, default): k_fused does aprod1 and aprod2 minus the instrumental
+# block of A^T u (6 x (8+4) B of matrix + 8 B of u per row = 80 B), which k_aprod2_instr does
+BYTES_INSTR = 80
+BYTES_FUSED = BYTES_APROD1 + BYTES_APROD2 - BYTES_INSTR   # 392 algorithmic bytes per row
 # DRAM bytes per row measured by `ncu --set full` (dram__bytes_read.sum + dram__bytes_write.sum
 # over the rows of the launch; profiles/r1_v2_aprod_ncu_full.md); multiplied by the rows of the
 # timed launch to give roofline.traffic
-NCU_TRAFFIC_PER_ROW = {"aprod1": 228.1, "aprod2": 220.3}
+NCU_TRAFFIC_PER_ROW = {"aprod1": 228.1, "aprod2": 220.3, "fused": 228.3, "aprod2_instr": 68.1}
 GEN_ROWS = 1 << 23                              # rows generated and appended per chunk
 
 
@@ -46,6 +50,8 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--oracle-rows", type=int, default=1 << 21)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--two-pass", action="store_true",
+                    help="GSR_OPT_FUSED = 0: aprod1 + aprod2 per iteration (two reads of the matrix)")
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE config 5: time aprod1/aprod2 alone from 1e6 to 3e8 rows")
     return ap.parse_args()
@@ -241,6 +247,7 @@ def main():
     g.gsr_aprod1(h, xt, b)
     g.gsr_precondition(h)
     g.gsr_set_option(h, g.GSR_OPT_FORCE_ITNLIM, 1)
+    g.gsr_set_option(h, g.GSR_OPT_FUSED, 0 if args.two_pass else 1)
     x = torch.empty(n, dtype=torch.float64, device=dev)
     torch.cuda.synchronize()
     t_setup = time.perf_counter() - t_setup
@@ -285,18 +292,25 @@ def main():
     reps = 10
     ms1 = g.gsr_time_product(h, 1, reps)
     ms2 = g.gsr_time_product(h, 2, reps)
+    ms3 = g.gsr_time_product(h, 3, reps)
+    ms4 = g.gsr_time_product(h, 4, reps)
 
-    t = torch.tensor([ms, t_e2e * 1e3, ms1, ms2], dtype=torch.float64, device=dev)
+    t = torch.tensor([ms, t_e2e * 1e3, ms1, ms2, ms3, ms4], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, ms_e2e, ms1, ms2 = [float(v) for v in t]
+    ms, ms_e2e, ms1, ms2, ms3, ms4 = [float(v) for v in t]
 
     if rank == 0:
         peak, peak_src = peaks()
         gb1, gb2 = BYTES_APROD1 * m / ms1 * 1e-6, BYTES_APROD2 * m / ms2 * 1e-6
         gb12 = (BYTES_APROD1 + BYTES_APROD2) * m / (ms1 + ms2) * 1e-6
-        dom = ("aprod2", gb2, ms2, BYTES_APROD2) if ms2 >= ms1 else ("aprod1", gb1, ms1, BYTES_APROD1)
-        traffic = NCU_TRAFFIC_PER_ROW[dom[0]] * m
+        gb3, gb4 = BYTES_FUSED * m / ms3 * 1e-6, BYTES_INSTR * m / ms4 * 1e-6
+        if args.two_pass:
+            dom = ("aprod2", gb2, ms2, BYTES_APROD2) if ms2 >= ms1 else ("aprod1", gb1, ms1, BYTES_APROD1)
+        else:
+            dom = ("fused", gb3, ms3, BYTES_FUSED)
+        tpr = NCU_TRAFFIC_PER_ROW[dom[0]]
+        traffic = tpr * m if tpr is not None else None
         line = {
             "metric": METRIC, "value": world * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
             "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True,
@@ -304,6 +318,8 @@ def main():
             "config": {"workload": cfg0.name, "rows": m, "cols": n, "stars": cfg.n_stars,
                        "knots_per_axis": cfg.n_dfa, "instr_cols": cfg.n_instr,
                        "preconditioned": True, "mode": "fixed-count (GSR_OPT_FORCE_ITNLIM)",
+                       "iteration": "two-pass (aprod1 + aprod2)" if args.two_pass else
+                                    "fused (one read of the matrix per iteration + instrumental pass)",
                        "l2": "matrix (%.1f GB) is far larger than L2; no flush needed" % (224e-9 * m)
                              if 224 * m > 1e9 else "matrix fits in or near L2: L2-assisted numbers",
                        "parallelism": "replicas" if world > 1 else "single"},
@@ -315,16 +331,23 @@ def main():
             "roofline": {"bound": "hbm", "kernel": dom[0], "achieved": dom[1], "peak": peak,
                          "unit": "GB/s", "frac": dom[1] / peak, "traffic": traffic,
                          "traffic_note": "DRAM bytes per launch: ncu --set full bytes per row "
-                                         "(profiles/r1_v2_aprod_ncu_full.md) x rows of this launch; the "
+                                         "(profiles/r1_v3_fused_ncu_full.md, r1_v2_aprod_ncu_full.md) x rows of this launch; the "
                                          "layout stores 212 B/row, so traffic < algorithmic bytes",
                          "peak_source": peak_src, "algorithmic_bytes_per_row": dom[3],
                          "ms_per_launch": dom[2]},
             "products": {"aprod1_gbs": gb1, "aprod2_gbs": gb2, "aprod1_ms": ms1, "aprod2_ms": ms2,
+                         "fused_ms": ms3, "fused_gbs": gb3, "instr_pass_ms": ms4, "instr_pass_gbs": gb4,
+                         "fused_plus_instr_gbs": (BYTES_APROD1 + BYTES_APROD2) * m / (ms3 + ms4) * 1e-6,
                          "aprod1_actual_gbs": TRAFFIC_APROD1 * m / ms1 * 1e-6,
                          "aprod2_actual_gbs": TRAFFIC_APROD2 * m / ms2 * 1e-6,
                          "combined_gbs": gb12, "combined_frac_of_measured": gb12 / peak,
                          "combined_frac_of_8tbs": gb12 / 8000.0,
-                         "iteration_gbs": 472 * m / (ms / K) * 1e-6},
+                         "iteration_gbs": 472 * m / (ms / K) * 1e-6,
+                         "iteration_frac_of_measured": 472 * m / (ms / K) * 1e-6 / peak,
+                         "iteration_frac_of_8tbs": 472 * m / (ms / K) * 1e-6 / 8000.0,
+                         "note": "GB/s are algorithmic (240 / 232 B per row per product, 472 per "
+                                 "iteration); the fused iteration reads the 212 B/row matrix once, so "
+                                 "its DRAM traffic is about 300 B/row"},
             "lsqr": {"istop": res.istop, "itn": res.itn, "rnorm": res.rnorm, "anorm": res.anorm,
                      "acond": res.acond, "xnorm": res.xnorm, "istop_natural": res.istop_natural,
                      "itn_natural": res.itn_natural},

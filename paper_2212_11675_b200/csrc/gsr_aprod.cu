@@ -476,17 +476,21 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
 }
 
 // Instrumental block of A^T u (row a7) over the instrumental planes only (1920 B per tile):
-// CTA-shared shared-memory accumulators, six fp64 shared atomicAdds per row.
+// shared-memory accumulators, six fp64 shared atomicAdds per row.  `ncopy` = 1: one accumulator
+// per CTA; `ncopy` = NWARP (small I): one private copy per warp, so that only lanes of the same
+// instruction ever contend for an address (config 4: 60 columns).
 __global__ void __launch_bounds__(TPB) k_aprod2_instr(const unsigned char* __restrict__ tiles,
                                                      int64_t n_tiles, const double* __restrict__ y,
-                                                     double* __restrict__ xins, int I,
+                                                     double* __restrict__ xins, int I, int ncopy,
                                                      const int* __restrict__ stop) {
     if (stop && *stop) return;
     extern __shared__ double sm[];
-    for (int i = threadIdx.x; i < I; i += TPB) sm[i] = 0.0;
+    const int ipad = (I + 1) & ~1;
+    for (int i = threadIdx.x; i < ipad * ncopy; i += TPB) sm[i] = 0.0;
     __syncthreads();
-    const int lane = threadIdx.x & 31;
-    const int64_t w0 = (int64_t)blockIdx.x * NWARP + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double* acc = sm + (ncopy > 1 ? warp * ipad : 0);
+    const int64_t w0 = (int64_t)blockIdx.x * NWARP + warp;
     const int64_t nw = (int64_t)gridDim.x * NWARP;
     for (int64_t tile = w0; tile < n_tiles; tile += nw) {
         const unsigned char* T = tiles + tile * TILE_BYTES;
@@ -498,13 +502,21 @@ __global__ void __launch_bounds__(TPB) k_aprod2_instr(const unsigned char* __res
         for (int k = 0; k < 6; ++k) v[k] = ld_stream_f64(T + OFF_INSTRV + (k * R + lane) * 8);
         const double yv = __ldcs(y + tile * R + lane);
 #pragma unroll
-        for (int k = 0; k < 6; ++k) atomicAdd(sm + c[k], v[k] * yv);
+        for (int k = 0; k < 6; ++k) atomicAdd(acc + c[k], v[k] * yv);
     }
     __syncthreads();
     for (int i = threadIdx.x; i < I; i += TPB) {
-        const double vacc = sm[i];
+        double vacc = 0.0;
+        for (int w = 0; w < ncopy; ++w) vacc += sm[w * ipad + i];
         if (vacc != 0.0) atomicAdd(xins + i, vacc);
     }
+}
+
+static int instr_copies(const gsr_matrix* A) {
+    return ((A->dims.n_instr + 1) / 2 * 16) * NWARP <= 96 * 1024 ? NWARP : 1;
+}
+static size_t instr_smem(const gsr_matrix* A) {
+    return (size_t)((A->dims.n_instr + 1) / 2 * 16) * instr_copies(A);
 }
 
 template <typename K>
@@ -532,7 +544,7 @@ int configure_product_kernels(gsr_matrix* A) {
     GSR_TRY(set_smem(k_aprod2<false, true>, b));
     GSR_TRY(set_smem(k_aprod2<true, false>, b));
     GSR_TRY(set_smem(k_fused, A->smem_fused));
-    GSR_TRY(set_smem(k_aprod2_instr, (int)((A->dims.n_instr + 1) / 2 * 16)));
+    GSR_TRY(set_smem(k_aprod2_instr, (int)instr_smem(A)));
     {
         int nb = 1;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_fused, TPB, A->smem_fused) != cudaSuccess || nb < 1) {
@@ -541,8 +553,7 @@ int configure_product_kernels(gsr_matrix* A) {
         }
         A->grid_fused = A->sm_count * nb;
         nb = 1;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_aprod2_instr, TPB,
-                                                          (size_t)((A->dims.n_instr + 1) / 2 * 16)) != cudaSuccess || nb < 1) {
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_aprod2_instr, TPB, instr_smem(A)) != cudaSuccess || nb < 1) {
             cudaGetLastError();
             nb = 1;
         }
@@ -616,8 +627,8 @@ int launch_fused(const gsr_matrix* A, const double* v, double* u, const double* 
 int launch_aprod2_instr(const gsr_matrix* A, const double* u, double* t, const int* stop,
                         cudaStream_t s) {
     if (A->n_tiles == 0) return GSR_OK;
-    k_aprod2_instr<<<A->grid_instr, TPB, (size_t)((A->dims.n_instr + 1) / 2 * 16), s>>>(
-        A->tiles, A->n_tiles, u, t + A->off_instr, (int)A->dims.n_instr, stop);
+    k_aprod2_instr<<<A->grid_instr, TPB, instr_smem(A), s>>>(
+        A->tiles, A->n_tiles, u, t + A->off_instr, (int)A->dims.n_instr, instr_copies(A), stop);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;
