@@ -48,7 +48,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="cfg3")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--oracle-rows", type=int, default=1 << 21)
+    ap.add_argument("--oracle-rows", type=int, default=1 << 22)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--two-pass", action="store_true",
                     help="GSR_OPT_FUSED = 0: aprod1 + aprod2 per iteration (two reads of the matrix)")
@@ -356,7 +356,7 @@ def main():
         if world == 1 and not args.no_cpu_baseline:
             from oracle import gsr_oracle
             gsr_oracle.build()
-            line["cpu_baseline"] = oracle_sample(cfg0, args.oracle_rows, 12)
+            line["cpu_baseline"] = oracle_sample(cfg0, args.oracle_rows, 20)
         print(json.dumps(line), flush=True)
     g.gsr_matrix_destroy(h)
     if world > 1:

@@ -131,6 +131,14 @@ int gsr_precondition(gsr_matrix* A, double* p_out_hd, gsr_stream stream);
 int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnlim, double atol,
                    double btol, double conlim, gsr_lsqr_result* result, gsr_stream stream);
 
+/* Standard errors of the unknowns of the LAST gsr_lsqr_solve on this handle ("Variances ...
+ * computation", Algorithm 3 line 17; "the standard errors" are re-multiplied by p
+ * like the solution).  The paper prints no formula; this is Paige & Saunders':
+ * var_j = sum over the iterations of (w_j / rho)^2, accumulated inside the fused vector update,
+ * se_j = p_j * rnorm * sqrt(var_j / max(m - n, 1)).  se_hd [n_cols], host or device.
+ * GSR_ESTATE if no solve has finished on the handle.  Synchronises if se_hd is host memory. */
+int gsr_lsqr_standard_errors(gsr_matrix* A, double* se_hd, gsr_stream stream);
+
 /* Options (per handle). */
 enum {
     GSR_OPT_FORCE_ITNLIM = 1, /* 1: rules 1-6 are evaluated and recorded in *_natural but only

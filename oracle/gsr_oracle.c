@@ -23,8 +23,10 @@
  * adjoint identity, dense lstsq / normal equations on tiny systems, Krylov-subspace
  * minimiser at fixed k, consistent-system recovery, block-diagonal per-star 5x5 solves,
  * unit column norms, scipy.sparse.linalg.lsqr as a black box.
- * parity unpinned: the authors' own "modified" LSQR, variances/covariances, constraints
- * (PAPER.md:27, 65, 67 give no formula) -- not implemented here.
+ * Standard errors (row f1): Paige & Saunders' var_j = sum_k (w_j/rho_k)^2, pinned by
+ * diag((A^T A)^-1) on tiny systems run to finite termination.
+ * parity unpinned: the authors' own "modified" LSQR and their variance formula, covariances,
+ * constraints (PAPER.md:27, 65, 67 give no formula) -- covariances / constraints not implemented.
  */
 #include <math.h>
 #include <stdint.h>
@@ -189,11 +191,16 @@ static double hyp(double a, double b) { return sqrt(a * a + b * b); } /* reading
  * force_itnlim != 0 (reading A9): rules 1-6 are evaluated and recorded in *_natural but only
  * the iteration limit ends the loop.  hist (may be NULL) receives per iteration
  * [rnorm, arnorm, anorm, acond, xnorm, alpha, beta] (7 doubles each, itnlim rows). */
-int orc_lsqr(const orc_dims* d, const int32_t* star_idx, const int32_t* att_start,
-             const int32_t* instr_col, const double* A_d, const double* b, double* x,
-             int64_t itnlim, double atol, double btol, double conlim, int force_itnlim,
-             orc_result* res, double* hist) {
+/* var (may be NULL): on return var[j] = sum over the iterations of (w_j / rho)^2, the LSQR
+ * estimate of diag((A^T A)^-1) from which standard errors follow ("Variances ... computation",
+ * Algorithm 3 line 17; the paper gives no formula: Paige & Saunders' one). */
+int orc_lsqr_var(const orc_dims* d, const int32_t* star_idx, const int32_t* att_start,
+                 const int32_t* instr_col, const double* A_d, const double* b, double* x,
+                 int64_t itnlim, double atol, double btol, double conlim, int force_itnlim,
+                 orc_result* res, double* hist, double* var) {
     const int64_t m = d->n_rows, n = n_cols(d);
+    if (var)
+        for (int64_t j = 0; j < n_cols(d); ++j) var[j] = 0.0;
     double* u = (double*)malloc(sizeof(double) * (size_t)(m > 0 ? m : 1));
     double* v = (double*)calloc((size_t)n, sizeof(double));
     double* w = (double*)malloc(sizeof(double) * (size_t)n);
@@ -250,6 +257,11 @@ int orc_lsqr(const orc_dims* d, const int32_t* star_idx, const int32_t* att_star
         /* update x and w */
         double t1 = phi / rho, t2 = -theta / rho;
         ddnorm = ddnorm + sumsq(w, n) / (rho * rho); /* reading A10 */
+        if (var)
+            for (int64_t j = 0; j < n; ++j) {
+                double dk = w[j] / rho;
+                var[j] = var[j] + dk * dk;
+            }
         for (int64_t j = 0; j < n; ++j) {
             x[j] = x[j] + t1 * w[j];
             w[j] = v[j] + t2 * w[j];
@@ -309,6 +321,26 @@ done_trivial:
     res->itn = 0;
     free(u); free(v); free(w);
     return 0;
+}
+
+int orc_lsqr(const orc_dims* d, const int32_t* star_idx, const int32_t* att_start,
+             const int32_t* instr_col, const double* A_d, const double* b, double* x,
+             int64_t itnlim, double atol, double btol, double conlim, int force_itnlim,
+             orc_result* res, double* hist) {
+    return orc_lsqr_var(d, star_idx, att_start, instr_col, A_d, b, x, itnlim, atol, btol, conlim,
+                        force_itnlim, res, hist, NULL);
+}
+
+/* Standard errors of the unknowns (Paige & Saunders): se_j = rnorm * sqrt(var_j / dof),
+ * dof = m - n if m > n, else 1; for a column-scaled system multiplied by p_j like the solution
+ * ("also ... the standard errors").  p may be NULL. */
+void orc_standard_errors(int64_t m, int64_t n, double rnorm, const double* var, const double* p,
+                         double* se) {
+    const double dof = m > n ? (double)(m - n) : 1.0;
+    for (int64_t j = 0; j < n; ++j) {
+        double e = rnorm * sqrt(var[j] / dof);
+        se[j] = p ? p[j] * e : e;
+    }
 }
 
 /* x = p (.) z : "we re-multiply the solution ... by the preconditioning vector p" */

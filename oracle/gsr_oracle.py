@@ -55,6 +55,8 @@ class LsqrResult:
     xnorm: float
     bnorm: float
     hist: np.ndarray | None = None
+    var: np.ndarray | None = None      # sum_k (w_j/rho_k)^2 of the iterated (scaled) system
+    se: np.ndarray | None = None       # standard errors of x (multiplied by p when scaled)
 
 
 _lib = None
@@ -66,6 +68,7 @@ def lib():
         _lib = C.CDLL(build())
         _lib.orc_validate.restype = C.c_int
         _lib.orc_lsqr.restype = C.c_int
+        _lib.orc_lsqr_var.restype = C.c_int
     return _lib
 
 
@@ -138,24 +141,31 @@ class OracleSystem:
         return p
 
     def lsqr(self, b, itnlim, atol=0.0, btol=0.0, conlim=0.0, force_itnlim=False,
-             want_hist=False) -> LsqrResult:
+             want_hist=False, want_se=False) -> LsqrResult:
         """min ||A x - b||.  If preconditioned, iterates on A.diag(p), returns x = p (.) z."""
         b = np.ascontiguousarray(b, dtype=np.float64)
         assert b.shape == (self.m,)
         x = np.empty(self.n)
         res = _Result()
         hist = np.zeros((int(itnlim), 7)) if want_hist else None
-        rc = lib().orc_lsqr(*self._idx(), _p(self.values, C.c_double), _p(b, C.c_double),
-                            _p(x, C.c_double), C.c_int64(itnlim), C.c_double(atol),
-                            C.c_double(btol), C.c_double(conlim), C.c_int(1 if force_itnlim else 0),
-                            C.byref(res), _p(hist, C.c_double))
+        var = np.zeros(self.n) if want_se else None
+        rc = lib().orc_lsqr_var(*self._idx(), _p(self.values, C.c_double), _p(b, C.c_double),
+                                _p(x, C.c_double), C.c_int64(itnlim), C.c_double(atol),
+                                C.c_double(btol), C.c_double(conlim),
+                                C.c_int(1 if force_itnlim else 0), C.byref(res),
+                                _p(hist, C.c_double), _p(var, C.c_double))
         assert rc == 0
+        se = None
+        if want_se:
+            se = np.empty(self.n)
+            lib().orc_standard_errors(C.c_int64(self.m), C.c_int64(self.n), C.c_double(res.rnorm),
+                                      _p(var, C.c_double), _p(self.p, C.c_double), _p(se, C.c_double))
         if self.p is not None:
             lib().orc_unscale(C.c_int64(self.n), _p(self.p, C.c_double), _p(x, C.c_double))
         if hist is not None:
             hist = hist[:res.itn]
         return LsqrResult(x, res.istop, res.itn, res.istop_natural, res.itn_natural, res.rnorm,
-                          res.arnorm, res.anorm, res.acond, res.xnorm, res.bnorm, hist)
+                          res.arnorm, res.anorm, res.acond, res.xnorm, res.bnorm, hist, var, se)
 
 
 def from_torch(cfg, star, att, instr, vals) -> OracleSystem:

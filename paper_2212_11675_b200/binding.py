@@ -20,7 +20,7 @@ EXPORTS = [
     "gsr_matrix_create", "gsr_matrix_begin", "gsr_matrix_append_rows", "gsr_matrix_finalize",
     "gsr_matrix_destroy", "gsr_matrix_dims", "gsr_matrix_device_bytes", "gsr_aprod1",
     "gsr_aprod2", "gsr_precondition", "gsr_lsqr_solve", "gsr_set_option", "gsr_strerror",
-    "gsr_debug_expand_rows", "gsr_time_product", "gsr_launch_count",
+    "gsr_debug_expand_rows", "gsr_time_product", "gsr_launch_count", "gsr_lsqr_standard_errors",
 ]
 
 
@@ -81,6 +81,7 @@ def lib():
         L.gsr_aprod2.argtypes = [vp, vp, vp, vp]
         L.gsr_precondition.argtypes = [vp, vp, vp]
         L.gsr_lsqr_solve.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl, C.POINTER(gsr_lsqr_result), vp]
+        L.gsr_lsqr_standard_errors.argtypes = [vp, vp, vp]
         L.gsr_set_option.argtypes = [vp, C.c_int, i64]
         L.gsr_strerror.argtypes = [C.c_int]
         L.gsr_strerror.restype = C.c_char_p
@@ -187,6 +188,10 @@ def gsr_lsqr_solve(h, b, x, itnlim, atol=0.0, btol=0.0, conlim=0.0, stream=None)
                                 float(conlim), C.byref(r), _stream(stream)), "gsr_lsqr_solve")
     return LsqrResult(r.istop, r.itn, r.istop_natural, r.itn_natural, r.rnorm, r.arnorm, r.anorm,
                       r.acond, r.xnorm, r.bnorm)
+
+
+def gsr_lsqr_standard_errors(h, se, stream=None):
+    _check(lib().gsr_lsqr_standard_errors(h, _ptr(se), _stream(stream)), "gsr_lsqr_standard_errors")
 
 
 def gsr_set_option(h, key, value):

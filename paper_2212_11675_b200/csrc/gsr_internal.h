@@ -89,6 +89,7 @@ struct LsqrState {
     double vscale;     // prescale: v <- vscale * v              (-beta)
     double inv_alpha;  // update: v <- v * inv_alpha
     double t1, t2;     // update: x += t1 w ; w = v + t2 w
+    double inv_rho;    // update: var += (w * inv_rho)^2
     // controls
     double atol, btol, ctol;
     long long itn, itnlim, itn_nat;
@@ -101,6 +102,9 @@ struct Workspace {
     double* w = nullptr;        // [n]
     double* x = nullptr;        // [n]  iterate z of the (scaled) system
     double* t = nullptr;        // [n]  A^T u_hat of the fused pass (zero between iterations)
+    double* var = nullptr;      // [n]  sum over the iterations of (w_j / rho)^2 (row f1)
+    bool solved = false;        // var / last_rnorm belong to a finished solve
+    double last_rnorm = 0.0;
     double* part_u = nullptr;   // [max(n_units, NB_N)] per-unit partial sums of u_hat^2
     double* part_v = nullptr;   // [NB_N]
     double* part_w = nullptr;   // [NB_N]

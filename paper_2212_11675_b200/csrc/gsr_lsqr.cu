@@ -113,10 +113,11 @@ template <bool INIT>
 __global__ void __launch_bounds__(TB_N) k_update(double* __restrict__ v, double* __restrict__ w,
                                                  double* __restrict__ x, int64_t len,
                                                  const LsqrState* __restrict__ st,
-                                                 double* __restrict__ part_w, double* __restrict__ tz) {
+                                                 double* __restrict__ part_w, double* __restrict__ tz,
+                                                 double* __restrict__ var) {
     if (st->stop) return;
     __shared__ double red[TB_N / 32];
-    const double ia = st->inv_alpha, t1 = st->t1, t2 = st->t2;
+    const double ia = st->inv_alpha, t1 = st->t1, t2 = st->t2, ir = st->inv_rho;
     double q = 0.0;
     for (int64_t i = (int64_t)blockIdx.x * TB_N + threadIdx.x; i < len; i += (int64_t)gridDim.x * TB_N) {
         double vn = v[i] * ia;
@@ -126,6 +127,8 @@ __global__ void __launch_bounds__(TB_N) k_update(double* __restrict__ v, double*
             wn = vn;
         } else {
             double wo = w[i];
+            const double dk = wo * ir;          // var_j += (w_j / rho)^2  (row f1)
+            var[i] = fma(dk, dk, var[i]);
             x[i] = fma(t1, wo, x[i]);
             wn = fma(t2, wo, vn);
         }
@@ -142,6 +145,16 @@ __global__ void k_finalize_x(const double* __restrict__ z, const double* __restr
                              double* __restrict__ out, int64_t len) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < len) out[i] = p ? p[i] * z[i] : z[i];
+}
+
+// se_j = p_j * rnorm * sqrt(var_j / dof)   (row f1; Paige & Saunders' standard errors, scaled
+// back by p like the solution)
+__global__ void k_standard_errors(const double* __restrict__ var, const double* __restrict__ p,
+                                  double rnorm, double dof, double* __restrict__ out, int64_t len) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= len) return;
+    const double e = rnorm * sqrt(var[i] / dof);
+    out[i] = p ? p[i] * e : e;
 }
 
 // ---- scalar kernels (rows a4, a9): one CTA, deterministic second-stage sums, then one
@@ -239,6 +252,7 @@ __global__ void __launch_bounds__(1024) k_scalar_main(LsqrState* __restrict__ st
     const double tau = sn * phi;
     st->t1 = phi / rho;
     st->t2 = -theta / rho;
+    st->inv_rho = 1.0 / rho;
     st->ddnorm = st->ddnorm + ssw / (rho * rho);
     // second rotation: ||x|| estimate
     const double delta = st->sn2 * rho;
@@ -302,6 +316,7 @@ int ensure_workspace(gsr_matrix* A) {
     GSR_TRY(dev_alloc(A, (void**)&W.w, n8));
     GSR_TRY(dev_alloc(A, (void**)&W.x, n8));
     GSR_TRY(dev_alloc(A, (void**)&W.t, n8));
+    GSR_TRY(dev_alloc(A, (void**)&W.var, n8));
     GSR_TRY(dev_alloc(A, (void**)&W.part_u, (size_t)npu * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.part_v, NB_N * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.part_w, NB_N * 8));
@@ -315,7 +330,7 @@ int ensure_workspace(gsr_matrix* A) {
 void free_workspace(gsr_matrix* A) {
     Workspace& W = A->ws;
     if (W.graph) cudaGraphExecDestroy(W.graph);
-    cudaFree(W.u); cudaFree(W.v); cudaFree(W.w); cudaFree(W.x); cudaFree(W.t);
+    cudaFree(W.u); cudaFree(W.v); cudaFree(W.w); cudaFree(W.x); cudaFree(W.t); cudaFree(W.var);
     cudaFree(W.part_u); cudaFree(W.part_v); cudaFree(W.part_w);
     cudaFree(W.stage_m); cudaFree(W.stage_n); cudaFree(W.st);
     if (W.stop_host) cudaFreeHost(W.stop_host);
@@ -342,14 +357,14 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
         GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s));
         k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop);
         k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N);
-        k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, nullptr);
+        k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, nullptr, W.var);
     } else {
         GSR_TRY(launch_fused(A, W.v, W.u, &W.st->ca, W.part_u, W.t, &W.st->stop, s));
         GSR_TRY(launch_aprod2_instr(A, W.u, W.t, &W.st->stop, s));
         k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_units);
         k_vnew<<<NB_N, TB_N, 0, s>>>(W.v, W.t, n, W.st, W.part_v);
         k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N);
-        k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, W.t);
+        k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, W.t, W.var);
     }
     k_raise_stop<<<1, 1, 0, s>>>(W.st);
     GSR_CUDA_TRY(cudaGetLastError());
@@ -433,6 +448,8 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     GSR_CUDA_TRY(cudaMemcpyAsync(W.st, &h, sizeof(h), cudaMemcpyHostToDevice, s));
     GSR_CUDA_TRY(cudaMemsetAsync(W.v, 0, (size_t)n * 8, s));
     GSR_CUDA_TRY(cudaMemsetAsync(W.x, 0, (size_t)n * 8, s));
+    GSR_CUDA_TRY(cudaMemsetAsync(W.var, 0, (size_t)n * 8, s));
+    W.solved = false;
     // initialisation (row a2): u_hat = b, beta_1, v = A^T u, alpha_1, w = v
     k_gather_sumsq<<<NB_N, TB_N, 0, s>>>(b_dev, A->perm, W.u, A->m_int, W.part_u);
     k_scalar_init1<<<1, 1024, 0, s>>>(W.st, W.part_u, NB_N);
@@ -440,7 +457,7 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s));
     k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop);
     k_scalar_init2<<<1, 1024, 0, s>>>(W.st, W.part_v, NB_N);
-    k_update<true><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, nullptr);
+    k_update<true><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, nullptr, nullptr);
     GSR_CUDA_TRY(cudaMemsetAsync(W.t, 0, (size_t)n * 8, s));
     count_launch(3);
     GSR_CUDA_TRY(cudaGetLastError());
@@ -482,6 +499,31 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     result->xnorm = h.xnorm;
     result->bnorm = h.bnorm;
     if (result->istop_natural == 0 && h.istop != 7) result->istop_natural = h.istop;
+    W.solved = true;
+    W.last_rnorm = h.rnorm;
+    return GSR_OK;
+}
+
+int gsr_lsqr_standard_errors(gsr_matrix* A, double* se_hd, gsr_stream stream) {
+    if (!A || !se_hd) return GSR_EINVAL;
+    Workspace& W = A->ws;
+    if (A->state != 1 || !W.solved) return GSR_ESTATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    const int64_t m = A->dims.n_rows, n = A->n_cols;
+    const bool dev = is_device_ptr(se_hd);
+    double* out = se_hd;
+    if (!dev) {
+        if (!W.stage_n) GSR_TRY(dev_alloc(A, (void**)&W.stage_n, (size_t)n * 8));
+        out = W.stage_n;
+    }
+    const double dof = m > n ? (double)(m - n) : 1.0;
+    k_standard_errors<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(W.var, A->p, W.last_rnorm, dof, out, n);
+    count_launch();
+    GSR_CUDA_TRY(cudaGetLastError());
+    if (!dev) {
+        GSR_CUDA_TRY(cudaMemcpyAsync(se_hd, out, (size_t)n * 8, cudaMemcpyDeviceToHost, s));
+        GSR_CUDA_TRY(cudaStreamSynchronize(s));
+    }
     return GSR_OK;
 }
 

@@ -144,18 +144,38 @@ def test_precondition_and_lsqr_parity(name, fused):
         rhs_ulp = rhs + np.spacing(rhs) * rng.integers(-1, 2, rhs.shape)
         for k in FIXED_COUNTS[name]:
             r = b.gsr_lsqr_solve(s.A.h, bd, x, k)
-            ro = s.o.lsqr(rhs, k, force_itnlim=True)
+            ro = s.o.lsqr(rhs, k, force_itnlim=True, want_se=True)
             assert (r.istop, r.itn) == (ro.istop, ro.itn) == (7, k)
             xg = x.cpu().numpy()
+            se = torch.empty(s.n, dtype=torch.float64, device="cuda")
+            b.gsr_lsqr_standard_errors(s.A.h, se)      # row f1: p * rnorm * sqrt(var / dof)
+            se_host = np.empty(s.n)
+            b.gsr_lsqr_standard_errors(s.A.h, se_host)
+            assert np.array_equal(se.cpu().numpy(), se_host)
             # Reading A20: at some intermediate k the Lanczos process is unstable (the oracle
             # itself moves by far more than 1e-9 when b changes by one ulp).  The bar is 1e-9
             # wherever the oracle is that stable, else 20x the oracle's own one-ulp sensitivity.
-            sens = np.linalg.norm(s.o.lsqr(rhs_ulp, k, force_itnlim=True).x - ro.x) / np.linalg.norm(ro.x)
+            ru = s.o.lsqr(rhs_ulp, k, force_itnlim=True, want_se=True)
+            sens = np.linalg.norm(ru.x - ro.x) / np.linalg.norm(ro.x)
+            sens_se = np.linalg.norm(ru.se - ro.se) / np.linalg.norm(ro.se)
             tol = max(X_TOL, 20.0 * sens)
             if k in STABLE_COUNTS[name]:
                 assert sens < 1e-10 and tol == X_TOL, (name, k, sens)
             assert np.linalg.norm(xg - ro.x) <= tol * np.linalg.norm(ro.x), (name, k, sens)
             assert abs(r.rnorm - ro.rnorm) <= tol * ro.rnorm
+            # var is a sum of squares of the w vectors.  Before the first natural stop rule fires
+            # it is as stable as x; past convergence the Lanczos vectors are rounding noise
+            # (reading A18) and the terms (w_j/rho)^2 added from then on are arbitrary on both
+            # sides (measured: oracle and GPU differ by O(1) at k = 60 on a system that
+            # converged at k = 38), so var is compared only up to convergence.
+            converged = ro.itn_natural != 0 and k >= ro.itn_natural
+            nz = ro.se > 0
+            assert np.all(np.isfinite(se_host)) and np.all(se_host[~nz] == 0.0)
+            if not converged:
+                se_tol = max(2 * tol, 20.0 * sens_se)    # same rule as for x (reading A20)
+                assert np.linalg.norm(se_host - ro.se) <= se_tol * np.linalg.norm(ro.se), (name, k, sens_se)
+                if tol == X_TOL:
+                    assert np.all(np.abs(se_host[nz] - ro.se[nz]) <= 1e-7 * ro.se[nz])
             assert abs(r.xnorm - ro.xnorm) <= tol * ro.xnorm
             assert abs(r.bnorm - ro.bnorm) <= 1e-12 * ro.bnorm
             if tol == X_TOL and (ro.itn_natural == 0 or k < ro.itn_natural):      # reading A18
@@ -171,6 +191,13 @@ def test_precondition_and_lsqr_parity(name, fused):
         ro = s.o.lsqr(rhs, 500, 1e-10, 1e-10, 1e8)
         assert r.istop == ro.istop and abs(r.itn - ro.itn) <= 1
         assert np.linalg.norm(x.cpu().numpy() - ro.x) <= X_TOL * np.linalg.norm(ro.x)
+        if r.itn == ro.itn:     # standard errors at the natural stop (row f1)
+            ro = s.o.lsqr(rhs, 500, 1e-10, 1e-10, 1e8, want_se=True)
+            se_host = np.empty(s.n)
+            b.gsr_lsqr_standard_errors(s.A.h, se_host)
+            # the last terms before the stop already come from nearly converged Lanczos vectors
+            # (measured 4e-4 on ragged_empty_stars): an estimate-level agreement, like anorm
+            assert np.linalg.norm(se_host - ro.se) <= 1e-2 * np.linalg.norm(ro.se), name
     finally:
         s.A.close()
 
@@ -191,6 +218,18 @@ def test_lsqr_unpreconditioned_host_buffers():
         xp = torch.empty(s.n, dtype=torch.float64).pin_memory()
         b.gsr_lsqr_solve(s.A.h, bp, xp, 4)                # pinned host tensors
         assert np.linalg.norm(xp.numpy() - xh) <= 1e-11 * np.linalg.norm(xh)   # atomics: order varies
+    finally:
+        s.A.close()
+
+
+def test_standard_errors_need_a_solve():
+    b = _binding()
+    s = Sys(CASES["cfg1"])
+    try:
+        se = torch.empty(s.n, dtype=torch.float64, device="cuda")
+        with pytest.raises(b.GsrError) as ei:
+            b.gsr_lsqr_standard_errors(s.A.h, se)
+        assert ei.value.code == b.GSR_ESTATE
     finally:
         s.A.close()
 

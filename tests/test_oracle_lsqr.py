@@ -200,3 +200,59 @@ def test_scipy_lsqr_black_box(precond):
     rk = o.lsqr(b, k, force_itnlim=True)
     assert ref[2] == k and rk.itn == k and rk.istop == 7 and ref[1] == 7
     assert np.linalg.norm(rk.x - xk) <= 1e-10 * np.linalg.norm(xk)
+
+
+# ---- row f1: variances / standard errors (Paige & Saunders; Algorithm 3 line 17)
+
+def _krylov_basis(A, b, k):
+    """Orthonormal basis of span{A^T b, (A^T A) A^T b, ...} by dense Gram-Schmidt (twice)."""
+    n = A.shape[1]
+    Q = np.zeros((n, k))
+    v = A.T @ b
+    for i in range(k):
+        for _ in range(2):
+            v = v - Q[:, :i] @ (Q[:, :i].T @ v)
+        v = v / np.linalg.norm(v)
+        Q[:, i] = v
+        v = A.T @ (A @ v)
+    return Q
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 5, 8, 10])
+def test_variance_is_diag_of_projected_inverse_normal_matrix(k):
+    """After k steps LSQR's var_j = sum (w_j/rho)^2 equals diag(Q (Q^T A^T A Q)^-1 Q^T) with Q an
+    orthonormal basis of the k-th Krylov space (D_k D_k^T = V_k (B_k^T B_k)^-1 V_k^T): a dense,
+    independent computation.  The standard error follows with the residual computed directly."""
+    cfg, star, att, instr, vals = small_system()
+    o = make_oracle(cfg, star, att, instr, vals)
+    A = csr_from_raw(cfg, star, att, instr, vals)[0].toarray()
+    b = np.random.default_rng(5).standard_normal(o.m)
+    r = o.lsqr(b, k, force_itnlim=True, want_se=True)
+    Q = _krylov_basis(A, b, k)
+    T = Q.T @ (A.T @ (A @ Q))
+    var_ref = np.einsum("ij,jk,ik->i", Q, np.linalg.inv(T), Q)
+    assert np.max(np.abs(r.var - var_ref)) <= 1e-11 * np.max(var_ref)
+    res = np.linalg.norm(b - A @ r.x)
+    se_ref = res * np.sqrt(var_ref / (o.m - o.n))
+    assert np.allclose(r.se, se_ref, rtol=1e-9, atol=1e-12 * se_ref.max())
+
+
+def test_variance_monotone_and_scaled_by_p():
+    """var never decreases with k; with column scaling se is multiplied by p like the solution
+    (PAPER.md:43): se(x) = p * rnorm * sqrt(var_z/dof)."""
+    cfg, star, att, instr, vals = small_system()
+    o = make_oracle(cfg, star, att, instr, vals)
+    b = np.random.default_rng(6).standard_normal(o.m)
+    prev = np.zeros(o.n)
+    for k in (1, 3, 6, 12):
+        r = o.lsqr(b, k, force_itnlim=True, want_se=True)
+        assert np.all(r.var >= prev)
+        prev = r.var
+    p = o.precondition()
+    r = o.lsqr(b, 6, force_itnlim=True, want_se=True)
+    assert np.allclose(r.se, p * r.rnorm * np.sqrt(r.var / (o.m - o.n)), rtol=1e-14)
+    # and the projected-inverse identity holds for the scaled matrix too
+    A = csr_from_raw(cfg, star, att, instr, vals)[0].toarray() * p[None, :]
+    Q = _krylov_basis(A, b, 6)
+    var_ref = np.einsum("ij,jk,ik->i", Q, np.linalg.inv(Q.T @ (A.T @ (A @ Q))), Q)
+    assert np.max(np.abs(r.var - var_ref)) <= 1e-11 * np.max(var_ref)
