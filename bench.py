@@ -52,6 +52,9 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--two-pass", action="store_true",
                     help="GSR_OPT_FUSED = 0: aprod1 + aprod2 per iteration (two reads of the matrix)")
+    ap.add_argument("--sharded", action="store_true",
+                    help="N > 1: ONE system of N x the config's rows, row-sharded over the ranks "
+                         "(NCCL all-reduce of the replicated slice inside the graph) instead of N replicas")
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE config 5: time aprod1/aprod2 alone from 1e6 to 3e8 rows")
     return ap.parse_args()
@@ -244,6 +247,19 @@ def main():
     for r0 in range(0, m, GEN_ROWS):
         nr = min(GEN_ROWS, m - r0)
         b[r0:r0 + nr] = inputs.noise(cfg, r0, nr, dev)
+    comm = None
+    if args.sharded:
+        if os.environ.get("NCCL_DEBUG", "VERSION").upper() == "VERSION":
+            os.environ["NCCL_DEBUG"] = "WARN"    # keep stdout to the one JSON line
+        # weak-scaled sharded system: rank r owns stars [r*S, (r+1)*S) of an N*S-star system; the
+        # attitude + instrumental + global unknowns are shared, so their x_true comes from rank 0's seed
+        xt0 = inputs.x_true(cfg0, dev)
+        xt[cfg.off_att:] = xt0[cfg0.off_att:]
+        uid = [g.gsr_comm_unique_id() if rank == 0 else None]
+        if world > 1:
+            dist.broadcast_object_list(uid, src=0)
+        comm = g.gsr_comm_create(rank, world, uid[0])
+        g.gsr_matrix_set_comm(h, comm, world * m, world * 5 * cfg.n_stars + (n - cfg.off_att))
     g.gsr_aprod1(h, xt, b)
     g.gsr_precondition(h)
     g.gsr_set_option(h, g.GSR_OPT_FORCE_ITNLIM, 1)
@@ -322,7 +338,8 @@ def main():
                                     "fused (one read of the matrix per iteration + instrumental pass)",
                        "l2": "matrix (%.1f GB) is far larger than L2; no flush needed" % (224e-9 * m)
                              if 224 * m > 1e9 else "matrix fits in or near L2: L2-assisted numbers",
-                       "parallelism": "replicas" if world > 1 else "single"},
+                       "parallelism": ("row-sharded x%d (NCCL all-reduce of the replicated slice)" % world
+                                       if args.sharded else "replicas" if world > 1 else "single")},
             "e2e": {"value": world * K / (ms_e2e * 1e-3), "unit": UNIT,
                     "h2d_bytes_per_step": 8 * m / K, "d2h_bytes_per_step": (8 * n + 80) / K,
                     "note": "gsr_lsqr_solve with pinned host b and host x; matrix resident"},
@@ -359,6 +376,8 @@ def main():
             line["cpu_baseline"] = oracle_sample(cfg0, args.oracle_rows, 20)
         print(json.dumps(line), flush=True)
     g.gsr_matrix_destroy(h)
+    if comm:
+        g.gsr_comm_destroy(comm)
     if world > 1:
         dist.destroy_process_group()
 

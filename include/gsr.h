@@ -40,6 +40,7 @@ extern "C" {
 #endif
 
 typedef struct gsr_matrix gsr_matrix; /* opaque, library-owned */
+typedef struct gsr_comm gsr_comm;     /* opaque: one rank of a row-sharded solve (NCCL) */
 typedef void* gsr_stream;             /* cudaStream_t */
 
 typedef enum {
@@ -138,6 +139,28 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
  * se_j = p_j * rnorm * sqrt(var_j / max(m - n, 1)).  se_hd [n_cols], host or device.
  * GSR_ESTATE if no solve has finished on the handle.  Synchronises if se_hd is host memory. */
 int gsr_lsqr_standard_errors(gsr_matrix* A, double* se_hd, gsr_stream stream);
+
+/* ---- row-sharded solve over several GPUs (Fig. 2; Algorithm 3 lines 8-16) --
+ * One process per GPU.  The observation rows are split into contiguous star-aligned blocks
+ * (paper_2212_11675_b200/sharding.py); every rank builds an ORDINARY matrix from its block, with
+ * its own stars renumbered from 0 and the same D and I.  The astrometric slice of every
+ * n-vector is then distributed with the rows, the attitude + instrumental + global slice
+ * (local columns [5*S_local, n_local)) is REPLICATED and summed over the ranks: the paper's
+ * MPI reduce, here one ncclAllReduce(sum, fp64) of 3D + I + 2 values per iteration (the local
+ * sum of u_hat^2 rides in the same buffer) and one of 2 scalars, both inside the CUDA graph.
+ *   gsr_comm_unique_id  rank 0: fills id_out (>= 128 bytes); the caller broadcasts it
+ *   gsr_comm_create     every rank, same id (collective: returns when all ranks have joined)
+ *   gsr_matrix_set_comm after create/finalize, before gsr_precondition and gsr_lsqr_solve;
+ *                       n_rows_global / n_cols_global are those of the whole system (standard
+ *                       errors).  comm = NULL restores the single-GPU behaviour.
+ * With a communicator gsr_precondition sums the column norms of the replicated slice over
+ * the ranks, gsr_lsqr_solve returns the local x (replicated slice identical on every rank)
+ * and the norms of the WHOLE system; only the fused iteration is supported.
+ * NCCL is loaded with dlopen (GSR_EUNSUPPORTED if libnccl.so.2 cannot be found). */
+int gsr_comm_unique_id(void* id_out, int64_t bytes);
+int gsr_comm_create(gsr_comm** out, int rank, int world, const void* id_in, int64_t bytes);
+int gsr_comm_destroy(gsr_comm* c);
+int gsr_matrix_set_comm(gsr_matrix* A, gsr_comm* c, int64_t n_rows_global, int64_t n_cols_global);
 
 /* Options (per handle). */
 enum {

@@ -21,6 +21,7 @@ EXPORTS = [
     "gsr_matrix_destroy", "gsr_matrix_dims", "gsr_matrix_device_bytes", "gsr_aprod1",
     "gsr_aprod2", "gsr_precondition", "gsr_lsqr_solve", "gsr_set_option", "gsr_strerror",
     "gsr_debug_expand_rows", "gsr_time_product", "gsr_launch_count", "gsr_lsqr_standard_errors",
+    "gsr_comm_unique_id", "gsr_comm_create", "gsr_comm_destroy", "gsr_matrix_set_comm",
 ]
 
 
@@ -82,6 +83,10 @@ def lib():
         L.gsr_precondition.argtypes = [vp, vp, vp]
         L.gsr_lsqr_solve.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl, C.POINTER(gsr_lsqr_result), vp]
         L.gsr_lsqr_standard_errors.argtypes = [vp, vp, vp]
+        L.gsr_comm_unique_id.argtypes = [vp, i64]
+        L.gsr_comm_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, vp, i64]
+        L.gsr_comm_destroy.argtypes = [vp]
+        L.gsr_matrix_set_comm.argtypes = [vp, vp, i64, i64]
         L.gsr_set_option.argtypes = [vp, C.c_int, i64]
         L.gsr_strerror.argtypes = [C.c_int]
         L.gsr_strerror.restype = C.c_char_p
@@ -192,6 +197,31 @@ def gsr_lsqr_solve(h, b, x, itnlim, atol=0.0, btol=0.0, conlim=0.0, stream=None)
 
 def gsr_lsqr_standard_errors(h, se, stream=None):
     _check(lib().gsr_lsqr_standard_errors(h, _ptr(se), _stream(stream)), "gsr_lsqr_standard_errors")
+
+
+GSR_COMM_ID_BYTES = 128
+
+
+def gsr_comm_unique_id() -> bytes:
+    """Rank 0: a fresh NCCL unique id, to be broadcast to the other ranks by the caller."""
+    buf = C.create_string_buffer(GSR_COMM_ID_BYTES)
+    _check(lib().gsr_comm_unique_id(buf, GSR_COMM_ID_BYTES), "gsr_comm_unique_id")
+    return buf.raw
+
+
+def gsr_comm_create(rank: int, world: int, unique_id: bytes) -> int:
+    c = C.c_void_p()
+    buf = C.create_string_buffer(bytes(unique_id), GSR_COMM_ID_BYTES)
+    _check(lib().gsr_comm_create(C.byref(c), int(rank), int(world), buf, GSR_COMM_ID_BYTES), "gsr_comm_create")
+    return c.value
+
+
+def gsr_comm_destroy(c):
+    _check(lib().gsr_comm_destroy(c), "gsr_comm_destroy")
+
+
+def gsr_matrix_set_comm(h, comm, n_rows_global, n_cols_global):
+    _check(lib().gsr_matrix_set_comm(h, comm, int(n_rows_global), int(n_cols_global)), "gsr_matrix_set_comm")
 
 
 def gsr_set_option(h, key, value):

@@ -106,8 +106,11 @@ struct Workspace {
     bool solved = false;        // var / last_rnorm belong to a finished solve
     double last_rnorm = 0.0;
     double* part_u = nullptr;   // [max(n_units, NB_N)] per-unit partial sums of u_hat^2
-    double* part_v = nullptr;   // [NB_N]
+    double* part_v = nullptr;   // [NB_N]  (sharded: replicated slice only)
     double* part_w = nullptr;   // [NB_N]
+    double* part_va = nullptr;  // [NB_N]  sharded: distributed (astrometric) slice of v^2 / w^2
+    double* part_wa = nullptr;  // [NB_N]
+    double* red = nullptr;      // [4] scalars that cross the ranks: sum v_a^2, sum w_a^2, sum b^2
     double* stage_m = nullptr;  // [m] staging for a host b
     double* stage_n = nullptr;  // [n] staging for a host x
     LsqrState* st = nullptr;
@@ -116,6 +119,7 @@ struct Workspace {
     cudaStream_t graph_stream = nullptr;
     bool graph_valid = false;
     int graph_two_pass = 0;
+    void* graph_comm = nullptr;
 };
 
 }  // namespace gsr
@@ -157,6 +161,8 @@ struct gsr_matrix {
     int64_t device_bytes;
     int opt_force_itnlim;
     int opt_two_pass;               // 1: aprod1 + aprod2 per iteration instead of the fused pass
+    gsr_comm* comm;                 // row e: this handle is one row shard (nullptr: whole system)
+    int64_t m_global, n_global;     // rows / columns of the whole system (= local without comm)
     int sm_count;
     gsr::Workspace ws;
 };
@@ -181,6 +187,7 @@ inline void count_launch(long long k = 1) { g_launches += k; }
         if (rc__ != GSR_OK) return rc__; \
     } while (0)
 
+int comm_allreduce_sum(gsr_comm* c, double* buf, size_t count, cudaStream_t s);
 int dev_alloc(gsr_matrix* A, void** p, size_t bytes);
 void dev_free(gsr_matrix* A, void* p, size_t bytes);
 bool is_device_ptr(const void* p);

@@ -29,6 +29,20 @@ __device__ __forceinline__ double block_sum_256(double v, double* red) {
     return t;  // valid in thread 0
 }
 
+// Row-sharded solve (row e): entries below `split` belong to the distributed (astrometric)
+// slice, whose sum of squares must still be summed over the ranks, entries from `split` on to
+// the replicated slice, counted once.  Without a communicator split = 0 and parta is unused.
+__device__ __forceinline__ void write_split_partials(double q, double qa, int64_t split, double* red,
+                                                     double* __restrict__ part, double* __restrict__ parta) {
+    q = block_sum_256(q, red);
+    if (threadIdx.x == 0) part[blockIdx.x] = q;
+    if (split > 0) {
+        __syncthreads();
+        qa = block_sum_256(qa, red);
+        if (threadIdx.x == 0) parta[blockIdx.x] = qa;
+    }
+}
+
 // Deterministic second stage: one CTA sums `np` partials in a fixed order.
 __device__ double reduce_partials_1024(const double* __restrict__ part, int64_t np, double* red) {
     double t = 0.0;
@@ -67,16 +81,27 @@ __global__ void __launch_bounds__(TB_N) k_gather_sumsq(const double* __restrict_
 }
 
 __global__ void __launch_bounds__(TB_N) k_sumsq(const double* __restrict__ v, int64_t len,
-                                                double* __restrict__ part, const int* __restrict__ stop) {
+                                                double* __restrict__ part, const int* __restrict__ stop,
+                                                int64_t split, double* __restrict__ parta) {
     if (*stop) return;
     __shared__ double red[TB_N / 32];
-    double q = 0.0;
+    double q = 0.0, qa = 0.0;
     for (int64_t i = (int64_t)blockIdx.x * TB_N + threadIdx.x; i < len; i += (int64_t)gridDim.x * TB_N) {
         double t = v[i];
-        q = fma(t, t, q);
+        if (i < split) qa = fma(t, t, qa);
+        else q = fma(t, t, q);
     }
-    q = block_sum_256(q, red);
-    if (threadIdx.x == 0) part[blockIdx.x] = q;
+    write_split_partials(q, qa, split, red, part, parta);
+}
+
+// out[0] = sum of np partials in a fixed order (one CTA); the scalar then crosses the ranks
+__global__ void __launch_bounds__(1024) k_sum_partials(const double* __restrict__ part, int64_t np,
+                                                       double* __restrict__ out,
+                                                       const int* __restrict__ stop) {
+    if (stop && *stop) return;
+    __shared__ double red[32];
+    double ss = reduce_partials_1024(part, np, red);
+    if (threadIdx.x == 0) out[0] = ss;
 }
 
 // v <- vscale * v   (v = -beta v before aprod2 adds A^T u)
@@ -92,18 +117,19 @@ __global__ void __launch_bounds__(TB_N) k_prescale(double* __restrict__ v, int64
 // partial sums of the new v squared
 __global__ void __launch_bounds__(TB_N) k_vnew(double* __restrict__ v, const double* __restrict__ t,
                                                int64_t len, const LsqrState* __restrict__ st,
-                                               double* __restrict__ part) {
+                                               double* __restrict__ part, int64_t split,
+                                               double* __restrict__ parta) {
     if (st->stop) return;
     __shared__ double red[TB_N / 32];
     const double ib = st->inv_beta, c = st->vscale;
-    double q = 0.0;
+    double q = 0.0, qa = 0.0;
     for (int64_t i = (int64_t)blockIdx.x * TB_N + threadIdx.x; i < len; i += (int64_t)gridDim.x * TB_N) {
         const double vn = fma(t[i], ib, c * v[i]);
         v[i] = vn;
-        q = fma(vn, vn, q);
+        if (i < split) qa = fma(vn, vn, qa);
+        else q = fma(vn, vn, q);
     }
-    q = block_sum_256(q, red);
-    if (threadIdx.x == 0) part[blockIdx.x] = q;
+    write_split_partials(q, qa, split, red, part, parta);
 }
 
 // fused n-sized update (row a10): v <- v*inv_alpha ; x += t1 w ; w = v + t2 w ; partials of
@@ -114,11 +140,12 @@ __global__ void __launch_bounds__(TB_N) k_update(double* __restrict__ v, double*
                                                  double* __restrict__ x, int64_t len,
                                                  const LsqrState* __restrict__ st,
                                                  double* __restrict__ part_w, double* __restrict__ tz,
-                                                 double* __restrict__ var) {
+                                                 double* __restrict__ var, int64_t split,
+                                                 double* __restrict__ part_wa) {
     if (st->stop) return;
     __shared__ double red[TB_N / 32];
     const double ia = st->inv_alpha, t1 = st->t1, t2 = st->t2, ir = st->inv_rho;
-    double q = 0.0;
+    double q = 0.0, qa = 0.0;
     for (int64_t i = (int64_t)blockIdx.x * TB_N + threadIdx.x; i < len; i += (int64_t)gridDim.x * TB_N) {
         double vn = v[i] * ia;
         v[i] = vn;
@@ -134,10 +161,10 @@ __global__ void __launch_bounds__(TB_N) k_update(double* __restrict__ v, double*
         }
         w[i] = wn;
         if (tz) tz[i] = 0.0;   // clears the accumulator of the next fused pass
-        q = fma(wn, wn, q);
+        if (i < split) qa = fma(wn, wn, qa);
+        else q = fma(wn, wn, q);
     }
-    q = block_sum_256(q, red);
-    if (threadIdx.x == 0) part_w[blockIdx.x] = q;
+    write_split_partials(q, qa, split, red, part_w, part_wa);
 }
 
 // x_out = p (.) z  ("re-multiply the solution by the preconditioning vector")
@@ -182,10 +209,12 @@ __global__ void __launch_bounds__(1024) k_scalar_init1(LsqrState* __restrict__ s
 
 // alpha_1 = ||A^T u_1||
 __global__ void __launch_bounds__(1024) k_scalar_init2(LsqrState* __restrict__ st,
-                                                       const double* __restrict__ part_v, int64_t np) {
+                                                       const double* __restrict__ part_v, int64_t np,
+                                                       const double* __restrict__ extra) {
     if (st->stop) return;
     __shared__ double red[32];
     double ss = reduce_partials_1024(part_v, np, red);
+    if (extra) ss += extra[0];   // distributed slice, already summed over the ranks
     if (threadIdx.x != 0) return;
     double alpha = sqrt(ss);
     st->alpha = alpha;
@@ -227,11 +256,16 @@ __global__ void __launch_bounds__(1024) k_scalar_beta(LsqrState* __restrict__ st
 // alpha_{k+1}, plane rotations, norms, stopping rules
 __global__ void __launch_bounds__(1024) k_scalar_main(LsqrState* __restrict__ st,
                                                       const double* __restrict__ part_v,
-                                                      const double* __restrict__ part_w, int64_t np) {
+                                                      const double* __restrict__ part_w, int64_t np,
+                                                      const double* __restrict__ extra) {
     if (st->stop) return;
     __shared__ double red[32];
     double ssv = reduce_partials_1024(part_v, np, red);
     double ssw = reduce_partials_1024(part_w, np, red);
+    if (extra) {                 // distributed slices, already summed over the ranks
+        ssv += extra[0];
+        ssw += extra[1];
+    }
     if (threadIdx.x != 0) return;
     double alpha = st->alpha;
     const double beta = st->beta;
@@ -315,11 +349,14 @@ int ensure_workspace(gsr_matrix* A) {
     GSR_TRY(dev_alloc(A, (void**)&W.v, n8));
     GSR_TRY(dev_alloc(A, (void**)&W.w, n8));
     GSR_TRY(dev_alloc(A, (void**)&W.x, n8));
-    GSR_TRY(dev_alloc(A, (void**)&W.t, n8));
+    GSR_TRY(dev_alloc(A, (void**)&W.t, n8 + 16));   // t[n]: local sum of u_hat^2 (sharded solve)
     GSR_TRY(dev_alloc(A, (void**)&W.var, n8));
     GSR_TRY(dev_alloc(A, (void**)&W.part_u, (size_t)npu * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.part_v, NB_N * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.part_w, NB_N * 8));
+    GSR_TRY(dev_alloc(A, (void**)&W.part_va, NB_N * 8));
+    GSR_TRY(dev_alloc(A, (void**)&W.part_wa, NB_N * 8));
+    GSR_TRY(dev_alloc(A, (void**)&W.red, 4 * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.st, sizeof(LsqrState)));
     GSR_CUDA_TRY(cudaMemset(W.u, 0, (size_t)A->m_int * 8));
     GSR_CUDA_TRY(cudaMemset(W.st, 0, sizeof(LsqrState)));
@@ -332,6 +369,7 @@ void free_workspace(gsr_matrix* A) {
     if (W.graph) cudaGraphExecDestroy(W.graph);
     cudaFree(W.u); cudaFree(W.v); cudaFree(W.w); cudaFree(W.x); cudaFree(W.t); cudaFree(W.var);
     cudaFree(W.part_u); cudaFree(W.part_v); cudaFree(W.part_w);
+    cudaFree(W.part_va); cudaFree(W.part_wa); cudaFree(W.red);
     cudaFree(W.stage_m); cudaFree(W.stage_n); cudaFree(W.st);
     if (W.stop_host) cudaFreeHost(W.stop_host);
     cudaGetLastError();
@@ -343,11 +381,14 @@ void free_workspace(gsr_matrix* A) {
 // Fused form (default): the matrix is read once -- k_fused produces u_hat and t = A^T u_hat
 // together, k_aprod2_instr adds the instrumental block of t, k_vnew forms v = t/beta - beta v.
 // Two-pass form (GSR_OPT_FUSED = 0): aprod1, then aprod2 on the pre-scaled v.
-static int kernels_per_iteration(const gsr_matrix* A) { return A->opt_two_pass ? 8 : 7; }
+static int kernels_per_iteration(const gsr_matrix* A) {
+    return A->opt_two_pass ? 8 : (A->comm ? 10 : 7);
+}
 
 static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
     Workspace& W = A->ws;
     const int64_t n = A->n_cols;
+    const int64_t split = A->comm ? A->off_att : 0;   // sharded: [0, split) distributed slice
     if (A->opt_two_pass) {
         // bidiagonalisation, first half: u_hat <- A v - (alpha/beta) u_hat ; partials of u_hat^2
         GSR_TRY(launch_aprod1(A, W.v, W.u, &W.st->ca, W.part_u, &W.st->stop, nullptr, s));
@@ -355,16 +396,31 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
         // second half: v <- A^T (u_hat/beta) - beta v
         k_prescale<<<NB_N, TB_N, 0, s>>>(W.v, n, W.st);
         GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s));
-        k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop);
-        k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N);
-        k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, nullptr, W.var);
-    } else {
+        k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop, 0, nullptr);
+        k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N, nullptr);
+        k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, nullptr, W.var, 0, nullptr);
+    } else if (!A->comm) {
         GSR_TRY(launch_fused(A, W.v, W.u, &W.st->ca, W.part_u, W.t, &W.st->stop, s));
         GSR_TRY(launch_aprod2_instr(A, W.u, W.t, &W.st->stop, s));
         k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_units);
-        k_vnew<<<NB_N, TB_N, 0, s>>>(W.v, W.t, n, W.st, W.part_v);
-        k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N);
-        k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, W.t, W.var);
+        k_vnew<<<NB_N, TB_N, 0, s>>>(W.v, W.t, n, W.st, W.part_v, 0, nullptr);
+        k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N, nullptr);
+        k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, W.t, W.var, 0, nullptr);
+    } else {
+        // row-sharded: the same sequence with the paper's two reductions (Alg. 3 lines 12, 16)
+        // as NCCL all-reduces inside the graph.  #1: replicated slice of t = A^T u_hat, with the
+        // local sum of u_hat^2 riding in t[n]; #2: the distributed parts of ||v||^2 and ||w||^2.
+        GSR_TRY(launch_fused(A, W.v, W.u, &W.st->ca, W.part_u, W.t, &W.st->stop, s));
+        GSR_TRY(launch_aprod2_instr(A, W.u, W.t, &W.st->stop, s));
+        k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units, W.t + n, &W.st->stop);
+        GSR_TRY(comm_allreduce_sum(A->comm, W.t + split, (size_t)(n - split + 1), s));
+        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.t + n, 1);
+        k_vnew<<<NB_N, TB_N, 0, s>>>(W.v, W.t, n, W.st, W.part_v, split, W.part_va);
+        k_sum_partials<<<1, 1024, 0, s>>>(W.part_va, NB_N, W.red, &W.st->stop);
+        GSR_TRY(comm_allreduce_sum(A->comm, W.red, 2, s));      // red[1]: from the last k_update
+        k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N, W.red);
+        k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, W.t, W.var, split, W.part_wa);
+        k_sum_partials<<<1, 1024, 0, s>>>(W.part_wa, NB_N, W.red + 1, &W.st->stop);
     }
     k_raise_stop<<<1, 1, 0, s>>>(W.st);
     GSR_CUDA_TRY(cudaGetLastError());
@@ -373,7 +429,8 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
 
 static int build_graph(gsr_matrix* A, cudaStream_t s) {
     Workspace& W = A->ws;
-    if (W.graph_valid && W.graph_stream == s && W.graph_two_pass == A->opt_two_pass) return GSR_OK;
+    if (W.graph_valid && W.graph_stream == s && W.graph_two_pass == A->opt_two_pass && W.graph_comm == (void*)A->comm)
+        return GSR_OK;
     if (W.graph) {
         cudaGraphExecDestroy(W.graph);
         W.graph = nullptr;
@@ -409,6 +466,7 @@ static int build_graph(gsr_matrix* A, cudaStream_t s) {
     W.graph_valid = true;
     W.graph_stream = s;
     W.graph_two_pass = A->opt_two_pass;
+    W.graph_comm = (void*)A->comm;
     return GSR_OK;
 }
 
@@ -451,13 +509,33 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     GSR_CUDA_TRY(cudaMemsetAsync(W.var, 0, (size_t)n * 8, s));
     W.solved = false;
     // initialisation (row a2): u_hat = b, beta_1, v = A^T u, alpha_1, w = v
+    if (A->comm && A->opt_two_pass) return GSR_EUNSUPPORTED;
+    const int64_t split = A->comm ? A->off_att : 0;
     k_gather_sumsq<<<NB_N, TB_N, 0, s>>>(b_dev, A->perm, W.u, A->m_int, W.part_u);
-    k_scalar_init1<<<1, 1024, 0, s>>>(W.st, W.part_u, NB_N);
+    if (A->comm) {   // ||b||^2 over all row shards
+        k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, NB_N, W.red + 2, nullptr);
+        GSR_TRY(comm_allreduce_sum(A->comm, W.red + 2, 1, s));
+        k_scalar_init1<<<1, 1024, 0, s>>>(W.st, W.red + 2, 1);
+        count_launch();
+    } else {
+        k_scalar_init1<<<1, 1024, 0, s>>>(W.st, W.part_u, NB_N);
+    }
     count_launch(2);
     GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s));
-    k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop);
-    k_scalar_init2<<<1, 1024, 0, s>>>(W.st, W.part_v, NB_N);
-    k_update<true><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, nullptr, nullptr);
+    if (A->comm)     // replicated slice of v = A^T u: sum of the shards' contributions
+        GSR_TRY(comm_allreduce_sum(A->comm, W.v + split, (size_t)(n - split), s));
+    k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop, split, W.part_va);
+    if (A->comm) {
+        k_sum_partials<<<1, 1024, 0, s>>>(W.part_va, NB_N, W.red, &W.st->stop);
+        GSR_TRY(comm_allreduce_sum(A->comm, W.red, 1, s));
+        count_launch();
+    }
+    k_scalar_init2<<<1, 1024, 0, s>>>(W.st, W.part_v, NB_N, A->comm ? W.red : nullptr);
+    k_update<true><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, nullptr, nullptr, split, W.part_wa);
+    if (A->comm) {
+        k_sum_partials<<<1, 1024, 0, s>>>(W.part_wa, NB_N, W.red + 1, &W.st->stop);
+        count_launch();
+    }
     GSR_CUDA_TRY(cudaMemsetAsync(W.t, 0, (size_t)n * 8, s));
     count_launch(3);
     GSR_CUDA_TRY(cudaGetLastError());
@@ -509,14 +587,14 @@ int gsr_lsqr_standard_errors(gsr_matrix* A, double* se_hd, gsr_stream stream) {
     Workspace& W = A->ws;
     if (A->state != 1 || !W.solved) return GSR_ESTATE;
     cudaStream_t s = (cudaStream_t)stream;
-    const int64_t m = A->dims.n_rows, n = A->n_cols;
+    const int64_t n = A->n_cols;
     const bool dev = is_device_ptr(se_hd);
     double* out = se_hd;
     if (!dev) {
         if (!W.stage_n) GSR_TRY(dev_alloc(A, (void**)&W.stage_n, (size_t)n * 8));
         out = W.stage_n;
     }
-    const double dof = m > n ? (double)(m - n) : 1.0;
+    const double dof = A->m_global > A->n_global ? (double)(A->m_global - A->n_global) : 1.0;
     k_standard_errors<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(W.var, A->p, W.last_rnorm, dof, out, n);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());

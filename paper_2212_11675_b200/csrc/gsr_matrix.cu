@@ -458,6 +458,8 @@ int gsr_matrix_finalize(gsr_matrix* A) {
     }
     GSR_CUDA_TRY(cudaStreamSynchronize(A->stream));
     GSR_TRY(configure_product_kernels(A));
+    A->m_global = A->dims.n_rows;
+    A->n_global = A->n_cols;
     A->state = 1;
     return GSR_OK;
 }
@@ -557,6 +559,8 @@ int gsr_precondition(gsr_matrix* A, double* p_out, gsr_stream stream) {
     GSR_TRY(dev_alloc(A, (void**)&A->p, (size_t)A->n_cols * 8));
     GSR_CUDA_TRY(cudaMemsetAsync(A->p, 0, (size_t)A->n_cols * 8, s));
     GSR_TRY(launch_colsumsq(A, A->p, s));
+    if (A->comm)   // column norms of the replicated slice are sums over all row shards
+        GSR_TRY(comm_allreduce_sum(A->comm, A->p + A->off_att, (size_t)(A->n_cols - A->off_att), s));
     k_make_p<<<(unsigned)((A->n_cols + 255) / 256), 256, 0, s>>>(A->p, A->n_cols);
     count_launch();
     if (A->n_tiles > 0) {

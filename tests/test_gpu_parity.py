@@ -288,3 +288,41 @@ def test_host_arrays_and_chunked_builder_equal_one_shot():
     for c, v, y in outs[1:]:
         assert np.array_equal(c, outs[0][0]) and np.array_equal(v, outs[0][1])
         assert np.array_equal(y, outs[0][2])
+
+
+def test_sharded_solve_world_1_nccl_matches_plain_solve():
+    """Row e: the sharded iteration (NCCL all-reduces inside the graph, split norm sums) with a
+    one-rank communicator must reproduce the plain solve and the oracle.  The N > 1 algebra is
+    covered on the CPU by tests/test_sharding_gloo.py."""
+    b = _binding()
+    s = Sys(CASES["cfg1"])
+    try:
+        rhs = _rhs(s)
+        comm = b.gsr_comm_create(0, 1, b.gsr_comm_unique_id())
+        b.gsr_matrix_set_comm(s.A.h, comm, s.m, s.n)
+        s.o.precondition()
+        b.gsr_precondition(s.A.h)
+        b.gsr_set_option(s.A.h, b.GSR_OPT_FORCE_ITNLIM, 1)
+        bd = torch.from_numpy(rhs).cuda()
+        x = torch.empty(s.n, dtype=torch.float64, device="cuda")
+        r = b.gsr_lsqr_solve(s.A.h, bd, x, 12)
+        ro = s.o.lsqr(rhs, 12, force_itnlim=True, want_se=True)
+        assert (r.istop, r.itn) == (7, 12)
+        assert np.linalg.norm(x.cpu().numpy() - ro.x) <= X_TOL * np.linalg.norm(ro.x)
+        assert abs(r.rnorm - ro.rnorm) <= X_TOL * ro.rnorm and abs(r.anorm - ro.anorm) <= X_TOL * ro.anorm
+        se = np.empty(s.n)
+        b.gsr_lsqr_standard_errors(s.A.h, se)
+        assert np.linalg.norm(se - ro.se) <= 1e-8 * np.linalg.norm(ro.se)
+        b.gsr_set_option(s.A.h, b.GSR_OPT_FUSED, 0)      # two-pass form is not sharded
+        with pytest.raises(b.GsrError) as ei:
+            b.gsr_lsqr_solve(s.A.h, bd, x, 3)
+        assert ei.value.code == b.GSR_EUNSUPPORTED
+        b.gsr_set_option(s.A.h, b.GSR_OPT_FUSED, 1)
+        b.gsr_set_option(s.A.h, b.GSR_OPT_FORCE_ITNLIM, 0)
+        r = b.gsr_lsqr_solve(s.A.h, bd, x, 500, 1e-10, 1e-10, 1e8)
+        ro = s.o.lsqr(rhs, 500, 1e-10, 1e-10, 1e8)
+        assert r.istop == ro.istop and abs(r.itn - ro.itn) <= 1
+        s.A.close()
+        b.gsr_comm_destroy(comm)
+    finally:
+        s.A.close()
