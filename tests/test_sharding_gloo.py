@@ -135,7 +135,7 @@ def _free_port():
 def test_sharded_lsqr_two_gloo_ranks_matches_single_process_oracle():
     k = 12
     world = 2
-    mgr = mp.Manager()
+    mgr = mp.get_context("spawn").Manager()
     out = mgr.dict()
     mp.spawn(_sharded_lsqr, args=(world, _free_port(), k, out), nprocs=world, join=True)
     cfg = _cfg()
