@@ -59,7 +59,7 @@ def _allsum(a):
     return t.numpy().reshape(np.shape(a))
 
 
-def _sharded_lsqr(rank, world, port, k_fixed, out):
+def _sharded_lsqr(rank, world, port, k_fixed, fused, out):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
@@ -108,8 +108,16 @@ def _sharded_lsqr(rank, world, port, k_fixed, out):
         for _ in range(k_fixed):
             u = o.aprod1(v, -alpha * u)
             beta = np.sqrt(float(_allsum(np.array([np.dot(u, u)]))[0]))
-            u /= beta
-            v = aprod2_sharded(u, -beta * v)
+            if fused:
+                # the CUDA path's form: t = A^T u_hat with u_hat unnormalised,
+                # replicated slice of t summed over the ranks, then v = t/beta - beta v everywhere
+                t = o.aprod2(u, np.zeros(nl))
+                t[ro:] = _allsum(t[ro:])
+                v = t / beta - beta * v
+                u /= beta
+            else:
+                u /= beta
+                v = aprod2_sharded(u, -beta * v)
             alpha = np.sqrt(norm2(v))
             v /= alpha
             rho = hyp(rhobar, beta)
@@ -132,12 +140,13 @@ def _free_port():
 
 
 @pytest.mark.timeout(300)
-def test_sharded_lsqr_two_gloo_ranks_matches_single_process_oracle():
+@pytest.mark.parametrize("fused", [True, False])
+def test_sharded_lsqr_two_gloo_ranks_matches_single_process_oracle(fused):
     k = 12
     world = 2
     mgr = mp.get_context("spawn").Manager()
     out = mgr.dict()
-    mp.spawn(_sharded_lsqr, args=(world, _free_port(), k, out), nprocs=world, join=True)
+    mp.spawn(_sharded_lsqr, args=(world, _free_port(), k, fused, out), nprocs=world, join=True)
     cfg = _cfg()
     star, att, instr, vals = [t.numpy() for t in inputs.gen_all(cfg)]
     o = make_oracle(cfg, star, att, instr, vals)
