@@ -198,6 +198,9 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double* xi = sm;
     double* xw = sm + ((I + 1) & ~1) + warp * 3 * ws;
+    double* ysm = sm + ((I + 1) & ~1) + NWARP * 3 * ws + warp * 32;   // y of the current tile: a
+                                                  // shared-memory broadcast costs the LSU pipe
+                                                  // less than two 32-bit shuffles per step
     for (int i = threadIdx.x; i < I; i += TPB) xi[i] = 0.0;
     const double sy = SQUARE ? 1.0 : *sy_p;
     __syncthreads();
@@ -233,6 +236,8 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
             // phase A -- attitude: rows 0-15 through lanes 0-11, rows 16-31
             // through lanes 16-27, one row per half and step; the two rows of a step go in one
             // instruction unless their windows overlap (then one after the other)
+            ysm[lane] = yv;
+            __syncwarp();
             const uint32_t a_other = __shfl_xor_sync(0xffffffffu, ra.aoff, 16);
             const int da = (int)ra.aoff - (int)a_other;
             const unsigned cmask = __ballot_sync(0xffffffffu, da > -4 && da < 4);
@@ -240,7 +245,7 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
             for (int qq = 0; qq < 16; ++qq) {
                 const int src = h * 16 + qq;
                 const uint32_t a = __shfl_sync(0xffffffffu, ra.aoff, src);
-                const double yy = __shfl_sync(0xffffffffu, yv, src);
+                const double yy = ysm[src];
                 const double add = SQUARE ? ra.at[qq] * ra.at[qq] : ra.at[qq] * yy;
                 double* pa = xw + a + axo;
                 if ((cmask >> qq) & 1u) {
@@ -344,6 +349,9 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
     double* xi = sm;
     double* xw = sm + ((I + 1) & ~1) + warp * 6 * ws;   // window of v (read)
     double* tw = xw + 3 * ws;                           // window of A^T u_hat (accumulate)
+    double* ysm = sm + ((I + 1) & ~1) + NWARP * 6 * ws + warp * 32;   // u_hat of the current tile,
+                                                  // broadcast to the attitude lanes through shared
+                                                  // memory (cheaper on the LSU pipe than shuffles)
     const double* xatt = x + 5 * S;
     const double* xins = x + 5 * S + 3 * D;
     double* tatt = tacc + 5 * S;
@@ -405,16 +413,18 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
             sum = fma(r.gl, xg, sum);
             const double yv = fma(ca, yold, sum);   // u_hat of this row (padding rows: 0)
             y[ri] = yv;
+            ysm[lane] = yv;
             q = fma(yv, yv, q);
             // ---- mode 2 for this tile, attitude
             const uint32_t a_other = __shfl_xor_sync(0xffffffffu, ra.aoff, 16);
             const int da = (int)ra.aoff - (int)a_other;
             const unsigned cmask = __ballot_sync(0xffffffffu, da > -4 && da < 4);
+            __syncwarp();   // ysm visible to the whole warp
 #pragma unroll
             for (int qq = 0; qq < 16; ++qq) {
                 const int src = h * 16 + qq;
                 const uint32_t a = __shfl_sync(0xffffffffu, ra.aoff, src);
-                const double yy = __shfl_sync(0xffffffffu, yv, src);
+                const double yy = ysm[src];
                 const double add = ra.at[qq] * yy;
                 double* pa = tw + a + axo;
                 if ((cmask >> qq) & 1u) {
