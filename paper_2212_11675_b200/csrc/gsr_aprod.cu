@@ -191,7 +191,7 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
                                                const double* __restrict__ y, double* __restrict__ x,
                                                const double* __restrict__ sy_p,
                                                const uint32_t* __restrict__ perm, int64_t S,
-                                               int64_t D, int I, int win, int ws,
+                                               int64_t D, int I, int win, int ws, int ncopy,
                                                const int* __restrict__ stop) {
     if (stop && *stop) return;
     extern __shared__ double sm[];
@@ -201,7 +201,13 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
     double* ysm = sm + ((I + 1) & ~1) + NWARP * 3 * ws + warp * 32;   // y of the current tile: a
                                                   // shared-memory broadcast costs the LSU pipe
                                                   // less than two 32-bit shuffles per step
+    // small I: one private copy of the instrumental accumulator per warp (copies 1.. behind the
+    // y tiles), so that only lanes of the same instruction contend for an address (config 4)
+    const int ipad = (I + 1) & ~1;
+    double* xcopies = sm + ipad + NWARP * 3 * ws + NWARP * 32;
     for (int i = threadIdx.x; i < I; i += TPB) xi[i] = 0.0;
+    for (int i = threadIdx.x; i < (ncopy - 1) * ipad; i += TPB) xcopies[i] = 0.0;
+    if (ncopy > 1 && warp > 0) xi = xcopies + (warp - 1) * ipad;
     const double sy = SQUARE ? 1.0 : *sy_p;
     __syncthreads();
 
@@ -323,7 +329,8 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
     __syncthreads();
     double* xins = x + 5 * S + 3 * D;
     for (int i = threadIdx.x; i < I; i += TPB) {
-        const double vacc = xi[i];
+        double vacc = sm[i];
+        for (int w = 1; w < ncopy; ++w) vacc += xcopies[(w - 1) * ipad + i];
         if (vacc != 0.0) atomicAdd(xins + i, vacc);
     }
 }
@@ -613,10 +620,10 @@ int launch_aprod2(const gsr_matrix* A, const double* y, double* x, const double*
     GSR_TRY(reset_counter(A, s));
     if (perm)
         k_aprod2<false, true><<<A->grid2, TPB, A->smem_bytes, s>>>(
-            A->tiles, A->units, A->n_units, A->unit_counter, y, x, sy, perm, S, D, I, A->win, A->wstride, stop);
+            A->tiles, A->units, A->n_units, A->unit_counter, y, x, sy, perm, S, D, I, A->win, A->wstride, instr_copies(A), stop);
     else
         k_aprod2<false, false><<<A->grid2, TPB, A->smem_bytes, s>>>(
-            A->tiles, A->units, A->n_units, A->unit_counter, y, x, sy, nullptr, S, D, I, A->win, A->wstride, stop);
+            A->tiles, A->units, A->n_units, A->unit_counter, y, x, sy, nullptr, S, D, I, A->win, A->wstride, instr_copies(A), stop);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;
@@ -649,7 +656,7 @@ int launch_colsumsq(const gsr_matrix* A, double* q, cudaStream_t s) {
     GSR_TRY(reset_counter(A, s));
     k_aprod2<true, false><<<A->grid2, TPB, A->smem_bytes, s>>>(
         A->tiles, A->units, A->n_units, A->unit_counter, nullptr, q, nullptr, nullptr, A->dims.n_stars,
-        A->dims.n_dfa, (int)A->dims.n_instr, A->win, A->wstride, nullptr);
+        A->dims.n_dfa, (int)A->dims.n_instr, A->win, A->wstride, instr_copies(A), nullptr);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;

@@ -348,7 +348,8 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
     if (nbins > NBIN_MAX) return GSR_EUNSUPPORTED;
     const int64_t bw = (n_start + nbins - 1) / nbins;
     const int64_t wstride = (bw + 3) + ((4 - (bw + 3)) % 16 + 16) % 16;   // >= bw+3, = 4 (mod 16)
-    const int64_t smem_bytes = instr_bytes + NWARP * 3 * wstride * 8 + NWARP * 32 * 8;
+    const int64_t instr_copies = instr_bytes * NWARP <= 96 * 1024 ? NWARP : 1;   // as in gsr_aprod.cu
+    const int64_t smem_bytes = instr_bytes * instr_copies + NWARP * 3 * wstride * 8 + NWARP * 32 * 8;
 
     int dev = 0;
     cudaDeviceProp prop;
