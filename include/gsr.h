@@ -168,10 +168,14 @@ enum {
                                  the iteration limit stops the loop (fixed-count mode, A9)    */
     GSR_OPT_DETERMINISTIC = 2, /* 1: aprod2 uses no floating-point atomics (bit-reproducible);
                                  reserved: any value but 0 returns GSR_EUNSUPPORTED           */
-    GSR_OPT_FUSED = 3         /* 1 (default): one LSQR iteration reads the matrix ONCE -- u_hat =
+    GSR_OPT_FUSED = 3,        /* 1 (default): one LSQR iteration reads the matrix ONCE -- u_hat =
                                  A v - (alpha/beta) u_hat and A^T u_hat are formed in the same
                                  pass, v = A^T u_hat / beta - beta v afterwards (same recurrences,
-                                 DESIGN.md 5.5); 0: aprod1 then aprod2, two reads per iteration  */
+                                 DESIGN.md 5.4); 0: aprod1 then aprod2, two reads per iteration  */
+    GSR_OPT_FIXED_POINT = 4   /* 1 (default): on a column-scaled matrix the instrumental pass of
+                                 the fused iteration accumulates in exact 64-bit fixed point
+                                 with native 32-bit shared atomics (order-independent sums,
+                                 normwise error <= n_j 2^-62 ||u|| per column); 0: fp64 atomics  */
 };
 int gsr_set_option(gsr_matrix* A, int key, int64_t value);
 

@@ -493,17 +493,36 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
 }
 
 // Instrumental block of A^T u (row a7) over the instrumental planes only (1920 B per tile):
-// shared-memory accumulators, six fp64 shared atomicAdds per row.  `ncopy` = 1: one accumulator
-// per CTA; `ncopy` = NWARP (small I): one private copy per warp, so that only lanes of the same
+// shared-memory accumulators, six scattered adds per row.  `ncopy` = 1: one accumulator per
+// CTA; `ncopy` = NWARP (small I): one private copy per warp, so that only lanes of the same
 // instruction ever contend for an address (config 4: 60 columns).
+//
+// FIXED = false: fp64 atomicAdd, a CAS loop on sm_100a (about 420 G adds/s on the chip).
+// FIXED = true : exact 64-bit fixed-point accumulation with NATIVE 32-bit shared atomics -- low
+//   word add (returns the old value, so the thread that wraps it knows), high word add with the
+//   carry; integer adds commute, so the sum is exact and independent of the order (about 770 G
+//   adds/s).  Only for a column-scaled matrix: every column has unit 2-norm, hence any partial
+//   sum of column j is bounded by sum_i |A_ij| |y_i| <= ||A_j|| ||y|| = ||y||, and with
+//   2^e >= ||y|| the scale 2^(61-e) keeps it below 2^62.  Each term is rounded once to a
+//   multiple of 2^(e-61): an absolute error <= n_j 2^(e-62) per column, i.e. normwise
+//   ~1e-18 ||y|| per term (fp64 atomics are componentwise accurate instead; LSQR only needs
+//   the normwise bound).  ss_p points to sum y_i^2 over the rows of this launch (device).
+template <bool FIXED>
 __global__ void __launch_bounds__(TPB) k_aprod2_instr(const unsigned char* __restrict__ tiles,
                                                      int64_t n_tiles, const double* __restrict__ y,
                                                      double* __restrict__ xins, int I, int ncopy,
+                                                     const double* __restrict__ ss_p,
                                                      const int* __restrict__ stop) {
     if (stop && *stop) return;
     extern __shared__ double sm[];
     const int ipad = (I + 1) & ~1;
-    for (int i = threadIdx.x; i < ipad * ncopy; i += TPB) sm[i] = 0.0;
+    for (int i = threadIdx.x; i < ipad * ncopy; i += TPB) sm[i] = 0.0;   // +0.0 = integer 0
+    int e = 0;
+    if (FIXED) {
+        const double ynorm = sqrt(*ss_p);
+        e = ynorm > 0.0 ? ilogb(ynorm) + 1 : 0;   // 2^e > ||y||
+    }
+    const double scale = FIXED ? scalbn(1.0, 61 - e) : 1.0;
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double* acc = sm + (ncopy > 1 ? warp * ipad : 0);
@@ -517,14 +536,34 @@ __global__ void __launch_bounds__(TPB) k_aprod2_instr(const unsigned char* __res
         for (int k = 0; k < 6; ++k) c[k] = ld_stream_u16(T + OFF_ICOL + (k * R + lane) * 2);
 #pragma unroll
         for (int k = 0; k < 6; ++k) v[k] = ld_stream_f64(T + OFF_INSTRV + (k * R + lane) * 8);
-        const double yv = __ldcs(y + tile * R + lane);
+        const double yv = __ldcs(y + tile * R + lane) * scale;
+        if (FIXED) {
+            unsigned* acc32 = (unsigned*)acc;
 #pragma unroll
-        for (int k = 0; k < 6; ++k) atomicAdd(acc + c[k], v[k] * yv);
+            for (int k = 0; k < 6; ++k) {
+                const long long q = __double2ll_rn(v[k] * yv);
+                const unsigned ql = (unsigned)q, qh = (unsigned)(q >> 32);
+                const unsigned old = atomicAdd(acc32 + 2 * c[k], ql);
+                const unsigned carry = (old + ql) < old ? 1u : 0u;
+                if (qh + carry != 0u) atomicAdd(acc32 + 2 * c[k] + 1, qh + carry);
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < 6; ++k) atomicAdd(acc + c[k], v[k] * yv);
+        }
     }
     __syncthreads();
+    const double unscale = FIXED ? scalbn(1.0, e - 61) : 1.0;
     for (int i = threadIdx.x; i < I; i += TPB) {
-        double vacc = 0.0;
-        for (int w = 0; w < ncopy; ++w) vacc += sm[w * ipad + i];
+        double vacc;
+        if (FIXED) {
+            long long tot = 0;
+            for (int w = 0; w < ncopy; ++w) tot += ((const long long*)sm)[w * ipad + i];
+            vacc = (double)tot * unscale;
+        } else {
+            vacc = 0.0;
+            for (int w = 0; w < ncopy; ++w) vacc += sm[w * ipad + i];
+        }
         if (vacc != 0.0) atomicAdd(xins + i, vacc);
     }
 }
@@ -561,7 +600,8 @@ int configure_product_kernels(gsr_matrix* A) {
     GSR_TRY(set_smem(k_aprod2<false, true>, b));
     GSR_TRY(set_smem(k_aprod2<true, false>, b));
     GSR_TRY(set_smem(k_fused, A->smem_fused));
-    GSR_TRY(set_smem(k_aprod2_instr, (int)instr_smem(A)));
+    GSR_TRY(set_smem(k_aprod2_instr<false>, (int)instr_smem(A)));
+    GSR_TRY(set_smem(k_aprod2_instr<true>, (int)instr_smem(A)));
     {
         int nb = 1;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_fused, TPB, A->smem_fused) != cudaSuccess || nb < 1) {
@@ -570,7 +610,7 @@ int configure_product_kernels(gsr_matrix* A) {
         }
         A->grid_fused = A->sm_count * nb;
         nb = 1;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_aprod2_instr, TPB, instr_smem(A)) != cudaSuccess || nb < 1) {
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_aprod2_instr<true>, TPB, instr_smem(A)) != cudaSuccess || nb < 1) {
             cudaGetLastError();
             nb = 1;
         }
@@ -641,11 +681,16 @@ int launch_fused(const gsr_matrix* A, const double* v, double* u, const double* 
     return GSR_OK;
 }
 
-int launch_aprod2_instr(const gsr_matrix* A, const double* u, double* t, const int* stop,
-                        cudaStream_t s) {
+int launch_aprod2_instr(const gsr_matrix* A, const double* u, double* t, const double* ss,
+                        const int* stop, cudaStream_t s) {
     if (A->n_tiles == 0) return GSR_OK;
-    k_aprod2_instr<<<A->grid_instr, TPB, instr_smem(A), s>>>(
-        A->tiles, A->n_tiles, u, t + A->off_instr, (int)A->dims.n_instr, instr_copies(A), stop);
+    // exact fixed-point accumulation needs unit column norms (see k_aprod2_instr) and ||u||^2
+    if (A->p != nullptr && ss != nullptr && !A->opt_no_fixed)
+        k_aprod2_instr<true><<<A->grid_instr, TPB, instr_smem(A), s>>>(
+            A->tiles, A->n_tiles, u, t + A->off_instr, (int)A->dims.n_instr, instr_copies(A), ss, stop);
+    else
+        k_aprod2_instr<false><<<A->grid_instr, TPB, instr_smem(A), s>>>(
+            A->tiles, A->n_tiles, u, t + A->off_instr, (int)A->dims.n_instr, instr_copies(A), nullptr, stop);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;

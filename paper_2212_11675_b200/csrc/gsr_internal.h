@@ -161,6 +161,7 @@ struct gsr_matrix {
     int64_t device_bytes;
     int opt_force_itnlim;
     int opt_two_pass;               // 1: aprod1 + aprod2 per iteration instead of the fused pass
+    int opt_no_fixed;               // 1: fp64 atomics in the instrumental pass even when scaled
     gsr_comm* comm;                 // row e: this handle is one row shard (nullptr: whole system)
     int64_t m_global, n_global;     // rows / columns of the whole system (= local without comm)
     int sm_count;
@@ -212,8 +213,8 @@ int launch_colsumsq(const gsr_matrix* A, double* q, cudaStream_t s);
 // instrumental planes only.  t must hold zeros (or the value to accumulate onto) on entry.
 int launch_fused(const gsr_matrix* A, const double* v, double* u, const double* ca,
                  double* partials, double* t, const int* stop, cudaStream_t s);
-int launch_aprod2_instr(const gsr_matrix* A, const double* u, double* t, const int* stop,
-                        cudaStream_t s);
+int launch_aprod2_instr(const gsr_matrix* A, const double* u, double* t, const double* ss,
+                        const int* stop, cudaStream_t s);   // ss: device sum of u^2 (or nullptr)
 int configure_product_kernels(gsr_matrix* A);
 
 }  // namespace gsr

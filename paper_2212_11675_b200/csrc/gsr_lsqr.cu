@@ -382,7 +382,7 @@ void free_workspace(gsr_matrix* A) {
 // together, k_aprod2_instr adds the instrumental block of t, k_vnew forms v = t/beta - beta v.
 // Two-pass form (GSR_OPT_FUSED = 0): aprod1, then aprod2 on the pre-scaled v.
 static int kernels_per_iteration(const gsr_matrix* A) {
-    return A->opt_two_pass ? 8 : (A->comm ? 10 : 7);
+    return A->opt_two_pass ? 8 : (A->comm ? 10 : 8);
 }
 
 static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
@@ -401,8 +401,9 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
         k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, nullptr, W.var, 0, nullptr);
     } else if (!A->comm) {
         GSR_TRY(launch_fused(A, W.v, W.u, &W.st->ca, W.part_u, W.t, &W.st->stop, s));
-        GSR_TRY(launch_aprod2_instr(A, W.u, W.t, &W.st->stop, s));
-        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_units);
+        k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units, W.red + 3, &W.st->stop);
+        GSR_TRY(launch_aprod2_instr(A, W.u, W.t, W.red + 3, &W.st->stop, s));
+        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.red + 3, 1);
         k_vnew<<<NB_N, TB_N, 0, s>>>(W.v, W.t, n, W.st, W.part_v, 0, nullptr);
         k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N, nullptr);
         k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, W.t, W.var, 0, nullptr);
@@ -411,8 +412,8 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
         // as NCCL all-reduces inside the graph.  #1: replicated slice of t = A^T u_hat, with the
         // local sum of u_hat^2 riding in t[n]; #2: the distributed parts of ||v||^2 and ||w||^2.
         GSR_TRY(launch_fused(A, W.v, W.u, &W.st->ca, W.part_u, W.t, &W.st->stop, s));
-        GSR_TRY(launch_aprod2_instr(A, W.u, W.t, &W.st->stop, s));
         k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units, W.t + n, &W.st->stop);
+        GSR_TRY(launch_aprod2_instr(A, W.u, W.t, W.t + n, &W.st->stop, s));   // local ||u_hat||^2
         GSR_TRY(comm_allreduce_sum(A->comm, W.t + split, (size_t)(n - split + 1), s));
         k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.t + n, 1);
         k_vnew<<<NB_N, TB_N, 0, s>>>(W.v, W.t, n, W.st, W.part_v, split, W.part_va);
@@ -615,6 +616,10 @@ int gsr_time_product(gsr_matrix* A, int which, int reps, float* ms_avg, gsr_stre
     GSR_CUDA_TRY(cudaEventCreate(&e0));
     GSR_CUDA_TRY(cudaEventCreate(&e1));
     int rc = GSR_OK;
+    if (which == 4) {   // the instrumental pass needs a consistent u_hat and its sum of squares
+        rc = launch_fused(A, W.v, W.u, A->coef_one, W.part_u, W.t, nullptr, s);
+        k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units, W.red + 3, nullptr);
+    }
     for (int pass = 0; pass < 2 && rc == GSR_OK; ++pass) {   // pass 0: warm-up
         int nrep = pass == 0 ? 1 : reps;
         cudaEventRecord(e0, s);
@@ -622,7 +627,7 @@ int gsr_time_product(gsr_matrix* A, int which, int reps, float* ms_avg, gsr_stre
             if (which == 1) rc = launch_aprod1(A, W.v, W.u, A->coef_one, W.part_u, nullptr, nullptr, s);
             else if (which == 2) rc = launch_aprod2(A, W.u, W.v, A->coef_one, nullptr, nullptr, s);
             else if (which == 3) rc = launch_fused(A, W.v, W.u, A->coef_one, W.part_u, W.t, nullptr, s);
-            else rc = launch_aprod2_instr(A, W.u, W.t, nullptr, s);
+            else rc = launch_aprod2_instr(A, W.u, W.t, W.red + 3, nullptr, s);
         }
         cudaEventRecord(e1, s);
         if (cudaEventSynchronize(e1) != cudaSuccess) rc = GSR_ECUDA;

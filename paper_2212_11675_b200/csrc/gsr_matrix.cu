@@ -518,6 +518,7 @@ int gsr_set_option(gsr_matrix* A, int key, int64_t value) {
         case GSR_OPT_FORCE_ITNLIM: A->opt_force_itnlim = value != 0; return GSR_OK;
         case GSR_OPT_DETERMINISTIC: return value == 0 ? GSR_OK : GSR_EUNSUPPORTED;
         case GSR_OPT_FUSED: A->opt_two_pass = value == 0; return GSR_OK;
+        case GSR_OPT_FIXED_POINT: A->opt_no_fixed = value == 0; return GSR_OK;
         default: return GSR_EINVAL;
     }
 }

@@ -326,3 +326,31 @@ def test_sharded_solve_world_1_nccl_matches_plain_solve():
         b.gsr_comm_destroy(comm)
     finally:
         s.A.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1", "skew_hot", "one_instr_col"])
+def test_fixed_point_instrumental_pass_matches_fp64_atomics(name):
+    """GSR_OPT_FIXED_POINT: on a column-scaled matrix the instrumental block of A^T u_hat is
+    accumulated in exact 64-bit fixed point (native 32-bit shared atomics); with the option off,
+    with fp64 atomics.  Both must match the oracle, and each other far more closely."""
+    b = _binding()
+    s = Sys(CASES[name])
+    try:
+        rhs = _rhs(s)
+        s.o.precondition()
+        b.gsr_precondition(s.A.h)
+        b.gsr_set_option(s.A.h, b.GSR_OPT_FORCE_ITNLIM, 1)
+        bd = torch.from_numpy(rhs).cuda()
+        k = 3
+        ro = s.o.lsqr(rhs, k, force_itnlim=True)
+        xs = []
+        for fixed in (1, 0):
+            b.gsr_set_option(s.A.h, b.GSR_OPT_FIXED_POINT, fixed)
+            x = torch.empty(s.n, dtype=torch.float64, device="cuda")
+            r = b.gsr_lsqr_solve(s.A.h, bd, x, k)
+            assert (r.istop, r.itn) == (7, k)
+            xs.append(x.cpu().numpy())
+            assert np.linalg.norm(xs[-1] - ro.x) <= X_TOL * np.linalg.norm(ro.x)
+        assert np.linalg.norm(xs[0] - xs[1]) <= 1e-12 * np.linalg.norm(ro.x)
+    finally:
+        s.A.close()
