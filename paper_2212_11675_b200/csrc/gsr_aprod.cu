@@ -356,9 +356,11 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
     double* xi = sm;
     double* xw = sm + ((I + 1) & ~1) + warp * 6 * ws;   // window of v (read)
     double* tw = xw + 3 * ws;                           // window of A^T u_hat (accumulate)
-    double* ysm = sm + ((I + 1) & ~1) + NWARP * 6 * ws + warp * 32;   // u_hat of the current tile,
-                                                  // broadcast to the attitude lanes through shared
-                                                  // memory (cheaper on the LSU pipe than shuffles)
+    // u_hat and the window offsets of the current tile reach the attitude lanes through shared
+    // memory: wide broadcast loads (two u_hat, four offsets per request) cost the LSU data pipe
+    // far less than one or two 32-bit shuffles per row and step
+    double* ysm = sm + ((I + 1) & ~1) + NWARP * 6 * ws + warp * 48;
+    uint32_t* asm_ = (uint32_t*)(ysm + 32);
     const double* xatt = x + 5 * S;
     const double* xins = x + 5 * S + 3 * D;
     double* tatt = tacc + 5 * S;
@@ -395,11 +397,17 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
             const double yold = __ldcs(y + ri);
             // ---- mode 1 for this tile
             double p[16];
+            asm_[lane] = ra.aoff;
+            __syncwarp();
 #pragma unroll
-            for (int qq = 0; qq < 16; ++qq) {
-                const uint32_t a = __shfl_sync(0xffffffffu, ra.aoff, h * 16 + qq);
-                const double pv = ra.at[qq] * xw[a + axo];
-                p[qq] = att_lane ? pv : 0.0;
+            for (int g4 = 0; g4 < 4; ++g4) {
+                const uint4 a4 = *(const uint4*)(asm_ + h * 16 + 4 * g4);
+                const uint32_t aa[4] = {a4.x, a4.y, a4.z, a4.w};
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const double pv = ra.at[4 * g4 + i] * xw[aa[i] + axo];
+                    p[4 * g4 + i] = att_lane ? pv : 0.0;
+                }
             }
 #pragma unroll
             for (int o = 8; o > 0; o >>= 1) {
@@ -428,20 +436,26 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
             const unsigned cmask = __ballot_sync(0xffffffffu, da > -4 && da < 4);
             __syncwarp();   // ysm visible to the whole warp
 #pragma unroll
-            for (int qq = 0; qq < 16; ++qq) {
-                const int src = h * 16 + qq;
-                const uint32_t a = __shfl_sync(0xffffffffu, ra.aoff, src);
-                const double yy = ysm[src];
-                const double add = ra.at[qq] * yy;
-                double* pa = tw + a + axo;
-                if ((cmask >> qq) & 1u) {
-                    if (lo12) *pa += add;
+            for (int g4 = 0; g4 < 4; ++g4) {
+                const uint4 a4 = *(const uint4*)(asm_ + h * 16 + 4 * g4);
+                const double2 y01 = *(const double2*)(ysm + h * 16 + 4 * g4);
+                const double2 y23 = *(const double2*)(ysm + h * 16 + 4 * g4 + 2);
+                const uint32_t aa[4] = {a4.x, a4.y, a4.z, a4.w};
+                const double yy4[4] = {y01.x, y01.y, y23.x, y23.y};
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const int qq = 4 * g4 + i;
+                    const double add = ra.at[qq] * yy4[i];
+                    double* pa = tw + aa[i] + axo;
+                    if ((cmask >> qq) & 1u) {
+                        if (lo12) *pa += add;
+                        __syncwarp();
+                        if (hi12) *pa += add;
+                    } else {
+                        if (lo12 || hi12) *pa += add;
+                    }
                     __syncwarp();
-                    if (hi12) *pa += add;
-                } else {
-                    if (lo12 || hi12) *pa += add;
                 }
-                __syncwarp();
             }
             if (t + 1 < un.ntiles) load_A(T + TILE_BYTES, lane, ra);
             // ---- mode 2, global and astrometric

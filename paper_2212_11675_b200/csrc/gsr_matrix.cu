@@ -337,7 +337,7 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
     const int64_t instr_bytes = (d->n_instr + 1) / 2 * 16;
     if (d->n_instr > 65535 || instr_bytes > SMEM_BUDGET - NWARP * 24 * 4) return GSR_EUNSUPPORTED;
     // (the fused iteration kernel keeps two windows per warp: v to read, A^T u to accumulate)
-    int64_t win_bytes = (SMEM_BUDGET - instr_bytes - NWARP * 32 * 8) / NWARP / 2;
+    int64_t win_bytes = (SMEM_BUDGET - instr_bytes - NWARP * 48 * 8) / NWARP / 2;
     if (win_bytes > WIN_BYTES_MAX) win_bytes = WIN_BYTES_MAX;
     const int64_t n_start = d->n_dfa - 3;
     int64_t ws_max = win_bytes / 24;                       // doubles per axis
@@ -371,7 +371,7 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
     A->win = (int)bw + 3;
     A->wstride = (int)wstride;
     A->smem_bytes = (int)smem_bytes;
-    A->smem_fused = (int)(instr_bytes + NWARP * 6 * wstride * 8 + NWARP * 32 * 8);
+    A->smem_fused = (int)(instr_bytes + NWARP * 6 * wstride * 8 + NWARP * 48 * 8);
     A->ctas_per_sm = 2 * (smem_bytes + 2048) <= 227 * 1024 ? 2 : 1;
     A->stream = (cudaStream_t)stream;
     A->sm_count = prop.multiProcessorCount;
