@@ -348,7 +348,7 @@ def main():
             "roofline": {"bound": "hbm", "kernel": dom[0], "achieved": dom[1], "peak": peak,
                          "unit": "GB/s", "frac": dom[1] / peak, "traffic": traffic,
                          "traffic_note": "DRAM bytes per launch: ncu --set full bytes per row "
-                                         "(profiles/r1_v4_fused_ncu_full.md, r1_v4_aprod_ncu_full.md) x rows of this launch; the "
+                                         "(profiles/r1_v5_fused_ncu_full.md, r1_v4_aprod_ncu_full.md) x rows of this launch; the "
                                          "layout stores 212 B/row, so traffic < algorithmic bytes",
                          "peak_source": peak_src, "algorithmic_bytes_per_row": dom[3],
                          "ms_per_launch": dom[2]},
