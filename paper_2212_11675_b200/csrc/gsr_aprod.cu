@@ -535,6 +535,7 @@ __global__ void __launch_bounds__(TPB) k_aprod2_instr(const unsigned char* __res
     if (FIXED) {
         const double ynorm = sqrt(*ss_p);
         e = ynorm > 0.0 ? ilogb(ynorm) + 1 : 0;   // 2^e > ||y||
+        if (e < -900) e = -900;                   // keeps 2^(61-e) finite for a vanishing y
     }
     const double scale = FIXED ? scalbn(1.0, 61 - e) : 1.0;
     __syncthreads();
