@@ -1,6 +1,8 @@
 // aprod mode 1 and mode 2 (rows a3, a5-a8): Algorithms 1 and 2 of the paper
 // on the warp-tiled, attitude-binned layout of gsr_internal.h.
 //
+// Kernels: k_aprod1 / k_aprod2 (the two products, also behind gsr_aprod1/2), k_fused (both in one
+// read of the matrix, the solver's default iteration) and k_aprod2_instr (its instrumental pass).
 // Warps are autonomous.  A persistent grid (one or two CTAs of 16 warps per SM) fetches UNITS
 // (runs of 32-row tiles whose attitude blocks start inside one window of `win` knots per axis)
 // from a global counter, one unit per warp at a time.  In shared memory
@@ -51,11 +53,6 @@ __device__ __forceinline__ double ld_stream_f64(const void* p) {
 __device__ __forceinline__ int32_t ld_stream_s32(const void* p) {
     int32_t v;
     asm volatile("ld.global.cs.s32 %0, [%1];" : "=r"(v) : "l"(p));
-    return v;
-}
-__device__ __forceinline__ uint32_t ld_stream_u32(const void* p) {
-    uint32_t v;
-    asm volatile("ld.global.cs.u32 %0, [%1];" : "=r"(v) : "l"(p));
     return v;
 }
 __device__ __forceinline__ uint32_t ld_stream_u16(const void* p) {

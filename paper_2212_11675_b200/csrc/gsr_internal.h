@@ -66,7 +66,6 @@ constexpr int TPB = NWARP * 32;
 constexpr int SMEM_BUDGET = 224 * 1024;      // dynamic shared memory a product CTA may use
 constexpr int WIN_BYTES_MAX = 6 * 1024;      // per-warp attitude window, 3 axes (the fused
                                              // iteration kernel keeps two of them per warp)
-constexpr int STAGE_BYTES = 0;               // per-warp scratch besides the window
 constexpr int UNIT_TILES_MAX = 128;          // tiles per unit (upper bound)
 constexpr uint32_t PERM_PAD = 0xFFFFFFFFu;
 
