@@ -393,21 +393,34 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
             const int64_t ri = ((int64_t)un.tile0 + t) * R + lane;
             const double yold = __ldcs(y + ri);
             // ---- mode 1 for this tile
-            double p[16];
+            // products of rows q and q+8 are formed together and go straight into the first
+            // butterfly step, so that only 8 of the 16 partial products are ever live
+            double p[8];
             asm_[lane] = ra.aoff;
             __syncwarp();
+            {
+                const bool up8 = (j & 8) != 0;
 #pragma unroll
-            for (int g4 = 0; g4 < 4; ++g4) {
-                const uint4 a4 = *(const uint4*)(asm_ + h * 16 + 4 * g4);
-                const uint32_t aa[4] = {a4.x, a4.y, a4.z, a4.w};
+                for (int g4 = 0; g4 < 2; ++g4) {
+                    const uint4 alo = *(const uint4*)(asm_ + h * 16 + 4 * g4);
+                    const uint4 ahi = *(const uint4*)(asm_ + h * 16 + 4 * g4 + 8);
+                    const uint32_t al[4] = {alo.x, alo.y, alo.z, alo.w};
+                    const uint32_t ah[4] = {ahi.x, ahi.y, ahi.z, ahi.w};
 #pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    const double pv = ra.at[4 * g4 + i] * xw[aa[i] + axo];
-                    p[4 * g4 + i] = att_lane ? pv : 0.0;
+                    for (int i = 0; i < 4; ++i) {
+                        const int q0 = 4 * g4 + i;
+                        double plo = ra.at[q0] * xw[al[i] + axo];
+                        double phi = ra.at[q0 + 8] * xw[ah[i] + axo];
+                        plo = att_lane ? plo : 0.0;
+                        phi = att_lane ? phi : 0.0;
+                        const double send = up8 ? plo : phi;
+                        const double keep = up8 ? phi : plo;
+                        p[q0] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+                    }
                 }
             }
 #pragma unroll
-            for (int o = 8; o > 0; o >>= 1) {
+            for (int o = 4; o > 0; o >>= 1) {
                 const bool up = (j & o) != 0;
 #pragma unroll
                 for (int i = 0; i < o; ++i) {
