@@ -77,6 +77,19 @@ __device__ __forceinline__ void load_B(const unsigned char* __restrict__ T, int 
     r.gl = ld_stream_f64(T + OFF_GLOBV + lane * 8);
 }
 
+__device__ __forceinline__ void load_B_instr(const unsigned char* __restrict__ T, int lane, RegsB& r) {
+#pragma unroll
+    for (int j = 0; j < 6; ++j) r.c[j] = ld_stream_u16(T + OFF_ICOL + (j * R + lane) * 2);
+#pragma unroll
+    for (int j = 0; j < 6; ++j) r.in[j] = ld_stream_f64(T + OFF_INSTRV + (j * R + lane) * 8);
+}
+__device__ __forceinline__ void load_B_rest(const unsigned char* __restrict__ T, int lane, RegsB& r) {
+    r.s = ld_stream_s32(T + OFF_STAR + lane * 4);
+#pragma unroll
+    for (int k = 0; k < 5; ++k) r.as[k] = ld_stream_f64(T + OFF_ASTRO + (k * R + lane) * 8);
+    r.gl = ld_stream_f64(T + OFF_GLOBV + lane * 8);
+}
+
 __device__ __forceinline__ int fetch_unit(int* counter, int lane) {
     int u = 0;
     if (lane == 0) u = atomicAdd(counter, 1);
@@ -385,11 +398,17 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
         __syncwarp();
         double q = 0.0;
         const unsigned char* T = tiles + (int64_t)un.tile0 * TILE_BYTES;
+        // Loads are issued as soon as the registers they fill are dead (volatile asm keeps the
+        // program order): the next tile's instrumental values and columns right after mode 1,
+        // its attitude coefficients group by group inside the read-modify-write loop, the rest
+        // (star, astrometric, global) at the top of its own iteration.
         RegsA ra;
+        RegsB r;
         load_A(T, lane, ra);
+        load_B_instr(T, lane, r);
         for (int t = 0; t < un.ntiles; ++t, T += TILE_BYTES) {
-            RegsB r;
-            load_B(T, lane, r);
+            const unsigned char* Tn = t + 1 < un.ntiles ? T + TILE_BYTES : T;   // (last: harmless reload)
+            load_B_rest(T, lane, r);
             const int64_t ri = ((int64_t)un.tile0 + t) * R + lane;
             const double yold = __ldcs(y + ri);
             // ---- mode 1 for this tile
@@ -440,10 +459,12 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
             y[ri] = yv;
             ysm[lane] = yv;
             q = fma(yv, yv, q);
+            load_B_instr(Tn, lane, r);
             // ---- mode 2 for this tile, attitude
             const uint32_t a_other = __shfl_xor_sync(0xffffffffu, ra.aoff, 16);
             const int da = (int)ra.aoff - (int)a_other;
             const unsigned cmask = __ballot_sync(0xffffffffu, da > -4 && da < 4);
+            ra.aoff = ld_stream_u16(Tn + OFF_AOFF + lane * 2);
             __syncwarp();   // ysm visible to the whole warp
 #pragma unroll
             for (int g4 = 0; g4 < 4; ++g4) {
@@ -466,8 +487,10 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
                     }
                     __syncwarp();
                 }
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    ra.at[4 * g4 + i] = ld_stream_f64(Tn + OFF_ATTV + (((4 * g4 + i) * 2 + h) * 12 + jj) * 8);
             }
-            if (t + 1 < un.ntiles) load_A(T + TILE_BYTES, lane, ra);
             // ---- mode 2, global and astrometric
             g = fma(r.gl, yv, g);
 #pragma unroll
