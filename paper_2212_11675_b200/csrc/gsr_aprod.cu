@@ -237,7 +237,6 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
         RegsA ra;
         load_A(T, lane, ra);
         for (int t = 0; t < un.ntiles; ++t, T += TILE_BYTES) {
-            const unsigned char* Tn = t + 1 < un.ntiles ? T + TILE_BYTES : T;   // (last: harmless reload)
             RegsB r;
             load_B(T, lane, r);
             const int64_t ri = ((int64_t)un.tile0 + t) * R + lane;
@@ -273,10 +272,8 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
                     if (lo12 || hi12) *pa += add;
                 }
                 __syncwarp();
-                // the next tile's coefficient goes into the register that has just died
-                ra.at[qq] = ld_stream_f64(Tn + OFF_ATTV + ((qq * 2 + h) * 12 + jj) * 8);
             }
-            ra.aoff = ld_stream_u16(Tn + OFF_AOFF + lane * 2);
+            if (t + 1 < un.ntiles) load_A(T + TILE_BYTES, lane, ra);   // in flight during phase B
             // phase B
 #pragma unroll
             for (int k = 0; k < 5; ++k) r.as[k] = SQUARE ? r.as[k] * r.as[k] : r.as[k] * yv;
