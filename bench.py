@@ -37,7 +37,7 @@ BYTES_FUSED = BYTES_APROD1 + BYTES_APROD2 - BYTES_INSTR   # 392 algorithmic byte
 # DRAM bytes per row measured by `ncu --set full` (dram__bytes_read.sum + dram__bytes_write.sum
 # over the rows of the launch; profiles/r1_v2_aprod_ncu_full.md); multiplied by the rows of the
 # timed launch to give roofline.traffic
-NCU_TRAFFIC_PER_ROW = {"aprod1": 228.2, "aprod2": 220.4, "fused": 228.3, "aprod2_instr": 68.1}
+NCU_TRAFFIC_PER_ROW = {"aprod1": 228.2, "aprod2": 220.4, "fused": 229.1, "aprod2_instr": 68.1}
 GEN_ROWS = 1 << 23                              # rows generated and appended per chunk
 
 
@@ -348,7 +348,7 @@ def main():
             "roofline": {"bound": "hbm", "kernel": dom[0], "achieved": dom[1], "peak": peak,
                          "unit": "GB/s", "frac": dom[1] / peak, "traffic": traffic,
                          "traffic_note": "DRAM bytes per launch: ncu --set full bytes per row "
-                                         "(profiles/r1_v5_fused_ncu_full.md, r1_v4_aprod_ncu_full.md) x rows of this launch; the "
+                                         "(profiles/r1_v6_fused_ncu_full.md, r1_v4_aprod_ncu_full.md) x rows of this launch; the "
                                          "layout stores 212 B/row, so traffic < algorithmic bytes",
                          "peak_source": peak_src, "algorithmic_bytes_per_row": dom[3],
                          "ms_per_launch": dom[2]},
