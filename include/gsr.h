@@ -140,6 +140,20 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
  * GSR_ESTATE if no solve has finished on the handle.  Synchronises if se_hd is host memory. */
 int gsr_lsqr_standard_errors(gsr_matrix* A, double* se_hd, gsr_stream stream);
 
+/* ---- constraint equations (PAPER.md:65; "constraints computation", Algorithms 1-2, :280, :390) --
+ * "To find a unique solution, an additional number of constraint equations have to be set."  The
+ * paper does not give their structure: here they are n_con extra rows in general CSR form
+ * appended BELOW the m observation rows (row m+r has val[e] at column col[e] for e in
+ * [row_ptr[r], row_ptr[r+1]); columns in [0, n_cols)).  Arrays may be host or device and are
+ * copied.  Call after create/finalize and before gsr_precondition / gsr_lsqr_solve; n_con = 0
+ * removes them.  Afterwards every m-sized vector of the API (y of gsr_aprod1/2, b of
+ * gsr_lsqr_solve) has m + n_con entries, observations first; gsr_precondition counts the
+ * constraint coefficients in the column norms and scales them too.
+ * Errors: GSR_EINVAL (bad row_ptr, column out of range), GSR_ESTATE, GSR_EUNSUPPORTED (with a
+ * communicator).  Synchronous. */
+int gsr_matrix_set_constraints(gsr_matrix* A, int64_t n_con, const int64_t* row_ptr_hd,
+                               const int32_t* col_hd, const double* val_hd);
+
 /* ---- row-sharded solve over several GPUs (Fig. 2; Algorithm 3 lines 8-16) --
  * One process per GPU.  The observation rows are split into contiguous star-aligned blocks
  * (paper_2212_11675_b200/sharding.py); every rank builds an ORDINARY matrix from its block, with

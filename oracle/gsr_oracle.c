@@ -58,6 +58,26 @@ typedef struct {
 
 static int64_t n_cols(const orc_dims* d) { return 5 * d->n_stars + 3 * d->n_dfa + d->n_instr + 1; }
 
+/* Constraint equations: "to find a unique solution, an additional number of constraint equations
+ * have to be set"; both aprod modes end with a "constraints computation"
+ * (Algorithms 1 and 2).  The paper does not give their structure, so
+ * they are n_con extra rows in general CSR form appended below the m observation rows: row m+r
+ * has coefficients val[e] at columns col[e], e in [row_ptr[r], row_ptr[r+1]).  Set once per call
+ * by the Python wrapper (the oracle is single-threaded test infrastructure); n_con = 0: none. */
+typedef struct {
+    int64_t n_con;
+    const int64_t* row_ptr;
+    const int32_t* col;
+    double* val;
+} orc_con;
+static orc_con g_con = {0, NULL, NULL, NULL};
+void orc_set_constraints(int64_t n_con, const int64_t* row_ptr, const int32_t* col, double* val) {
+    g_con.n_con = n_con;
+    g_con.row_ptr = row_ptr;
+    g_con.col = col;
+    g_con.val = val;
+}
+
 /* Column of stored coefficient k of row i.  Section 3 and the index
  * expressions of Algorithm 1: astrometric x[j+offset[i]], offset = 5*star;
  * attitude k2 = j1*N_DFA + offset[i], x[j2+k2]; instrumental
@@ -118,6 +138,17 @@ void orc_aprod1(const orc_dims* d, const int32_t* star_idx, const int32_t* att_s
         if (scale) scale[i] = fabs(b[i]) + asum;
         b[i] = b[i] + sum;
     }
+    for (int64_t r = 0; r < g_con.n_con; ++r) { /* constraints computation */
+        const int64_t i = d->n_rows + r;
+        double sum = 0.0, asum = 0.0;
+        for (int64_t e = g_con.row_ptr[r]; e < g_con.row_ptr[r + 1]; ++e) {
+            double t = g_con.val[e] * x[g_con.col[e]];
+            sum = sum + t;
+            asum = asum + fabs(t);
+        }
+        if (scale) scale[i] = fabs(b[i]) + asum;
+        b[i] = b[i] + sum;
+    }
 }
 
 /* aprod mode 2: x[col] = x[col] + A_d[k]*b[i], rows in order,
@@ -141,6 +172,12 @@ void orc_aprod2(const orc_dims* d, const int32_t* star_idx, const int32_t* att_s
             if (aacc) aacc[c] += fabs(t);
         }
     }
+    for (int64_t r = 0; r < g_con.n_con; ++r) /* constraints computation */
+        for (int64_t e = g_con.row_ptr[r]; e < g_con.row_ptr[r + 1]; ++e) {
+            double t = g_con.val[e] * b[d->n_rows + r];
+            acc[g_con.col[e]] += t;
+            if (aacc) aacc[g_con.col[e]] += fabs(t);
+        }
     for (int64_t j = 0; j < n; ++j) {
         x[j] = (double)acc[j];
         if (aacc) scale[j] = (double)aacc[j];
@@ -159,6 +196,8 @@ void orc_colsumsq(const orc_dims* d, const int32_t* star_idx, const int32_t* att
             double a = A_d[i * N_PAR + k];
             acc[col_of(d, star_idx, att_start, instr_col, i, k)] += (long double)a * a;
         }
+    for (int64_t e = 0; g_con.n_con > 0 && e < g_con.row_ptr[g_con.n_con]; ++e)
+        acc[g_con.col[e]] += (long double)g_con.val[e] * g_con.val[e];
     for (int64_t j = 0; j < n; ++j) q[j] = (double)acc[j];
     free(acc);
 }
@@ -173,6 +212,8 @@ void orc_precondition(const orc_dims* d, const int32_t* star_idx, const int32_t*
     for (int64_t i = 0; i < d->n_rows; ++i)
         for (int k = 0; k < N_PAR; ++k)
             A_d[i * N_PAR + k] = A_d[i * N_PAR + k] * p[col_of(d, star_idx, att_start, instr_col, i, k)];
+    for (int64_t e = 0; g_con.n_con > 0 && e < g_con.row_ptr[g_con.n_con]; ++e)
+        g_con.val[e] = g_con.val[e] * p[g_con.col[e]];
 }
 
 static double nrm2(const double* v, int64_t len) {
@@ -198,7 +239,7 @@ int orc_lsqr_var(const orc_dims* d, const int32_t* star_idx, const int32_t* att_
                  const int32_t* instr_col, const double* A_d, const double* b, double* x,
                  int64_t itnlim, double atol, double btol, double conlim, int force_itnlim,
                  orc_result* res, double* hist, double* var) {
-    const int64_t m = d->n_rows, n = n_cols(d);
+    const int64_t m = d->n_rows + g_con.n_con, n = n_cols(d);   /* b, u: observations then constraints */
     if (var)
         for (int64_t j = 0; j < n_cols(d); ++j) var[j] = 0.0;
     double* u = (double*)malloc(sizeof(double) * (size_t)(m > 0 ? m : 1));

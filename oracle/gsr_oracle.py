@@ -91,6 +91,28 @@ class OracleSystem:
         self.n = 5 * self.n_stars + 3 * self.n_dfa + self.n_instr + 1
         self.dims = _Dims(self.m, self.n_stars, self.n_dfa, self.n_instr)
         self.p = None
+        self.n_con, self.con_ptr, self.con_col, self.con_val = 0, None, None, None
+
+    def set_constraints(self, row_ptr, col, val):
+        """n_con extra rows in CSR form appended below the observations.
+        From now on m-vectors have m + n_con entries.  `val` is copied (precondition scales it)."""
+        self.con_ptr = np.ascontiguousarray(row_ptr, dtype=np.int64)
+        self.con_col = np.ascontiguousarray(col, dtype=np.int32)
+        self.con_val = np.array(val, dtype=np.float64, order="C", copy=True)
+        self.n_con = int(self.con_ptr.shape[0]) - 1
+        assert self.con_ptr[0] == 0 and self.con_ptr[-1] == self.con_col.shape[0] == self.con_val.shape[0]
+        assert self.con_col.size == 0 or (self.con_col.min() >= 0 and self.con_col.max() < self.n)
+
+    @property
+    def m_total(self) -> int:
+        return self.m + self.n_con
+
+    def _con(self, on=True):
+        if self.n_con and on:
+            lib().orc_set_constraints(C.c_int64(self.n_con), _p(self.con_ptr, C.c_int64),
+                                      _p(self.con_col, C.c_int32), _p(self.con_val, C.c_double))
+        else:
+            lib().orc_set_constraints(C.c_int64(0), None, None, None)
 
     def _idx(self):
         return (C.byref(self.dims), _p(self.star_idx, C.c_int32), _p(self.att_start, C.c_int32),
@@ -111,32 +133,40 @@ class OracleSystem:
         """y += A x (in place on a copy); returns y or (y, scale)."""
         x = np.ascontiguousarray(x, dtype=np.float64)
         y = np.array(y, dtype=np.float64, copy=True)
-        assert x.shape == (self.n,) and y.shape == (self.m,)
-        sc = np.empty(self.m) if want_scale else None
+        assert x.shape == (self.n,) and y.shape == (self.m_total,)
+        sc = np.empty(self.m_total) if want_scale else None
+        self._con()
         lib().orc_aprod1(*self._idx(), _p(self.values, C.c_double), _p(x, C.c_double),
                          _p(y, C.c_double), _p(sc, C.c_double))
+        self._con(False)
         return (y, sc) if want_scale else y
 
     def aprod2(self, y, x, want_scale=False):
         """x += A^T y (on a copy); returns x or (x, scale)."""
         y = np.ascontiguousarray(y, dtype=np.float64)
         x = np.array(x, dtype=np.float64, copy=True)
-        assert x.shape == (self.n,) and y.shape == (self.m,)
+        assert x.shape == (self.n,) and y.shape == (self.m_total,)
         sc = np.empty(self.n) if want_scale else None
+        self._con()
         lib().orc_aprod2(*self._idx(), _p(self.values, C.c_double), _p(y, C.c_double),
                          _p(x, C.c_double), _p(sc, C.c_double))
+        self._con(False)
         return (x, sc) if want_scale else x
 
     def colsumsq(self):
         q = np.empty(self.n)
+        self._con()
         lib().orc_colsumsq(*self._idx(), _p(self.values, C.c_double), _p(q, C.c_double))
+        self._con(False)
         return q
 
     def precondition(self):
         """Scales self.values in place, keeps and returns p."""
         assert self.p is None, "already preconditioned"
         p = np.empty(self.n)
+        self._con()
         lib().orc_precondition(*self._idx(), _p(self.values, C.c_double), _p(p, C.c_double))
+        self._con(False)
         self.p = p
         return p
 
@@ -144,21 +174,23 @@ class OracleSystem:
              want_hist=False, want_se=False) -> LsqrResult:
         """min ||A x - b||.  If preconditioned, iterates on A.diag(p), returns x = p (.) z."""
         b = np.ascontiguousarray(b, dtype=np.float64)
-        assert b.shape == (self.m,)
+        assert b.shape == (self.m_total,)
         x = np.empty(self.n)
         res = _Result()
         hist = np.zeros((int(itnlim), 7)) if want_hist else None
         var = np.zeros(self.n) if want_se else None
+        self._con()
         rc = lib().orc_lsqr_var(*self._idx(), _p(self.values, C.c_double), _p(b, C.c_double),
                                 _p(x, C.c_double), C.c_int64(itnlim), C.c_double(atol),
                                 C.c_double(btol), C.c_double(conlim),
                                 C.c_int(1 if force_itnlim else 0), C.byref(res),
                                 _p(hist, C.c_double), _p(var, C.c_double))
+        self._con(False)
         assert rc == 0
         se = None
         if want_se:
             se = np.empty(self.n)
-            lib().orc_standard_errors(C.c_int64(self.m), C.c_int64(self.n), C.c_double(res.rnorm),
+            lib().orc_standard_errors(C.c_int64(self.m_total), C.c_int64(self.n), C.c_double(res.rnorm),
                                       _p(var, C.c_double), _p(self.p, C.c_double), _p(se, C.c_double))
         if self.p is not None:
             lib().orc_unscale(C.c_int64(self.n), _p(self.p, C.c_double), _p(x, C.c_double))

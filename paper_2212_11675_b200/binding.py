@@ -21,7 +21,7 @@ EXPORTS = [
     "gsr_matrix_destroy", "gsr_matrix_dims", "gsr_matrix_device_bytes", "gsr_aprod1",
     "gsr_aprod2", "gsr_precondition", "gsr_lsqr_solve", "gsr_set_option", "gsr_strerror",
     "gsr_debug_expand_rows", "gsr_time_product", "gsr_launch_count", "gsr_lsqr_standard_errors",
-    "gsr_comm_unique_id", "gsr_comm_create", "gsr_comm_destroy", "gsr_matrix_set_comm",
+    "gsr_matrix_set_constraints", "gsr_comm_unique_id", "gsr_comm_create", "gsr_comm_destroy", "gsr_matrix_set_comm",
 ]
 
 
@@ -83,6 +83,7 @@ def lib():
         L.gsr_precondition.argtypes = [vp, vp, vp]
         L.gsr_lsqr_solve.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl, C.POINTER(gsr_lsqr_result), vp]
         L.gsr_lsqr_standard_errors.argtypes = [vp, vp, vp]
+        L.gsr_matrix_set_constraints.argtypes = [vp, i64, vp, vp, vp]
         L.gsr_comm_unique_id.argtypes = [vp, i64]
         L.gsr_comm_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, vp, i64]
         L.gsr_comm_destroy.argtypes = [vp]
@@ -197,6 +198,12 @@ def gsr_lsqr_solve(h, b, x, itnlim, atol=0.0, btol=0.0, conlim=0.0, stream=None)
 
 def gsr_lsqr_standard_errors(h, se, stream=None):
     _check(lib().gsr_lsqr_standard_errors(h, _ptr(se), _stream(stream)), "gsr_lsqr_standard_errors")
+
+
+def gsr_matrix_set_constraints(h, n_con, row_ptr, col, val):
+    """row_ptr int64 [n_con+1], col int32 [nnz], val float64 [nnz] (numpy, torch or None)."""
+    _check(lib().gsr_matrix_set_constraints(h, int(n_con), _ptr(row_ptr), _ptr(col), _ptr(val)),
+           "gsr_matrix_set_constraints")
 
 
 GSR_COMM_ID_BYTES = 128

@@ -764,13 +764,15 @@ extern "C" {
 int gsr_aprod1(const gsr_matrix* A, const double* x_dev, double* y_dev, gsr_stream stream) {
     if (!A || !x_dev || (!y_dev && A->dims.n_rows > 0)) return GSR_EINVAL;
     if (A->state != 1) return GSR_ESTATE;
-    return launch_aprod1(A, x_dev, y_dev, A->coef_one, nullptr, nullptr, A->perm, (cudaStream_t)stream);
+    GSR_TRY(launch_aprod1(A, x_dev, y_dev, A->coef_one, nullptr, nullptr, A->perm, (cudaStream_t)stream));
+    return launch_con_aprod1(A, x_dev, y_dev + A->dims.n_rows, A->coef_one, nullptr, nullptr, (cudaStream_t)stream);
 }
 
 int gsr_aprod2(const gsr_matrix* A, const double* y_dev, double* x_dev, gsr_stream stream) {
     if (!A || !x_dev || (!y_dev && A->dims.n_rows > 0)) return GSR_EINVAL;
     if (A->state != 1) return GSR_ESTATE;
-    return launch_aprod2(A, y_dev, x_dev, A->coef_one, nullptr, A->perm, (cudaStream_t)stream);
+    GSR_TRY(launch_aprod2(A, y_dev, x_dev, A->coef_one, nullptr, A->perm, (cudaStream_t)stream));
+    return launch_con_aprod2(A, y_dev + A->dims.n_rows, x_dev, A->coef_one, nullptr, (cudaStream_t)stream);
 }
 
 }  // extern "C"

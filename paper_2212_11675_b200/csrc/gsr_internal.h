@@ -161,6 +161,10 @@ struct gsr_matrix {
     int opt_force_itnlim;
     int opt_two_pass;               // 1: aprod1 + aprod2 per iteration instead of the fused pass
     int opt_no_fixed;               // 1: fp64 atomics in the instrumental pass even when scaled
+    int64_t n_con, con_nnz;         // row f3: constraint rows (CSR) appended below the observations
+    int64_t* con_ptr;
+    int32_t* con_col;
+    double* con_val;
     gsr_comm* comm;                 // row e: this handle is one row shard (nullptr: whole system)
     int64_t m_global, n_global;     // rows / columns of the whole system (= local without comm)
     int sm_count;
@@ -188,6 +192,16 @@ inline void count_launch(long long k = 1) { g_launches += k; }
     } while (0)
 
 int comm_allreduce_sum(gsr_comm* c, double* buf, size_t count, cudaStream_t s);
+// constraint rows (gsr_constraints.cu); all are no-ops when the handle has none
+int launch_con_aprod1(const gsr_matrix* A, const double* x, double* ycon, const double* ca,
+                      double* partial, const int* stop, cudaStream_t s);
+int launch_con_aprod2(const gsr_matrix* A, const double* ycon, double* x, const double* sy,
+                      const int* stop, cudaStream_t s);
+int launch_con_colsumsq(const gsr_matrix* A, double* q, cudaStream_t s);
+int launch_con_scale(const gsr_matrix* A, const double* p, cudaStream_t s);
+int launch_con_copy_sumsq(const gsr_matrix* A, const double* bcon, double* ucon, double* partial,
+                          cudaStream_t s);
+void free_constraints(gsr_matrix* A);
 int dev_alloc(gsr_matrix* A, void** p, size_t bytes);
 void dev_free(gsr_matrix* A, void* p, size_t bytes);
 bool is_device_ptr(const void* p);

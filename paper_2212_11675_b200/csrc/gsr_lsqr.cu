@@ -345,20 +345,20 @@ int ensure_workspace(gsr_matrix* A) {
     if (W.st) return GSR_OK;
     const size_t n8 = (size_t)A->n_cols * 8;
     int64_t npu = A->n_units > NB_N ? A->n_units : NB_N;
-    GSR_TRY(dev_alloc(A, (void**)&W.u, (size_t)A->m_int * 8));
+    GSR_TRY(dev_alloc(A, (void**)&W.u, (size_t)(A->m_int + A->n_con) * 8));   // constraint rows at the end
     GSR_TRY(dev_alloc(A, (void**)&W.v, n8));
     GSR_TRY(dev_alloc(A, (void**)&W.w, n8));
     GSR_TRY(dev_alloc(A, (void**)&W.x, n8));
     GSR_TRY(dev_alloc(A, (void**)&W.t, n8 + 16));   // t[n]: local sum of u_hat^2 (sharded solve)
     GSR_TRY(dev_alloc(A, (void**)&W.var, n8));
-    GSR_TRY(dev_alloc(A, (void**)&W.part_u, (size_t)npu * 8));
+    GSR_TRY(dev_alloc(A, (void**)&W.part_u, (size_t)(npu + 1) * 8));   // + one slot for the constraint rows
     GSR_TRY(dev_alloc(A, (void**)&W.part_v, NB_N * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.part_w, NB_N * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.part_va, NB_N * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.part_wa, NB_N * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.red, 4 * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.st, sizeof(LsqrState)));
-    GSR_CUDA_TRY(cudaMemset(W.u, 0, (size_t)A->m_int * 8));
+    GSR_CUDA_TRY(cudaMemset(W.u, 0, (size_t)(A->m_int + A->n_con) * 8));
     GSR_CUDA_TRY(cudaMemset(W.st, 0, sizeof(LsqrState)));
     GSR_CUDA_TRY(cudaMallocHost((void**)&W.stop_host, 64));
     return GSR_OK;
@@ -382,26 +382,32 @@ void free_workspace(gsr_matrix* A) {
 // together, k_aprod2_instr adds the instrumental block of t, k_vnew forms v = t/beta - beta v.
 // Two-pass form (GSR_OPT_FUSED = 0): aprod1, then aprod2 on the pre-scaled v.
 static int kernels_per_iteration(const gsr_matrix* A) {
-    return A->opt_two_pass ? 8 : (A->comm ? 10 : 8);
+    return (A->opt_two_pass ? 8 : (A->comm ? 10 : 8)) + (A->n_con > 0 ? 2 : 0);
 }
 
 static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
     Workspace& W = A->ws;
     const int64_t n = A->n_cols;
     const int64_t split = A->comm ? A->off_att : 0;   // sharded: [0, split) distributed slice
+    const int ncp = A->n_con > 0 ? 1 : 0;             // one more partial of u_hat^2 (constraint rows)
     if (A->opt_two_pass) {
         // bidiagonalisation, first half: u_hat <- A v - (alpha/beta) u_hat ; partials of u_hat^2
         GSR_TRY(launch_aprod1(A, W.v, W.u, &W.st->ca, W.part_u, &W.st->stop, nullptr, s));
-        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_units);
+        GSR_TRY(launch_con_aprod1(A, W.v, W.u + A->m_int, &W.st->ca, W.part_u + A->n_units, &W.st->stop, s));
+        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_units + ncp);
         // second half: v <- A^T (u_hat/beta) - beta v
         k_prescale<<<NB_N, TB_N, 0, s>>>(W.v, n, W.st);
         GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s));
+        GSR_TRY(launch_con_aprod2(A, W.u + A->m_int, W.v, &W.st->inv_beta, &W.st->stop, s));
         k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop, 0, nullptr);
         k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N, nullptr);
         k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, nullptr, W.var, 0, nullptr);
     } else if (!A->comm) {
         GSR_TRY(launch_fused(A, W.v, W.u, &W.st->ca, W.part_u, W.t, &W.st->stop, s));
-        k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units, W.red + 3, &W.st->stop);
+        // constraint rows (row f3): same two steps on the CSR block, u_hat[m_int ..]
+        GSR_TRY(launch_con_aprod1(A, W.v, W.u + A->m_int, &W.st->ca, W.part_u + A->n_units, &W.st->stop, s));
+        GSR_TRY(launch_con_aprod2(A, W.u + A->m_int, W.t, A->coef_one, &W.st->stop, s));
+        k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units + ncp, W.red + 3, &W.st->stop);
         GSR_TRY(launch_aprod2_instr(A, W.u, W.t, W.red + 3, &W.st->stop, s));
         k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.red + 3, 1);
         k_vnew<<<NB_N, TB_N, 0, s>>>(W.v, W.t, n, W.st, W.part_v, 0, nullptr);
@@ -484,8 +490,9 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     cudaStream_t s = (cudaStream_t)stream;
     Workspace& W = A->ws;
     GSR_TRY(ensure_workspace(A));
-    const int64_t m = A->dims.n_rows, n = A->n_cols;
+    const int64_t m = A->dims.n_rows + A->n_con, n = A->n_cols;   // b: observations then constraints
     memset(result, 0, sizeof(*result));
+    if (A->comm && A->n_con > 0) return GSR_EUNSUPPORTED;
 
     // b -> device
     const double* b_dev = b_hd;
@@ -519,10 +526,13 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
         k_scalar_init1<<<1, 1024, 0, s>>>(W.st, W.red + 2, 1);
         count_launch();
     } else {
-        k_scalar_init1<<<1, 1024, 0, s>>>(W.st, W.part_u, NB_N);
+        if (A->n_con > 0)
+            GSR_TRY(launch_con_copy_sumsq(A, b_dev + A->dims.n_rows, W.u + A->m_int, W.part_u + NB_N, s));
+        k_scalar_init1<<<1, 1024, 0, s>>>(W.st, W.part_u, NB_N + (A->n_con > 0 ? 1 : 0));
     }
     count_launch(2);
     GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s));
+    GSR_TRY(launch_con_aprod2(A, W.u + A->m_int, W.v, &W.st->inv_beta, &W.st->stop, s));
     if (A->comm)     // replicated slice of v = A^T u: sum of the shards' contributions
         GSR_TRY(comm_allreduce_sum(A->comm, W.v + split, (size_t)(n - split), s));
     k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop, split, W.part_va);

@@ -488,6 +488,7 @@ int gsr_matrix_destroy(gsr_matrix* A) {
     if (!A) return GSR_OK;
     free_workspace(A);
     free_staging(A);
+    free_constraints(A);
     cudaFree(A->tiles);
     cudaFree(A->perm);
     cudaFree(A->units);
@@ -561,6 +562,7 @@ int gsr_precondition(gsr_matrix* A, double* p_out, gsr_stream stream) {
     GSR_TRY(dev_alloc(A, (void**)&A->p, (size_t)A->n_cols * 8));
     GSR_CUDA_TRY(cudaMemsetAsync(A->p, 0, (size_t)A->n_cols * 8, s));
     GSR_TRY(launch_colsumsq(A, A->p, s));
+    GSR_TRY(launch_con_colsumsq(A, A->p, s));
     if (A->comm)   // column norms of the replicated slice are sums over all row shards
         GSR_TRY(comm_allreduce_sum(A->comm, A->p + A->off_att, (size_t)(A->n_cols - A->off_att), s));
     k_make_p<<<(unsigned)((A->n_cols + 255) / 256), 256, 0, s>>>(A->p, A->n_cols);
@@ -570,6 +572,7 @@ int gsr_precondition(gsr_matrix* A, double* p_out, gsr_stream stream) {
             A->tiles, A->n_tiles, A->p, A->dims.n_stars, A->dims.n_dfa, A->dims.n_instr);
         count_launch();
     }
+    GSR_TRY(launch_con_scale(A, A->p, s));
     GSR_CUDA_TRY(cudaGetLastError());
     if (p_out) {
         GSR_CUDA_TRY(cudaMemcpyAsync(p_out, A->p, (size_t)A->n_cols * 8, cudaMemcpyDefault, s));
