@@ -23,6 +23,8 @@
  * adjoint identity, dense lstsq / normal equations on tiny systems, Krylov-subspace
  * minimiser at fixed k, consistent-system recovery, block-diagonal per-star 5x5 solves,
  * unit column norms, scipy.sparse.linalg.lsqr as a black box.
+ * Constraint equations (row f3): extra CSR rows below the observations, pinned by the dense
+ * augmented matrix (tests/test_constraints.py).
  * Standard errors (row f1): Paige & Saunders' var_j = sum_k (w_j/rho_k)^2, pinned by
  * diag((A^T A)^-1) on tiny systems run to finite termination.
  * parity unpinned: the authors' own "modified" LSQR and their variance formula, covariances,
