@@ -286,7 +286,9 @@ def main():
     torch.cuda.profiler.stop()
     barrier()
     launches = g.gsr_launch_count() - l0
-    ms = e0.elapsed_time(e1)
+    ms_solve = e0.elapsed_time(e1)            # whole call: initialisation + K iterations + x
+    ms = g.gsr_lsqr_last_loop_ms(h)           # exactly the K iterations (CUDA events on the stream)
+    assert 0.0 < ms <= ms_solve
     clocks = sampler.finish()
     assert res.itn == K and res.istop == 7, res
 
@@ -368,6 +370,10 @@ def main():
             "lsqr": {"istop": res.istop, "itn": res.itn, "rnorm": res.rnorm, "anorm": res.anorm,
                      "acond": res.acond, "xnorm": res.xnorm, "istop_natural": res.istop_natural,
                      "itn_natural": res.itn_natural},
+            "solve_call_ms": ms_solve,
+            "timing": "value = K / device time of the K iterations (CUDA events inside gsr_lsqr_solve on "
+                      "the launching stream); solve_call_ms also has the initialisation (one aprod2) "
+                      "and the finalisation; e2e is the wall clock of the whole call with host buffers",
             "setup_s": t_setup, "matrix_device_gb": g.gsr_matrix_device_bytes(h) * 1e-9,
         }
         if world == 1 and not args.no_cpu_baseline:

@@ -211,6 +211,12 @@ int gsr_debug_expand_rows(const gsr_matrix* A, int64_t row0, int64_t nrows, int6
  * Scratch vectors inside the handle are used; results are discarded.  Synchronous. */
 int gsr_time_product(gsr_matrix* A, int which, int reps, float* ms_avg, gsr_stream stream);
 
+/* Device time (ms, CUDA events on the solve's stream) of the ITERATION LOOP of the last
+ * gsr_lsqr_solve on this handle: from the first iteration's first kernel to the last iteration's
+ * last one, without the initialisation (row a2) and the finalisation (row a12).  -1 before any
+ * solve.  bench.py times "exactly K steps" with it. */
+double gsr_lsqr_last_loop_ms(const gsr_matrix* A);
+
 /* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */
 int64_t gsr_launch_count(void);
 

@@ -104,6 +104,8 @@ struct Workspace {
     double* var = nullptr;      // [n]  sum over the iterations of (w_j / rho)^2 (row f1)
     bool solved = false;        // var / last_rnorm belong to a finished solve
     double last_rnorm = 0.0;
+    double last_loop_ms = 0.0;  // device time of the iteration loop of the last solve
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     double* part_u = nullptr;   // [max(n_units, NB_N)] per-unit partial sums of u_hat^2
     double* part_v = nullptr;   // [NB_N]  (sharded: replicated slice only)
     double* part_w = nullptr;   // [NB_N]
