@@ -41,6 +41,8 @@ class GsrConfig:
     counts: Optional[tuple] = None    # explicit rows per star (micro cases)
     att_hot: Optional[tuple] = None   # (frac_rows, win_lo_frac, win_hi_frac) concentrated knots
     col_scales: bool = False          # per-column scale 10^U(-4,4) (config 4)
+    att_time_ordered: bool = False    # rows of a star in time order: att_start non-decreasing
+                                      # inside every star (per generation chunk), as in real scans
     noise_sigma: float = 1e-3
     iterations: int = 0
 
@@ -246,6 +248,8 @@ def gen_rows(cfg: GsrConfig, row0: int, nrows: int, device="cpu",
             hot = torch.rand(n, device=device, generator=gh, dtype=torch.float64) < frac
             ah = torch.randint(lo, hi, (n,), device=device, generator=gh, dtype=torch.int64)
             a = torch.where(hot, ah, a)
+        if cfg.att_time_ordered:   # same multiset of knots per star, visited in increasing order
+            a = a[torch.argsort(st * n_start + a)]
         att[sl] = a.to(torch.int32)
         g = _gen(device, cfg.seed, _S_INSTR, c)
         ic = _instr_distinct(n, cfg.n_instr, device, g)

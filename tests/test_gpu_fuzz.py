@@ -20,7 +20,8 @@ def _case(rng, it):
     I = int(rng.choice([1, 2, 6, 60, 700, 768, 769, 3000, 12000]))
     hot = (0.9, 0.4, 0.45) if rng.random() < 0.3 else None
     return inputs.micro_config(f"fuzz{it}", int(rng.integers(1, 1 << 30)), counts, D, I, att_hot=hot,
-                               col_scales=bool(rng.random() < 0.3))
+                               col_scales=bool(rng.random() < 0.3),
+                               att_time_ordered=bool(rng.random() < 0.3))   # time-ordered scans (row f4)
 
 
 @pytest.mark.parametrize("seed", [11, 12, 13])
