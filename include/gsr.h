@@ -176,6 +176,12 @@ int gsr_comm_create(gsr_comm** out, int rank, int world, const void* id_in, int6
 int gsr_comm_destroy(gsr_comm* c);
 int gsr_matrix_set_comm(gsr_matrix* A, gsr_comm* c, int64_t n_rows_global, int64_t n_cols_global);
 
+/* Damped LSQR (Paige & Saunders' damp parameter; the paper's solver is undamped, damp = 0, the
+ * default): the next solves on this handle minimise || [A; damp I] x - [b; 0] ||_2 (on the
+ * column-scaled system if A was preconditioned); result->rnorm is then the norm of that
+ * augmented residual.  damp >= 0, else GSR_EINVAL. */
+int gsr_lsqr_set_damp(gsr_matrix* A, double damp);
+
 /* Options (per handle). */
 enum {
     GSR_OPT_FORCE_ITNLIM = 1, /* 1: rules 1-6 are evaluated and recorded in *_natural but only

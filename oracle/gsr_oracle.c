@@ -230,6 +230,12 @@ static double sumsq(const double* v, int64_t len) {
 }
 static double hyp(double a, double b) { return sqrt(a * a + b * b); } /* reading A15 */
 
+/* Damping (row f4; Paige & Saunders 1982, section 2 of the algorithm paper): with damp > 0 LSQR
+ * minimises || [A; damp I] x - [b; 0] ||.  The paper does not use it (damp = 0, the default);
+ * set by the Python wrapper around a call, like the constraints. */
+static double g_damp = 0.0;
+void orc_set_damp(double damp) { g_damp = damp; }
+
 /* LSQR, Paige & Saunders 1982 (cited PAPER.md:27, 699-700), damp = 0; reading C3.
  * force_itnlim != 0 (reading A9): rules 1-6 are evaluated and recorded in *_natural but only
  * the iteration limit ends the loop.  hist (may be NULL) receives per iteration
@@ -250,6 +256,8 @@ int orc_lsqr_var(const orc_dims* d, const int32_t* star_idx, const int32_t* att_
     const double ctol = conlim > 0.0 ? 1.0 / conlim : 0.0;
     double anorm = 0, acond = 0, ddnorm = 0, xxnorm = 0, z = 0, cs2 = -1, sn2 = 0;
     double alpha = 0, beta, rhobar, phibar, bnorm, rnorm, arnorm = 0, xnorm = 0;
+    const double damp = g_damp;
+    double res2 = 0.0; /* sum of psi^2: the part of the residual that the damping rows hold */
     int istop = 0;
     int64_t itn = 0;
     memset(res, 0, sizeof(*res));
@@ -283,15 +291,24 @@ int orc_lsqr_var(const orc_dims* d, const int32_t* star_idx, const int32_t* att_
         if (beta > 0.0) {
             for (int64_t i = 0; i < m; ++i) u[i] = u[i] / beta;
             anorm = hyp(hyp(anorm, alpha), beta);
+            if (damp > 0.0) anorm = hyp(anorm, damp);
             for (int64_t j = 0; j < n; ++j) v[j] = -beta * v[j];
             orc_aprod2(d, star_idx, att_start, instr_col, A_d, u, v, NULL);
             alpha = nrm2(v, n);
             if (alpha > 0.0)
                 for (int64_t j = 0; j < n; ++j) v[j] = v[j] / alpha;
         }
+        /* plane rotation eliminating the damping parameter (only when damp > 0) */
+        double rhobar1 = rhobar, psi = 0.0;
+        if (damp > 0.0) {
+            rhobar1 = hyp(rhobar, damp);
+            double cs1 = rhobar / rhobar1, sn1 = damp / rhobar1;
+            psi = sn1 * phibar;
+            phibar = cs1 * phibar;
+        }
         /* plane rotation eliminating beta */
-        double rho = hyp(rhobar, beta);
-        double cs = rhobar / rho, sn = beta / rho;
+        double rho = hyp(rhobar1, beta);
+        double cs = rhobar1 / rho, sn = beta / rho;
         double theta = sn * alpha;
         rhobar = -cs * alpha;
         double phi = cs * phibar;
@@ -322,7 +339,8 @@ int orc_lsqr_var(const orc_dims* d, const int32_t* star_idx, const int32_t* att_
         xxnorm = xxnorm + z * z;
         /* norms and stopping tests */
         acond = anorm * sqrt(ddnorm);
-        rnorm = phibar;
+        res2 = res2 + psi * psi;
+        rnorm = damp > 0.0 ? sqrt(phibar * phibar + res2) : phibar;
         arnorm = alpha * fabs(tau);
         double test1 = rnorm / bnorm;
         double test2 = (anorm * rnorm > 0.0) ? arnorm / (anorm * rnorm) : INFINITY; /* A8 */

@@ -171,7 +171,7 @@ class OracleSystem:
         return p
 
     def lsqr(self, b, itnlim, atol=0.0, btol=0.0, conlim=0.0, force_itnlim=False,
-             want_hist=False, want_se=False) -> LsqrResult:
+             want_hist=False, want_se=False, damp=0.0) -> LsqrResult:
         """min ||A x - b||.  If preconditioned, iterates on A.diag(p), returns x = p (.) z."""
         b = np.ascontiguousarray(b, dtype=np.float64)
         assert b.shape == (self.m_total,)
@@ -180,12 +180,14 @@ class OracleSystem:
         hist = np.zeros((int(itnlim), 7)) if want_hist else None
         var = np.zeros(self.n) if want_se else None
         self._con()
+        lib().orc_set_damp(C.c_double(damp))
         rc = lib().orc_lsqr_var(*self._idx(), _p(self.values, C.c_double), _p(b, C.c_double),
                                 _p(x, C.c_double), C.c_int64(itnlim), C.c_double(atol),
                                 C.c_double(btol), C.c_double(conlim),
                                 C.c_int(1 if force_itnlim else 0), C.byref(res),
                                 _p(hist, C.c_double), _p(var, C.c_double))
         self._con(False)
+        lib().orc_set_damp(C.c_double(0.0))
         assert rc == 0
         se = None
         if want_se:

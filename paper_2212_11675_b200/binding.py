@@ -20,7 +20,7 @@ EXPORTS = [
     "gsr_matrix_create", "gsr_matrix_begin", "gsr_matrix_append_rows", "gsr_matrix_finalize",
     "gsr_matrix_destroy", "gsr_matrix_dims", "gsr_matrix_device_bytes", "gsr_aprod1",
     "gsr_aprod2", "gsr_precondition", "gsr_lsqr_solve", "gsr_set_option", "gsr_strerror",
-    "gsr_debug_expand_rows", "gsr_time_product", "gsr_launch_count", "gsr_lsqr_standard_errors", "gsr_lsqr_last_loop_ms",
+    "gsr_debug_expand_rows", "gsr_time_product", "gsr_launch_count", "gsr_lsqr_standard_errors", "gsr_lsqr_last_loop_ms", "gsr_lsqr_set_damp",
     "gsr_matrix_set_constraints", "gsr_comm_unique_id", "gsr_comm_create", "gsr_comm_destroy", "gsr_matrix_set_comm",
 ]
 
@@ -83,6 +83,7 @@ def lib():
         L.gsr_precondition.argtypes = [vp, vp, vp]
         L.gsr_lsqr_solve.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl, C.POINTER(gsr_lsqr_result), vp]
         L.gsr_lsqr_standard_errors.argtypes = [vp, vp, vp]
+        L.gsr_lsqr_set_damp.argtypes = [vp, dbl]
         L.gsr_lsqr_last_loop_ms.argtypes = [vp]
         L.gsr_lsqr_last_loop_ms.restype = dbl
         L.gsr_matrix_set_constraints.argtypes = [vp, i64, vp, vp, vp]
@@ -196,6 +197,10 @@ def gsr_lsqr_solve(h, b, x, itnlim, atol=0.0, btol=0.0, conlim=0.0, stream=None)
                                 float(conlim), C.byref(r), _stream(stream)), "gsr_lsqr_solve")
     return LsqrResult(r.istop, r.itn, r.istop_natural, r.itn_natural, r.rnorm, r.arnorm, r.anorm,
                       r.acond, r.xnorm, r.bnorm)
+
+
+def gsr_lsqr_set_damp(h, damp: float):
+    _check(lib().gsr_lsqr_set_damp(h, float(damp)), "gsr_lsqr_set_damp")
 
 
 def gsr_lsqr_last_loop_ms(h) -> float:

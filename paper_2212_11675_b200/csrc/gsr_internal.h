@@ -82,6 +82,7 @@ struct LsqrState {
     // recurrences (C3)
     double alpha, beta, rhobar, phibar, anorm, ddnorm, xxnorm, z, cs2, sn2;
     double bnorm, rnorm, arnorm, acond, xnorm;
+    double damp, res2;  // damping parameter (0: none) and the residual part held by its rows
     // coefficients consumed by the vector kernels
     double ca;         // aprod1: u_hat <- A v + ca * u_hat      (ca = -alpha/beta)
     double inv_beta;   // aprod2 input scale: v += A^T (u_hat * inv_beta)
@@ -163,6 +164,7 @@ struct gsr_matrix {
     int opt_force_itnlim;
     int opt_two_pass;               // 1: aprod1 + aprod2 per iteration instead of the fused pass
     int opt_no_fixed;               // 1: fp64 atomics in the instrumental pass even when scaled
+    double damp;                    // gsr_lsqr_set_damp (row f4); 0 = the paper's undamped LSQR
     int64_t n_con, con_nnz;         // row f3: constraint rows (CSR) appended below the observations
     int64_t* con_ptr;
     int32_t* con_col;

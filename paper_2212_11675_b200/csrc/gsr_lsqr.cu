@@ -244,6 +244,7 @@ __global__ void __launch_bounds__(1024) k_scalar_beta(LsqrState* __restrict__ st
     if (beta > 0.0) {
         st->beta_pos = 1;
         st->anorm = hyp(hyp(st->anorm, st->alpha), beta);   // uses the OLD alpha
+        if (st->damp > 0.0) st->anorm = hyp(st->anorm, st->damp);
         st->inv_beta = 1.0 / beta;
         st->vscale = -beta;
     } else {
@@ -276,9 +277,17 @@ __global__ void __launch_bounds__(1024) k_scalar_main(LsqrState* __restrict__ st
         st->inv_alpha = 1.0;
     }
     st->alpha = alpha;
+    // plane rotation eliminating the damping parameter (row f4; only when damp > 0)
+    double rhobar1 = st->rhobar, psi = 0.0;
+    if (st->damp > 0.0) {
+        rhobar1 = hyp(st->rhobar, st->damp);
+        const double cs1 = st->rhobar / rhobar1, sn1 = st->damp / rhobar1;
+        psi = sn1 * st->phibar;
+        st->phibar = cs1 * st->phibar;
+    }
     // plane rotation eliminating beta
-    const double rho = hyp(st->rhobar, beta);
-    const double cs = st->rhobar / rho, sn = beta / rho;
+    const double rho = hyp(rhobar1, beta);
+    const double cs = rhobar1 / rho, sn = beta / rho;
     const double theta = sn * alpha;
     st->rhobar = -cs * alpha;
     const double phi = cs * st->phibar;
@@ -302,7 +311,8 @@ __global__ void __launch_bounds__(1024) k_scalar_main(LsqrState* __restrict__ st
     // norms and stopping tests
     const double anorm = st->anorm, bnorm = st->bnorm;
     const double acond = anorm * sqrt(st->ddnorm);
-    const double rnorm = st->phibar;
+    st->res2 = st->res2 + psi * psi;
+    const double rnorm = st->damp > 0.0 ? sqrt(st->phibar * st->phibar + st->res2) : st->phibar;
     const double arnorm = alpha * fabs(tau);
     st->acond = acond;
     st->rnorm = rnorm;
@@ -512,6 +522,7 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     h.ctol = conlim > 0.0 ? 1.0 / conlim : 0.0;
     h.itnlim = itnlim;
     h.force = A->opt_force_itnlim;
+    h.damp = A->damp;
     h.inv_alpha = 1.0;
     GSR_CUDA_TRY(cudaMemcpyAsync(W.st, &h, sizeof(h), cudaMemcpyHostToDevice, s));
     GSR_CUDA_TRY(cudaMemsetAsync(W.v, 0, (size_t)n * 8, s));
@@ -601,6 +612,12 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     float loop_ms = 0.f;
     if (cudaEventElapsedTime(&loop_ms, W.ev0, W.ev1) != cudaSuccess) cudaGetLastError();
     W.last_loop_ms = loop_ms;
+    return GSR_OK;
+}
+
+int gsr_lsqr_set_damp(gsr_matrix* A, double damp) {
+    if (!A || !(damp >= 0.0)) return GSR_EINVAL;
+    A->damp = damp;
     return GSR_OK;
 }
 

@@ -354,3 +354,40 @@ def test_fixed_point_instrumental_pass_matches_fp64_atomics(name):
         assert np.linalg.norm(xs[0] - xs[1]) <= 1e-12 * np.linalg.norm(ro.x)
     finally:
         s.A.close()
+
+
+@pytest.mark.parametrize("fused", [1, 0])
+def test_damped_lsqr_parity(fused):
+    """Row f4: gsr_lsqr_set_damp against the oracle's damped LSQR, fixed count and standard mode."""
+    b = _binding()
+    s = Sys(CASES["cfg1"])
+    try:
+        rhs = _rhs(s)
+        s.o.precondition()
+        b.gsr_precondition(s.A.h)
+        b.gsr_set_option(s.A.h, b.GSR_OPT_FUSED, fused)
+        with pytest.raises(b.GsrError):
+            b.gsr_lsqr_set_damp(s.A.h, -1.0)
+        damp = 0.4
+        b.gsr_lsqr_set_damp(s.A.h, damp)
+        bd = torch.from_numpy(rhs).cuda()
+        x = torch.empty(s.n, dtype=torch.float64, device="cuda")
+        b.gsr_set_option(s.A.h, b.GSR_OPT_FORCE_ITNLIM, 1)
+        for k in (1, 6):
+            r = b.gsr_lsqr_solve(s.A.h, bd, x, k)
+            ro = s.o.lsqr(rhs, k, force_itnlim=True, damp=damp)
+            assert (r.istop, r.itn) == (ro.istop, ro.itn) == (7, k)
+            assert np.linalg.norm(x.cpu().numpy() - ro.x) <= X_TOL * np.linalg.norm(ro.x)
+            for f in ("rnorm", "anorm", "xnorm", "acond"):
+                assert abs(getattr(r, f) - getattr(ro, f)) <= X_TOL * getattr(ro, f), f
+        b.gsr_set_option(s.A.h, b.GSR_OPT_FORCE_ITNLIM, 0)
+        r = b.gsr_lsqr_solve(s.A.h, bd, x, 500, 1e-10, 1e-10, 1e8)
+        ro = s.o.lsqr(rhs, 500, 1e-10, 1e-10, 1e8, damp=damp)
+        assert r.istop == ro.istop and abs(r.itn - ro.itn) <= 1
+        assert np.linalg.norm(x.cpu().numpy() - ro.x) <= X_TOL * np.linalg.norm(ro.x)
+        b.gsr_lsqr_set_damp(s.A.h, 0.0)                       # back to the paper's undamped LSQR
+        r = b.gsr_lsqr_solve(s.A.h, bd, x, 500, 1e-10, 1e-10, 1e8)
+        ro = s.o.lsqr(rhs, 500, 1e-10, 1e-10, 1e8)
+        assert r.istop == ro.istop and np.linalg.norm(x.cpu().numpy() - ro.x) <= X_TOL * np.linalg.norm(ro.x)
+    finally:
+        s.A.close()

@@ -256,3 +256,23 @@ def test_variance_monotone_and_scaled_by_p():
     Q = _krylov_basis(A, b, 6)
     var_ref = np.einsum("ij,jk,ik->i", Q, np.linalg.inv(Q.T @ (A.T @ (A @ Q))), Q)
     assert np.max(np.abs(r.var - var_ref)) <= 1e-11 * np.max(var_ref)
+
+
+# ---- row f4: damping (Paige & Saunders' damp; the paper's solver is undamped)
+
+@pytest.mark.parametrize("damp", [0.3, 2.5])
+def test_damped_lsqr_solves_the_augmented_problem(damp):
+    """min ||[A; damp I] x - [b; 0]||: dense lstsq on the augmented matrix; rnorm is the norm of
+    the augmented residual, computed directly."""
+    cfg, star, att, instr, vals = small_system()
+    o = make_oracle(cfg, star, att, instr, vals)
+    A = csr_from_raw(cfg, star, att, instr, vals)[0].toarray()
+    b = np.random.default_rng(8).standard_normal(o.m)
+    r = o.lsqr(b, 2000, 1e-15, 1e-15, 1e12, damp=damp)
+    aug = np.vstack([A, damp * np.eye(o.n)])
+    xl = np.linalg.lstsq(aug, np.concatenate([b, np.zeros(o.n)]), rcond=None)[0]
+    assert np.linalg.norm(r.x - xl) <= 1e-11 * np.linalg.norm(xl)
+    direct = np.sqrt(np.linalg.norm(b - A @ r.x) ** 2 + damp ** 2 * np.linalg.norm(r.x) ** 2)
+    assert abs(r.rnorm - direct) <= 1e-11 * direct
+    r0 = o.lsqr(b, 2000, 1e-15, 1e-15, 1e12)
+    assert np.linalg.norm(r.x) < np.linalg.norm(r0.x)          # damping shrinks the solution
