@@ -4,8 +4,8 @@
 // the CPU because it is 100-1000x cheaper than the products.  The paper does not
 // give their structure, so they are n_con extra rows in general CSR form appended below the m
 // observation rows; m-sized vectors then carry n_con more entries at the end.
-// One CTA, one warp per constraint row: the work is tiny next to the products, and a single CTA
-// gives a fixed summation order for the row sums and for sum y^2.
+// One CTA per constraint row (at most CON_GRID_MAX CTAs, grid-stride over the rows), block
+// reductions in a fixed order, one partial sum of y^2 per CTA: deterministic for a given system.
 #include <vector>
 
 #include "gsr_internal.h"
@@ -18,52 +18,60 @@ __device__ __forceinline__ double wsum(double v) {
     return v;
 }
 
-// y[r] = ca*y[r] + sum_e val[e] x[col[e]]; partial[0] = sum_r y_new[r]^2 (if partial != nullptr)
-__global__ void __launch_bounds__(1024) k_con_aprod1(int64_t n_con, const int64_t* __restrict__ ptr,
-                                                     const int32_t* __restrict__ col,
-                                                     const double* __restrict__ val,
-                                                     const double* __restrict__ x, double* __restrict__ y,
-                                                     const double* __restrict__ ca_p,
-                                                     double* __restrict__ partial,
-                                                     const int* __restrict__ stop) {
+constexpr int CON_TPB = 256;
+
+// deterministic block sum (fixed order): valid in thread 0
+__device__ __forceinline__ double con_block_sum(double v, double* red) {
+    v = wsum(v);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (threadIdx.x == 0)
+        for (int w = 0; w < CON_TPB / 32; ++w) t += red[w];
+    __syncthreads();
+    return t;
+}
+
+// One CTA per constraint row (grid-stride over the rows), the row's entries strided over the
+// threads: y[r] = ca*y[r] + sum_e val[e] x[col[e]]; partial[blockIdx.x] = sum over the CTA's
+// rows of y_new[r]^2 (if partial != nullptr).  Fixed summation order for a fixed grid.
+__global__ void __launch_bounds__(CON_TPB) k_con_aprod1(int64_t n_con, const int64_t* __restrict__ ptr,
+                                                        const int32_t* __restrict__ col,
+                                                        const double* __restrict__ val,
+                                                        const double* __restrict__ x, double* __restrict__ y,
+                                                        const double* __restrict__ ca_p,
+                                                        double* __restrict__ partial,
+                                                        const int* __restrict__ stop) {
     if (stop && *stop) return;
-    __shared__ double red[32];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    __shared__ double red[CON_TPB / 32];
     const double ca = *ca_p;
-    double q = 0.0;
-    for (int64_t r = warp; r < n_con; r += 32) {
+    double q = 0.0;   // meaningful in thread 0
+    for (int64_t r = blockIdx.x; r < n_con; r += gridDim.x) {
         double sum = 0.0;
-        for (int64_t e = ptr[r] + lane; e < ptr[r + 1]; e += 32) sum = fma(val[e], x[col[e]], sum);
-        sum = wsum(sum);
-        const double ynew = fma(ca, y[r], sum);
-        if (lane == 0) y[r] = ynew;
-        q = fma(ynew, ynew, q);   // identical in every lane
-    }
-    if (partial) {
-        if (lane == 0) red[warp] = q;
-        __syncthreads();
+        for (int64_t e = ptr[r] + threadIdx.x; e < ptr[r + 1]; e += CON_TPB) sum = fma(val[e], x[col[e]], sum);
+        sum = con_block_sum(sum, red);
         if (threadIdx.x == 0) {
-            double t = 0.0;
-            for (int w = 0; w < 32; ++w) t += red[w];
-            partial[0] = t;
+            const double ynew = fma(ca, y[r], sum);
+            y[r] = ynew;
+            q = fma(ynew, ynew, q);
         }
     }
+    if (partial && threadIdx.x == 0) partial[blockIdx.x] = q;
 }
 
 // x[col[e]] += val[e] * (y[r] * sy)   (SQUARE: x[col[e]] += val[e]^2)
 template <bool SQUARE>
-__global__ void __launch_bounds__(1024) k_con_aprod2(int64_t n_con, const int64_t* __restrict__ ptr,
-                                                     const int32_t* __restrict__ col,
-                                                     const double* __restrict__ val,
-                                                     const double* __restrict__ y, double* __restrict__ x,
-                                                     const double* __restrict__ sy_p,
-                                                     const int* __restrict__ stop) {
+__global__ void __launch_bounds__(CON_TPB) k_con_aprod2(int64_t n_con, const int64_t* __restrict__ ptr,
+                                                        const int32_t* __restrict__ col,
+                                                        const double* __restrict__ val,
+                                                        const double* __restrict__ y, double* __restrict__ x,
+                                                        const double* __restrict__ sy_p,
+                                                        const int* __restrict__ stop) {
     if (stop && *stop) return;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const double sy = SQUARE ? 1.0 : *sy_p;
-    for (int64_t r = warp; r < n_con; r += 32) {
+    for (int64_t r = blockIdx.x; r < n_con; r += gridDim.x) {
         const double yr = SQUARE ? 1.0 : y[r] * sy;
-        for (int64_t e = ptr[r] + lane; e < ptr[r + 1]; e += 32) {
+        for (int64_t e = ptr[r] + threadIdx.x; e < ptr[r + 1]; e += CON_TPB) {
             const double a = val[e];
             const double t = SQUARE ? a * a : a * yr;
             if (t != 0.0) atomicAdd(x + col[e], t);
@@ -97,10 +105,15 @@ __global__ void __launch_bounds__(1024) k_con_copy_sumsq(const double* __restric
     }
 }
 
+// CTAs of the constraint kernels = partial sums of y^2 they write (CON_GRID_MAX at most)
+int con_grid(const gsr_matrix* A) {
+    return (int)(A->n_con < CON_GRID_MAX ? A->n_con : CON_GRID_MAX);
+}
+
 int launch_con_aprod1(const gsr_matrix* A, const double* x, double* ycon, const double* ca,
                       double* partial, const int* stop, cudaStream_t s) {
     if (A->n_con == 0) return GSR_OK;
-    k_con_aprod1<<<1, 1024, 0, s>>>(A->n_con, A->con_ptr, A->con_col, A->con_val, x, ycon, ca, partial, stop);
+    k_con_aprod1<<<con_grid(A), CON_TPB, 0, s>>>(A->n_con, A->con_ptr, A->con_col, A->con_val, x, ycon, ca, partial, stop);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;
@@ -109,7 +122,7 @@ int launch_con_aprod1(const gsr_matrix* A, const double* x, double* ycon, const 
 int launch_con_aprod2(const gsr_matrix* A, const double* ycon, double* x, const double* sy,
                       const int* stop, cudaStream_t s) {
     if (A->n_con == 0) return GSR_OK;
-    k_con_aprod2<false><<<1, 1024, 0, s>>>(A->n_con, A->con_ptr, A->con_col, A->con_val, ycon, x, sy, stop);
+    k_con_aprod2<false><<<con_grid(A), CON_TPB, 0, s>>>(A->n_con, A->con_ptr, A->con_col, A->con_val, ycon, x, sy, stop);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;
@@ -117,7 +130,7 @@ int launch_con_aprod2(const gsr_matrix* A, const double* ycon, double* x, const 
 
 int launch_con_colsumsq(const gsr_matrix* A, double* q, cudaStream_t s) {
     if (A->n_con == 0) return GSR_OK;
-    k_con_aprod2<true><<<1, 1024, 0, s>>>(A->n_con, A->con_ptr, A->con_col, A->con_val, nullptr, q, nullptr, nullptr);
+    k_con_aprod2<true><<<con_grid(A), CON_TPB, 0, s>>>(A->n_con, A->con_ptr, A->con_col, A->con_val, nullptr, q, nullptr, nullptr);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;

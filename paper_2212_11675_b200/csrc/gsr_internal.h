@@ -197,6 +197,8 @@ inline void count_launch(long long k = 1) { g_launches += k; }
 
 int comm_allreduce_sum(gsr_comm* c, double* buf, size_t count, cudaStream_t s);
 // constraint rows (gsr_constraints.cu); all are no-ops when the handle has none
+constexpr int CON_GRID_MAX = 592;
+int con_grid(const gsr_matrix* A);   // CTAs = partial sums of y^2 written by launch_con_aprod1
 int launch_con_aprod1(const gsr_matrix* A, const double* x, double* ycon, const double* ca,
                       double* partial, const int* stop, cudaStream_t s);
 int launch_con_aprod2(const gsr_matrix* A, const double* ycon, double* x, const double* sy,

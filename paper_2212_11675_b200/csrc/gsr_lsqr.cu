@@ -361,7 +361,7 @@ int ensure_workspace(gsr_matrix* A) {
     GSR_TRY(dev_alloc(A, (void**)&W.x, n8));
     GSR_TRY(dev_alloc(A, (void**)&W.t, n8 + 16));   // t[n]: local sum of u_hat^2 (sharded solve)
     GSR_TRY(dev_alloc(A, (void**)&W.var, n8));
-    GSR_TRY(dev_alloc(A, (void**)&W.part_u, (size_t)(npu + 1) * 8));   // + one slot for the constraint rows
+    GSR_TRY(dev_alloc(A, (void**)&W.part_u, (size_t)(npu + CON_GRID_MAX + 1) * 8));   // + slots of the constraint rows
     GSR_TRY(dev_alloc(A, (void**)&W.part_v, NB_N * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.part_w, NB_N * 8));
     GSR_TRY(dev_alloc(A, (void**)&W.part_va, NB_N * 8));
@@ -401,7 +401,7 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
     Workspace& W = A->ws;
     const int64_t n = A->n_cols;
     const int64_t split = A->comm ? A->off_att : 0;   // sharded: [0, split) distributed slice
-    const int ncp = A->n_con > 0 ? 1 : 0;             // one more partial of u_hat^2 (constraint rows)
+    const int ncp = con_grid(A);                      // more partials of u_hat^2 (constraint rows)
     if (A->opt_two_pass) {
         // bidiagonalisation, first half: u_hat <- A v - (alpha/beta) u_hat ; partials of u_hat^2
         GSR_TRY(launch_aprod1(A, W.v, W.u, &W.st->ca, W.part_u, &W.st->stop, nullptr, s));

@@ -68,19 +68,19 @@ def test_constraints_make_a_rank_deficient_system_unique():
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("fused", [1, 0])
-def test_gpu_constraints_parity(fused):
+@pytest.mark.parametrize("fused,n_con,nnz_row", [(1, 7, 200), (0, 7, 200), (1, 700, 30), (0, 3, 100000)])
+def test_gpu_constraints_parity(fused, n_con, nnz_row):
     import torch
     from paper_2212_11675_b200 import binding as g
     cfg = inputs.scaled(inputs.named_config("cfg1"), 10, "cfg1/10")
     star, att, instr, vals = inputs.gen_all(cfg)
     from oracle import gsr_oracle
     o = gsr_oracle.from_torch(cfg, star, att, instr, vals)
-    C, ptr, col, val = _constraints(o.n, 7, 200, 9)
+    C, ptr, col, val = _constraints(o.n, n_con, nnz_row, 9)     # few / many (> grid) / dense rows
     o.set_constraints(ptr, col, val)
     A = g.GsrMatrix.create(cfg, star.cuda(), att.cuda(), instr.cuda(), vals.cuda())
     try:
-        g.gsr_matrix_set_constraints(A.h, 7, ptr, torch.from_numpy(col).cuda(), val)    # host and device arrays
+        g.gsr_matrix_set_constraints(A.h, n_con, ptr, torch.from_numpy(col).cuda(), val)    # host and device arrays
         rng = np.random.default_rng(2)
         x, y = rng.standard_normal(o.n), rng.standard_normal(o.m_total)
         y0, x0 = rng.standard_normal(o.m_total), rng.standard_normal(o.n)
