@@ -10,16 +10,25 @@
 //     xw[warp][0 .. 3*win)            the unit's attitude window, PRIVATE to the warp
 // so the 18 irregular column accesses of a row never leave the SM; only the
 // astrometric columns (5 per star, rows star-sorted inside a unit) and the global column go
-// to L1/L2.  The matrix is streamed exactly once, every request coalesced.
+// to L1/L2.  The matrix is streamed exactly once, every request covers whole 128-byte lines.
 //
-// Attitude block.  Lane j < 12 of each half-warp owns COEFFICIENT j of 16 rows (the tile stores
-// the 32x12 attitude block row-major, see gsr_internal.h), so for one row the 12 lanes touch
-// 12 distinct, conflict-free window addresses:
-//   aprod2: plain shared-memory read-modify-write, row after row, no atomics (the window is
-//           private to the warp, and rows of the same warp are serialised);
-//   aprod1: 12 products per row, transposed back to "lane r owns row r" by a 15-shuffle
-//           butterfly inside each half-warp.
+// Attitude block.  Lane (h, j), j < 12, of each half-warp owns COEFFICIENT j of the 16 attitude
+// slots of its half (gsr_internal.h), so for one slot the 12 lanes touch 12 distinct,
+// conflict-free window addresses:
+//   aprod2: plain shared-memory read-modify-write, slot after slot, no atomics (the window is
+//           private to the warp, and slots of the same warp are serialised);
+//   aprod1: 12 products per slot, summed over the 12 lanes by fp64 tensor-core MMAs with
+//           constant 0/1 operands (reduce_slots) -- no shuffles, nothing on the LSU pipe.
 #include "gsr_internal.h"
+
+// compute-sanitizer is closed on the GPU pool this was developed on: -DGSR_BOUNDS_CHECK turns the
+// index computations of the product kernels into device asserts instead.
+#ifdef GSR_BOUNDS_CHECK
+#include <assert.h>
+#define GSR_ASSERT(c) assert(c)
+#else
+#define GSR_ASSERT(c) ((void)0)
+#endif
 
 namespace gsr {
 
@@ -29,19 +38,60 @@ __device__ __forceinline__ double warp_sum(double v) {
     return v;
 }
 
+// D(8x8) += A(8x4) B(4x8), fp64 (DMMA).  Fragments: lane l holds A[l>>2][l&3], B[l&3][l>>2] and
+// D[l>>2][2(l&3) + {0,1}].
+__device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+// Lane (h, j) = 16h + j holds p[q], its term of attitude slot (h, q), q < 16 (lanes j >= 12
+// hold zeros).  Returns, in lane l, the sum over the 12 lanes of the slot att_slot(l).
+//   stage 1, one MMA per q:  D1_b[q&7][n] += sum_k [p of lane 4n+k][q]   (A = row selector,
+//            B = the terms; n = lane group = (h, axis), k = knot: the sum over the 4 knots)
+//   stage 2, four MMAs:      S[i][q'] = sum over the 4 lane groups of half (i&1) of D1_b[q'][.]
+//            with b = (i>>1)&1; rows i and i+4 are duplicates, so that every lane finds one slot
+//            sum in its own D fragment: lanes 0-15 take column 2(l&3), lanes 16-31 the next.
+// The MMAs run on the fp64 tensor pipe (4 cycles each per SM, measured), which is otherwise idle;
+// the 15-shuffle butterfly this replaces cost 30 LSU wavefronts per tile.
+__device__ __forceinline__ double reduce_slots(const double (&p)[16], int lane) {
+    const int grp = lane >> 2;
+    double d1[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        const double sel = __hiloint2double(grp == (q & 7) ? 0x3FF00000 : 0, 0);
+        dmma(d1[q >> 3][0], d1[q >> 3][1], sel, p[q]);
+    }
+    double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {
+        const double a2 = __hiloint2double((grp & 3) == 2 * b + ((lane & 3) >> 1) ? 0x3FF00000 : 0, 0);
+        dmma(s0, s1, a2, d1[b][0]);
+        dmma(s0, s1, a2, d1[b][1]);
+    }
+    return (lane >> 4) ? s1 : s0;
+}
+
 // A tile is consumed in two phases so that the loads of one phase are in flight while the
 // other phase computes (software pipeline, no extra registers):
 //   phase A: the attitude block (16 coefficients per lane) + window offsets
 //   phase B: astrometric, instrumental and global coefficients + star and column indices
 struct RegsA {
-    double at[16];             // lane (h, j): attitude coefficient min(j, 11) of rows 16h .. 16h+15
-    uint32_t aoff;             // lane r: att_start - a0 of row r
+    double at[16];             // lane (h, j): attitude coefficient j of slots (h, 0 .. 15); j >= 12: 0
+    uint32_t aw[4];            // the 16 window offsets (u8) of the slots of half h
+    uint32_t cmask;            // bit q: slots (0, q) and (1, q) overlap
 };
 struct RegsB {
-    double as[5], in[6], gl;   // lane r: coefficients of row r
+    double as[5], in[6], gl;   // home lane l: coefficients of row l
     int32_t s;
-    uint32_t c[6];
+    uint32_t cw[3];            // instrumental columns, two per word
 };
+__device__ __forceinline__ uint32_t aoff_of(const uint32_t (&aw)[4], int q) {
+    return (aw[q >> 2] >> (8 * (q & 3))) & 0xffu;
+}
+__device__ __forceinline__ uint32_t icol_of(const uint32_t (&cw)[3], int j) {
+    return (j & 1) ? cw[j >> 1] >> 16 : cw[j >> 1] & 0xffffu;
+}
 
 // Streaming loads, all of a phase issued back to back (volatile asm keeps them together and
 // ahead of their first use).
@@ -55,31 +105,36 @@ __device__ __forceinline__ int32_t ld_stream_s32(const void* p) {
     asm volatile("ld.global.cs.s32 %0, [%1];" : "=r"(v) : "l"(p));
     return v;
 }
-__device__ __forceinline__ uint32_t ld_stream_u16(const void* p) {
-    uint16_t v;
-    asm volatile("ld.global.cs.u16 %0, [%1];" : "=h"(v) : "l"(p));
+__device__ __forceinline__ uint32_t ld_stream_u32(const void* p) {
+    uint32_t v;
+    asm volatile("ld.global.cs.u32 %0, [%1];" : "=r"(v) : "l"(p));
     return v;
 }
+// two attitude coefficients (slots 2i, 2i+1); lanes j >= 12 keep their zeros
+__device__ __forceinline__ void ld_att_pair(const void* p, int active, double& a, double& b) {
+    asm volatile("{\n\t.reg .pred pa;\n\tsetp.ne.s32 pa, %2, 0;\n\t"
+                 "@pa ld.global.cs.v2.f64 {%0, %1}, [%3];\n\t}"
+                 : "+d"(a), "+d"(b) : "r"(active), "l"(p));
+}
+__device__ __forceinline__ void ld_aoff(const unsigned char* T, int h, uint32_t (&aw)[4]) {
+    asm volatile("ld.global.cs.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(aw[0]), "=r"(aw[1]), "=r"(aw[2]), "=r"(aw[3]) : "l"(T + OFF_AOFF + h * 16));
+}
 __device__ __forceinline__ void load_A(const unsigned char* __restrict__ T, int lane, RegsA& r) {
-    r.aoff = ld_stream_u16(T + OFF_AOFF + lane * 2);
-    const int h = lane >> 4, jj = min(lane & 15, 11);
+    const int h = lane >> 4, jj = min(lane & 15, 11), act = (lane & 15) < 12;
+    ld_aoff(T, h, r.aw);
+    r.cmask = ld_stream_u32(T + OFF_CMASK);
 #pragma unroll
-    for (int q = 0; q < 16; ++q) r.at[q] = ld_stream_f64(T + OFF_ATTV + ((q * 2 + h) * 12 + jj) * 8);
+    for (int i = 0; i < 8; ++i)
+        ld_att_pair(T + OFF_ATTV + ((i * 2 + h) * 12 + jj) * 16, act, r.at[2 * i], r.at[2 * i + 1]);
 }
-__device__ __forceinline__ void load_B(const unsigned char* __restrict__ T, int lane, RegsB& r) {
-    r.s = ld_stream_s32(T + OFF_STAR + lane * 4);
+__device__ __forceinline__ void zero_A(RegsA& r) {
 #pragma unroll
-    for (int j = 0; j < 6; ++j) r.c[j] = ld_stream_u16(T + OFF_ICOL + (j * R + lane) * 2);
-#pragma unroll
-    for (int k = 0; k < 5; ++k) r.as[k] = ld_stream_f64(T + OFF_ASTRO + (k * R + lane) * 8);
-#pragma unroll
-    for (int j = 0; j < 6; ++j) r.in[j] = ld_stream_f64(T + OFF_INSTRV + (j * R + lane) * 8);
-    r.gl = ld_stream_f64(T + OFF_GLOBV + lane * 8);
+    for (int q = 0; q < 16; ++q) r.at[q] = 0.0;
 }
-
 __device__ __forceinline__ void load_B_instr(const unsigned char* __restrict__ T, int lane, RegsB& r) {
 #pragma unroll
-    for (int j = 0; j < 6; ++j) r.c[j] = ld_stream_u16(T + OFF_ICOL + (j * R + lane) * 2);
+    for (int j = 0; j < 3; ++j) r.cw[j] = ld_stream_u32(T + OFF_ICOL + (j * R + lane) * 4);
 #pragma unroll
     for (int j = 0; j < 6; ++j) r.in[j] = ld_stream_f64(T + OFF_INSTRV + (j * R + lane) * 8);
 }
@@ -89,11 +144,98 @@ __device__ __forceinline__ void load_B_rest(const unsigned char* __restrict__ T,
     for (int k = 0; k < 5; ++k) r.as[k] = ld_stream_f64(T + OFF_ASTRO + (k * R + lane) * 8);
     r.gl = ld_stream_f64(T + OFF_GLOBV + lane * 8);
 }
+__device__ __forceinline__ void load_B(const unsigned char* __restrict__ T, int lane, RegsB& r) {
+    load_B_rest(T, lane, r);
+    load_B_instr(T, lane, r);
+}
+
+// fp64 add to shared memory.  sm_100a has no native fp64 (or 64-bit add) shared atomic; the
+// builtin atomicAdd(double*) is expanded by ptxas into an LDS + ATOMS.CAST.SPIN loop AFTER its
+// convergence analysis, and with this file's kernels it came out without the reconvergence
+// barrier around the loop (lanes that lost a round were still spinning when the rest of the
+// warp went on to the segmented-scan shuffles).  An explicit compare-and-swap loop keeps the
+// divergence visible to the compiler.
+__device__ __forceinline__ void smem_add_f64(double* addr, double v) {
+    unsigned long long* a = (unsigned long long*)addr;
+    unsigned long long old = *a, assumed;
+    do {
+        assumed = old;
+        old = atomicCAS(a, assumed, (unsigned long long)__double_as_longlong(v + __longlong_as_double((long long)assumed)));
+    } while (assumed != old);
+}
 
 __device__ __forceinline__ int fetch_unit(int* counter, int lane) {
     int u = 0;
     if (lane == 0) u = atomicAdd(counter, 1);
     return __shfl_sync(0xffffffffu, u, 0);
+}
+
+// attitude part of aprod1 for one tile: lane l returns the attitude sum of its own row
+__device__ __forceinline__ double att_mode1(const RegsA& ra, const double* xw, int axo, int lane) {
+    double p[16];
+#pragma unroll
+    for (int q = 0; q < 16; ++q) p[q] = ra.at[q] * xw[aoff_of(ra.aw, q) + axo];
+    return reduce_slots(p, lane);
+}
+
+// attitude part of aprod2 for one slot pair: slot (0, q) through lanes 0-11,
+// slot (1, q) through lanes 16-27, one slot per half and step; the two slots of a step go in
+// one instruction unless their windows overlap (cmask; then one after the other).
+// SQUARE: add the squared coefficients instead.
+template <bool SQUARE>
+__device__ __forceinline__ void att_mode2_step(const RegsA& ra, int q, double yy, double* tw, int axo,
+                                               bool lo12, bool hi12, int ws_dbg) {
+    double* pa = tw + aoff_of(ra.aw, q) + axo;
+    GSR_ASSERT((int)aoff_of(ra.aw, q) + 3 < ws_dbg);
+    const double c = ra.at[q];
+    if ((ra.cmask >> q) & 1u) {
+        if (lo12) *pa = SQUARE ? fma(c, c, *pa) : fma(c, yy, *pa);
+        __syncwarp();
+        if (hi12) *pa = SQUARE ? fma(c, c, *pa) : fma(c, yy, *pa);
+    } else {
+        if (lo12 || hi12) *pa = SQUARE ? fma(c, c, *pa) : fma(c, yy, *pa);
+    }
+    __syncwarp();
+}
+
+// astrometric part of aprod2 for one tile: segmented reduction over the
+// star-sorted home lanes, one global atomic per (tile, star, coefficient).  vs[k] = A[l,k]*y[l].
+__device__ __forceinline__ void astro_mode2(double (&vs)[5], int32_t s, int lane, double* __restrict__ x,
+                                            int64_t S) {
+    GSR_ASSERT(s >= 0 && s < S);
+    const int32_t s_up = __shfl_up_sync(0xffffffffu, s, 1);
+    const bool head = lane == 0 || s_up != s;
+    const unsigned heads = __ballot_sync(0xffffffffu, head);
+    if (heads == 1u) {   // the whole warp lies inside one star
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            const double tsum = warp_sum(vs[k]);
+            if (lane == 0 && tsum != 0.0) atomicAdd(x + 5 * (int64_t)s + k, tsum);
+        }
+    } else {
+        // segmented inclusive scan; the last lane of each segment holds its sum.  A step of
+        // distance o is needed only if some run is longer than o rows, i.e. if there are o
+        // consecutive non-head lanes (shuffles cost LSU data-pipe wavefronts).
+        const unsigned below = heads & ((2u << lane) - 1u);        // heads at or below me
+        const int seg_start = 31 - __clz(below);
+        const bool tail = lane == 31 || ((heads >> (lane + 1)) & 1u);
+        const unsigned n1 = ~heads, n2 = n1 & (n1 >> 1), n4 = n2 & (n2 >> 2),
+                       n8 = n4 & (n4 >> 4), n16 = n8 & (n8 >> 8);
+        const unsigned need = 1u | (n2 ? 2u : 0u) | (n4 ? 4u : 0u) | (n8 ? 8u : 0u) | (n16 ? 16u : 0u);
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            if (need & o) {
+#pragma unroll
+                for (int k = 0; k < 5; ++k) {
+                    const double up = __shfl_up_sync(0xffffffffu, vs[k], o);
+                    if (lane - o >= seg_start) vs[k] += up;
+                }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 5; ++k)
+            if (tail && vs[k] != 0.0) atomicAdd(x + 5 * (int64_t)s + k, vs[k]);
+    }
 }
 
 // ---- aprod1: y[i] = ca*y[i] + sum_k A[i,k] x[col(i,k)]  (Algorithm 1) --------------------
@@ -119,9 +261,10 @@ __global__ void __launch_bounds__(TPB) k_aprod1(const unsigned char* __restrict_
     const double ca = *ca_p;
     __syncthreads();
 
-    const int h = lane >> 4, j = lane & 15, jj = min(j, 11);
+    const int jj = min(lane & 15, 11);
     const int axo = (jj >> 2) * ws + (jj & 3);   // my coefficient's column, relative to aoff
-    const bool att_lane = j < 12;
+    RegsA ra;
+    zero_A(ra);
     for (;;) {
         const int u = fetch_unit(counter, lane);
         if (u >= n_units) break;
@@ -135,7 +278,6 @@ __global__ void __launch_bounds__(TPB) k_aprod1(const unsigned char* __restrict_
         __syncwarp();
         double q = 0.0;
         const unsigned char* T = tiles + (int64_t)un.tile0 * TILE_BYTES;
-        RegsA ra;
         load_A(T, lane, ra);
         for (int t = 0; t < un.ntiles; ++t, T += TILE_BYTES) {
             RegsB r;
@@ -149,32 +291,15 @@ __global__ void __launch_bounds__(TPB) k_aprod1(const unsigned char* __restrict_
                 ry = pe;
             }
             const double yold = live ? __ldcs(y + ry) : 0.0;
-            // phase A -- attitude: 12 lanes per row, products transposed back by a butterfly
-            double p[16];
-#pragma unroll
-            for (int qq = 0; qq < 16; ++qq) {
-                const uint32_t a = __shfl_sync(0xffffffffu, ra.aoff, h * 16 + qq);
-                const double pv = ra.at[qq] * xw[a + axo];
-                p[qq] = att_lane ? pv : 0.0;
-            }
-#pragma unroll
-            for (int o = 8; o > 0; o >>= 1) {
-                const bool up = (j & o) != 0;
-#pragma unroll
-                for (int i = 0; i < o; ++i) {
-                    const double send = up ? p[i] : p[i + o];
-                    const double keep = up ? p[i + o] : p[i];
-                    p[i] = keep + __shfl_xor_sync(0xffffffffu, send, o);
-                }
-            }
-            double sum = p[0];   // lane (h, j) now holds the attitude part of row 16h + j
+            // phase A -- attitude
+            double sum = att_mode1(ra, xw, axo, lane);
             if (t + 1 < un.ntiles) load_A(T + TILE_BYTES, lane, ra);   // in flight during phase B
             // phase B
             const double* xa = x + 5 * (int64_t)r.s;
 #pragma unroll
             for (int k = 0; k < 5; ++k) sum = fma(r.as[k], __ldg(xa + k), sum);
 #pragma unroll
-            for (int k = 0; k < 6; ++k) sum = fma(r.in[k], xi[r.c[k]], sum);
+            for (int k = 0; k < 6; ++k) sum = fma(r.in[k], xi[icol_of(r.cw, k)], sum);
             sum = fma(r.gl, xg, sum);
             const double ynew = fma(ca, yold, sum);
             if (live) y[ry] = ynew;
@@ -208,9 +333,9 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double* xi = sm;
     double* xw = sm + ((I + 1) & ~1) + warp * 3 * ws;
-    double* ysm = sm + ((I + 1) & ~1) + NWARP * 3 * ws + warp * 32;   // y of the current tile: a
-                                                  // shared-memory broadcast costs the LSU pipe
-                                                  // less than two 32-bit shuffles per step
+    double* ysm = sm + ((I + 1) & ~1) + NWARP * 3 * ws + warp * 32;   // y of the current tile by
+                                                  // attitude slot: wide shared-memory broadcasts
+                                                  // cost the LSU pipe less than shuffles
     // small I: one private copy of the instrumental accumulator per warp (copies 1.. behind the
     // y tiles), so that only lanes of the same instruction contend for an address (config 4)
     const int ipad = (I + 1) & ~1;
@@ -221,11 +346,14 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
     const double sy = SQUARE ? 1.0 : *sy_p;
     __syncthreads();
 
-    const int h = lane >> 4, j = lane & 15, jj = min(j, 11);
+    const int h = lane >> 4, jj = min(lane & 15, 11);
     const int axo = (jj >> 2) * ws + (jj & 3);
     const bool lo12 = lane < 12, hi12 = lane >= 16 && lane < 28;
+    const int myslot = att_slot(lane);
     double* xatt = x + 5 * S;
     double g = 0.0;
+    RegsA ra;
+    zero_A(ra);
     for (;;) {
         const int u = fetch_unit(counter, lane);
         if (u >= n_units) break;
@@ -234,7 +362,6 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
         for (int i = lane; i < 3 * ws; i += 32) xw[i] = 0.0;
         __syncwarp();
         const unsigned char* T = tiles + (int64_t)un.tile0 * TILE_BYTES;
-        RegsA ra;
         load_A(T, lane, ra);
         for (int t = 0; t < un.ntiles; ++t, T += TILE_BYTES) {
             RegsB r;
@@ -248,30 +375,20 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
                 } else {
                     yv = __ldcs(y + ri) * sy;
                 }
-            }
-            // phase A -- attitude: rows 0-15 through lanes 0-11, rows 16-31
-            // through lanes 16-27, one row per half and step; the two rows of a step go in one
-            // instruction unless their windows overlap (then one after the other)
-            ysm[lane] = yv;
-            __syncwarp();
-            const uint32_t a_other = __shfl_xor_sync(0xffffffffu, ra.aoff, 16);
-            const int da = (int)ra.aoff - (int)a_other;
-            const unsigned cmask = __ballot_sync(0xffffffffu, da > -4 && da < 4);
-#pragma unroll
-            for (int qq = 0; qq < 16; ++qq) {
-                const int src = h * 16 + qq;
-                const uint32_t a = __shfl_sync(0xffffffffu, ra.aoff, src);
-                const double yy = ysm[src];
-                const double add = SQUARE ? ra.at[qq] * ra.at[qq] : ra.at[qq] * yy;
-                double* pa = xw + a + axo;
-                if ((cmask >> qq) & 1u) {
-                    if (lo12) *pa += add;
-                    __syncwarp();
-                    if (hi12) *pa += add;
-                } else {
-                    if (lo12 || hi12) *pa += add;
-                }
+                ysm[myslot] = yv;
                 __syncwarp();
+            }
+            // phase A -- attitude
+#pragma unroll
+            for (int g4 = 0; g4 < 4; ++g4) {
+                double yy4[4] = {0.0, 0.0, 0.0, 0.0};
+                if (!SQUARE) {
+                    const double2 y01 = *(const double2*)(ysm + h * 16 + 4 * g4);
+                    const double2 y23 = *(const double2*)(ysm + h * 16 + 4 * g4 + 2);
+                    yy4[0] = y01.x; yy4[1] = y01.y; yy4[2] = y23.x; yy4[3] = y23.y;
+                }
+#pragma unroll
+                for (int i = 0; i < 4; ++i) att_mode2_step<SQUARE>(ra, 4 * g4 + i, yy4[i], xw, axo, lo12, hi12, win);
             }
             if (t + 1 < un.ntiles) load_A(T + TILE_BYTES, lane, ra);   // in flight during phase B
             // phase B
@@ -281,55 +398,21 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
             for (int k = 0; k < 6; ++k) r.in[k] = SQUARE ? r.in[k] * r.in[k] : r.in[k] * yv;
             // instrumental
 #pragma unroll
-            for (int k = 0; k < 6; ++k) atomicAdd(xi + r.c[k], r.in[k]);
+            for (int k = 0; k < 6; ++k) {
+                GSR_ASSERT((int)icol_of(r.cw, k) < I);
+                smem_add_f64(xi + icol_of(r.cw, k), r.in[k]);
+            }
+            __syncwarp();
             // global
             g += SQUARE ? r.gl * r.gl : r.gl * yv;
-            // astrometric: segmented reduction, rows are star-sorted
-            const int32_t s_up = __shfl_up_sync(0xffffffffu, r.s, 1);
-            const bool head = lane == 0 || s_up != r.s;
-            const unsigned heads = __ballot_sync(0xffffffffu, head);
-            if (heads == 1u) {   // the whole warp lies inside one star
-#pragma unroll
-                for (int k = 0; k < 5; ++k) {
-                    const double tsum = warp_sum(r.as[k]);
-                    if (lane == 0 && tsum != 0.0) atomicAdd(x + 5 * (int64_t)r.s + k, tsum);
-                }
-            } else {
-                // segmented inclusive scan; the last lane of each segment holds its sum.  A step
-                // of distance o is needed only if some run is longer than o rows, i.e. if there
-                // are o consecutive non-head lanes (shuffles cost LSU data-pipe wavefronts).
-                const unsigned below = heads & ((2u << lane) - 1u);        // heads at or below me
-                const int seg_start = 31 - __clz(below);
-                const bool tail = lane == 31 || ((heads >> (lane + 1)) & 1u);
-                const unsigned n1 = ~heads, n2 = n1 & (n1 >> 1), n4 = n2 & (n2 >> 2),
-                               n8 = n4 & (n4 >> 4), n16 = n8 & (n8 >> 8);
-                const unsigned need = 1u | (n2 ? 2u : 0u) | (n4 ? 4u : 0u) | (n8 ? 8u : 0u) | (n16 ? 16u : 0u);
-                double vs[5];
-#pragma unroll
-                for (int k = 0; k < 5; ++k) vs[k] = r.as[k];
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    if (need & o) {
-#pragma unroll
-                        for (int k = 0; k < 5; ++k) {
-                            const double up = __shfl_up_sync(0xffffffffu, vs[k], o);
-                            if (lane - o >= seg_start) vs[k] += up;
-                        }
-                    }
-                }
-#pragma unroll
-                for (int k = 0; k < 5; ++k)
-                    if (tail && vs[k] != 0.0) atomicAdd(x + 5 * (int64_t)r.s + k, vs[k]);
-            }
+            astro_mode2(r.as, r.s, lane, x, S);
         }
         // flush the unit's window
         __syncwarp();
         for (int i = lane; i < 3 * win; i += 32) {
             const int ax = i / win, k = i - ax * win;
             const double vacc = xw[ax * ws + k];
-            if (vacc != 0.0) {
-                atomicAdd(xatt + ax * D + un.a0 + k, vacc);   // knot < D whenever vacc != 0
-            }
+            if (vacc != 0.0 && un.a0 + k < D) atomicAdd(xatt + ax * D + un.a0 + k, vacc);
         }
     }
     // global column: one atomic per warp
@@ -366,11 +449,10 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
     double* xi = sm;
     double* xw = sm + ((I + 1) & ~1) + warp * 6 * ws;   // window of v (read)
     double* tw = xw + 3 * ws;                           // window of A^T u_hat (accumulate)
-    // u_hat and the window offsets of the current tile reach the attitude lanes through shared
-    // memory: wide broadcast loads (two u_hat, four offsets per request) cost the LSU data pipe
-    // far less than one or two 32-bit shuffles per row and step
+    // u_hat of the current tile reaches the attitude lanes through shared memory (by attitude
+    // slot): wide broadcast loads, two u_hat per request, cost the LSU data pipe far less than
+    // two 32-bit shuffles per slot
     double* ysm = sm + ((I + 1) & ~1) + NWARP * 6 * ws + warp * 48;
-    uint32_t* asm_ = (uint32_t*)(ysm + 32);
     const double* xatt = x + 5 * S;
     const double* xins = x + 5 * S + 3 * D;
     double* tatt = tacc + 5 * S;
@@ -379,11 +461,13 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
     const double ca = *ca_p;
     __syncthreads();
 
-    const int h = lane >> 4, j = lane & 15, jj = min(j, 11);
+    const int h = lane >> 4, jj = min(lane & 15, 11), act = (lane & 15) < 12;
     const int axo = (jj >> 2) * ws + (jj & 3);
-    const bool att_lane = j < 12;
     const bool lo12 = lane < 12, hi12 = lane >= 16 && lane < 28;
+    const int myslot = att_slot(lane);
     double g = 0.0;
+    RegsA ra;
+    zero_A(ra);
     for (;;) {
         const int u = fetch_unit(counter, lane);
         if (u >= n_units) break;
@@ -399,10 +483,9 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
         double q = 0.0;
         const unsigned char* T = tiles + (int64_t)un.tile0 * TILE_BYTES;
         // Loads are issued as soon as the registers they fill are dead (volatile asm keeps the
-        // program order): the next tile's instrumental values and columns right after mode 1,
-        // its attitude coefficients group by group inside the read-modify-write loop, the rest
-        // (star, astrometric, global) at the top of its own iteration.
-        RegsA ra;
+        // program order): the next tile's window offsets, instrumental values and columns right
+        // after mode 1, its attitude coefficients pair by pair inside the read-modify-write
+        // loop, the rest (star, astrometric, global) at the top of its own iteration.
         RegsB r;
         load_A(T, lane, ra);
         load_B_instr(T, lane, r);
@@ -412,119 +495,44 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
             const int64_t ri = ((int64_t)un.tile0 + t) * R + lane;
             const double yold = __ldcs(y + ri);
             // ---- mode 1 for this tile
-            // products of rows q and q+8 are formed together and go straight into the first
-            // butterfly step, so that only 8 of the 16 partial products are ever live
-            double p[8];
-            asm_[lane] = ra.aoff;
-            __syncwarp();
-            {
-                const bool up8 = (j & 8) != 0;
-#pragma unroll
-                for (int g4 = 0; g4 < 2; ++g4) {
-                    const uint4 alo = *(const uint4*)(asm_ + h * 16 + 4 * g4);
-                    const uint4 ahi = *(const uint4*)(asm_ + h * 16 + 4 * g4 + 8);
-                    const uint32_t al[4] = {alo.x, alo.y, alo.z, alo.w};
-                    const uint32_t ah[4] = {ahi.x, ahi.y, ahi.z, ahi.w};
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const int q0 = 4 * g4 + i;
-                        double plo = ra.at[q0] * xw[al[i] + axo];
-                        double phi = ra.at[q0 + 8] * xw[ah[i] + axo];
-                        plo = att_lane ? plo : 0.0;
-                        phi = att_lane ? phi : 0.0;
-                        const double send = up8 ? plo : phi;
-                        const double keep = up8 ? phi : plo;
-                        p[q0] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-                    }
-                }
-            }
-#pragma unroll
-            for (int o = 4; o > 0; o >>= 1) {
-                const bool up = (j & o) != 0;
-#pragma unroll
-                for (int i = 0; i < o; ++i) {
-                    const double send = up ? p[i] : p[i + o];
-                    const double keep = up ? p[i + o] : p[i];
-                    p[i] = keep + __shfl_xor_sync(0xffffffffu, send, o);
-                }
-            }
-            double sum = p[0];
+            double sum = att_mode1(ra, xw, axo, lane);
+            uint32_t awn[4];
+            ld_aoff(Tn, h, awn);
+            const uint32_t cmaskn = ld_stream_u32(Tn + OFF_CMASK);
             const double* xa = x + 5 * (int64_t)r.s;
 #pragma unroll
             for (int k = 0; k < 5; ++k) sum = fma(r.as[k], __ldg(xa + k), sum);
 #pragma unroll
-            for (int k = 0; k < 6; ++k) sum = fma(r.in[k], xi[r.c[k]], sum);
+            for (int k = 0; k < 6; ++k) sum = fma(r.in[k], xi[icol_of(r.cw, k)], sum);
             sum = fma(r.gl, xg, sum);
             const double yv = fma(ca, yold, sum);   // u_hat of this row (padding rows: 0)
             y[ri] = yv;
-            ysm[lane] = yv;
+            ysm[myslot] = yv;
             q = fma(yv, yv, q);
             load_B_instr(Tn, lane, r);
-            // ---- mode 2 for this tile, attitude
-            const uint32_t a_other = __shfl_xor_sync(0xffffffffu, ra.aoff, 16);
-            const int da = (int)ra.aoff - (int)a_other;
-            const unsigned cmask = __ballot_sync(0xffffffffu, da > -4 && da < 4);
-            ra.aoff = ld_stream_u16(Tn + OFF_AOFF + lane * 2);
             __syncwarp();   // ysm visible to the whole warp
+            // ---- mode 2 for this tile, attitude
 #pragma unroll
             for (int g4 = 0; g4 < 4; ++g4) {
-                const uint4 a4 = *(const uint4*)(asm_ + h * 16 + 4 * g4);
                 const double2 y01 = *(const double2*)(ysm + h * 16 + 4 * g4);
                 const double2 y23 = *(const double2*)(ysm + h * 16 + 4 * g4 + 2);
-                const uint32_t aa[4] = {a4.x, a4.y, a4.z, a4.w};
                 const double yy4[4] = {y01.x, y01.y, y23.x, y23.y};
 #pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    const int qq = 4 * g4 + i;
-                    const double add = ra.at[qq] * yy4[i];
-                    double* pa = tw + aa[i] + axo;
-                    if ((cmask >> qq) & 1u) {
-                        if (lo12) *pa += add;
-                        __syncwarp();
-                        if (hi12) *pa += add;
-                    } else {
-                        if (lo12 || hi12) *pa += add;
-                    }
-                    __syncwarp();
-                }
+                for (int i = 0; i < 4; ++i) att_mode2_step<false>(ra, 4 * g4 + i, yy4[i], tw, axo, lo12, hi12, win);
 #pragma unroll
-                for (int i = 0; i < 4; ++i)
-                    ra.at[4 * g4 + i] = ld_stream_f64(Tn + OFF_ATTV + (((4 * g4 + i) * 2 + h) * 12 + jj) * 8);
+                for (int i = 0; i < 2; ++i) {
+                    const int ip = 2 * g4 + i;
+                    ld_att_pair(Tn + OFF_ATTV + ((ip * 2 + h) * 12 + jj) * 16, act, ra.at[2 * ip], ra.at[2 * ip + 1]);
+                }
             }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) ra.aw[i] = awn[i];
+            ra.cmask = cmaskn;
             // ---- mode 2, global and astrometric
             g = fma(r.gl, yv, g);
 #pragma unroll
             for (int k = 0; k < 5; ++k) r.as[k] *= yv;
-            const int32_t s_up = __shfl_up_sync(0xffffffffu, r.s, 1);
-            const bool head = lane == 0 || s_up != r.s;
-            const unsigned heads = __ballot_sync(0xffffffffu, head);
-            if (heads == 1u) {
-#pragma unroll
-                for (int k = 0; k < 5; ++k) {
-                    const double tsum = warp_sum(r.as[k]);
-                    if (lane == 0 && tsum != 0.0) atomicAdd(tacc + 5 * (int64_t)r.s + k, tsum);
-                }
-            } else {
-                const unsigned below = heads & ((2u << lane) - 1u);
-                const int seg_start = 31 - __clz(below);
-                const bool tail = lane == 31 || ((heads >> (lane + 1)) & 1u);
-                const unsigned n1 = ~heads, n2 = n1 & (n1 >> 1), n4 = n2 & (n2 >> 2),
-                               n8 = n4 & (n4 >> 4), n16 = n8 & (n8 >> 8);
-                const unsigned need = 1u | (n2 ? 2u : 0u) | (n4 ? 4u : 0u) | (n8 ? 8u : 0u) | (n16 ? 16u : 0u);
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    if (need & o) {
-#pragma unroll
-                        for (int k = 0; k < 5; ++k) {
-                            const double up = __shfl_up_sync(0xffffffffu, r.as[k], o);
-                            if (lane - o >= seg_start) r.as[k] += up;
-                        }
-                    }
-                }
-#pragma unroll
-                for (int k = 0; k < 5; ++k)
-                    if (tail && r.as[k] != 0.0) atomicAdd(tacc + 5 * (int64_t)r.s + k, r.as[k]);
-            }
+            astro_mode2(r.as, r.s, lane, tacc, S);
         }
         q = warp_sum(q);
         if (lane == 0) partials[u] = q;
@@ -532,7 +540,7 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
         for (int i = lane; i < 3 * win; i += 32) {
             const int ax = i / win, k = i - ax * win;
             const double vacc = tw[ax * ws + k];
-            if (vacc != 0.0) atomicAdd(tatt + ax * D + un.a0 + k, vacc);
+            if (vacc != 0.0 && un.a0 + k < D) atomicAdd(tatt + ax * D + un.a0 + k, vacc);
         }
     }
     g = warp_sum(g);
@@ -578,12 +586,14 @@ __global__ void __launch_bounds__(TPB) k_aprod2_instr(const unsigned char* __res
     const int64_t nw = (int64_t)gridDim.x * NWARP;
     for (int64_t tile = w0; tile < n_tiles; tile += nw) {
         const unsigned char* T = tiles + tile * TILE_BYTES;
-        uint32_t c[6];
+        uint32_t cw[3], c[6];
         double v[6];
 #pragma unroll
-        for (int k = 0; k < 6; ++k) c[k] = ld_stream_u16(T + OFF_ICOL + (k * R + lane) * 2);
+        for (int k = 0; k < 3; ++k) cw[k] = ld_stream_u32(T + OFF_ICOL + (k * R + lane) * 4);
 #pragma unroll
         for (int k = 0; k < 6; ++k) v[k] = ld_stream_f64(T + OFF_INSTRV + (k * R + lane) * 8);
+#pragma unroll
+        for (int k = 0; k < 6; ++k) c[k] = icol_of(cw, k);
         const double yv = __ldcs(y + tile * R + lane) * scale;
         if (FIXED) {
             unsigned* acc32 = (unsigned*)acc;
@@ -597,7 +607,8 @@ __global__ void __launch_bounds__(TPB) k_aprod2_instr(const unsigned char* __res
             }
         } else {
 #pragma unroll
-            for (int k = 0; k < 6; ++k) atomicAdd(acc + c[k], v[k] * yv);
+            for (int k = 0; k < 6; ++k) smem_add_f64(acc + c[k], v[k] * yv);
+            __syncwarp();
         }
     }
     __syncthreads();

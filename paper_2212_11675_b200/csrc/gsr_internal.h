@@ -11,22 +11,30 @@ namespace gsr {
 
 // ---- device layout ------------------------------------
 // Rows are stored in WARP TILES of R = 32 rows; a tile is one contiguous, 128-byte-aligned
-// record that one warp streams (lane r <-> row r of the tile):
-//   astro [5][32] f64   plane-major: lane r reads consecutive addresses, 256 B per request
-//   att   [16][2][12] f64  ROW-major and half-interleaved: record q holds the 12 attitude
-//         coefficients of row q and then those of row 16+q, so that lanes 0-11 (rows 0-15) and
-//         lanes 16-27 (rows 16-31) each fetch one coefficient of one row per request (192
-//         contiguous bytes) and end up owning a COLUMN of the 32x12 block: lane j holds
-//         coefficient j of 16 rows.  aprod2 then adds row after row into the window with 12
-//         lanes at 12 distinct addresses (plain read-modify-write, no atomics); aprod1 forms
-//         the 12 products per row the same way and transposes them back with 15 shuffles.
+// record that one warp streams.  Lane l of the warp is the HOME LANE of tile row l: the
+// plane-major fields below (astro, instr, icol, glob, star) and the m-sized vectors are indexed
+// by home lane, and rows are star-sorted along the home lanes.
+//   astro [5][32] f64   plane-major: lane l reads consecutive addresses, 256 B per request
+//   att   [8][2][12][2] f64  the 32x12 attitude block by ATTITUDE SLOT (h, q), h < 2, q < 16
+//         (att_slot() maps a home lane to its slot): record (i, h) holds coefficient j of slots
+//         (h, 2i) and (h, 2i+1) side by side, so that lane (h, j), j < 12, fetches 16 bytes per
+//         request and the 24 lanes of a request cover 384 contiguous bytes = 3 whole lines.  A
+//         lane ends up owning a COLUMN of the 32x12 block: coefficient j of the 16 slots of its
+//         half.  aprod2 then adds slot after slot into the window with 12 lanes at 12 distinct
+//         addresses (plain read-modify-write, no atomics); aprod1 forms the 12 products per
+//         slot the same way and sums them over the lanes with fp64 tensor-core MMAs whose
+//         constant operands select and add (reduce_slots() in gsr_aprod.cu).
 //   instr [6][32] f64   plane-major
-//   icol  [6][32] u16   instrumental columns (I <= 65535 is implied by the shared-memory plan)
+//   icol  [3][32] u32   instrumental columns, two u16 per word: columns 2k | 2k+1 << 16
+//                       (I <= 65535 is implied by the shared-memory plan)
 //   glob  [32] f64
 //   star  [32] i32
-//   aoff  [32] u16      att_start - a0 of the unit (offset inside the warp's window)
+//   aoff  [2][16] u8    att_start - a0 of the unit (offset inside the warp's window), by
+//                       attitude slot; the window is at most 256 knots wide
 //   a0    i32           first knot of the window (same for every tile of a unit)
-//   60 bytes of padding                                                = 6784 B = 212 B/row
+//   cmask u32           bit q: the windows of slots (0, q) and (1, q) overlap (|da| < 4), so
+//                       aprod2 must add them one after the other
+//   padding up to                                                       6784 B = 212 B/row
 //
 // INTERNAL ROW ORDER.  LSQR only ever touches the m-sized vectors through A and A^T, so the
 // solver is free to keep them in any row order.  Rows are ingested in segments of SEG rows;
@@ -48,15 +56,29 @@ constexpr int OFF_ICOL = OFF_INSTRV + 6 * R * 8;    // 5888 (instrumental values
 constexpr int OFF_GLOBV = OFF_ICOL + 6 * R * 2;     // 6272
 constexpr int OFF_STAR = OFF_GLOBV + R * 8;         // 6528
 constexpr int OFF_AOFF = OFF_STAR + R * 4;          // 6656
-constexpr int OFF_A0 = OFF_AOFF + R * 2;            // 6720: i32 first knot of the tile's window
+constexpr int OFF_A0 = OFF_AOFF + R;                // 6688: i32 first knot of the tile's window
+constexpr int OFF_CMASK = OFF_A0 + 4;               // 6692
 constexpr int TILE_BYTES = 6784;                    // 53 * 128
-static_assert(OFF_A0 + 4 <= TILE_BYTES && TILE_BYTES % 128 == 0, "tile record");
-// byte offset of coefficient k (paper order) of row lr inside a tile record
+static_assert(OFF_CMASK + 4 <= TILE_BYTES && TILE_BYTES % 128 == 0, "tile record");
+// attitude slot 16*h + q of home lane l.  The mapping is the one the MMA reduction of aprod1
+// delivers its sums in (reduce_slots() in gsr_aprod.cu): lane l receives the sum of slot
+//   h = bit 2 of l,  q = 8 * (bit 3 of l) + 2 * (l & 3) + (bit 4 of l).
+__host__ __device__ inline int att_slot(int l) {
+    return 16 * ((l >> 2) & 1) + 8 * ((l >> 3) & 1) + 2 * (l & 3) + (l >> 4);
+}
+// byte offset of coefficient k (paper order) of home lane lr inside a tile record
 __host__ __device__ inline int val_offset(int k, int lr) {
     if (k < 5) return OFF_ASTRO + (k * R + lr) * 8;
-    if (k < 17) return OFF_ATTV + (((lr & 15) * 2 + (lr >> 4)) * 12 + (k - 5)) * 8;
+    if (k < 17) {
+        const int sl = att_slot(lr), h = sl >> 4, q = sl & 15;
+        return OFF_ATTV + ((((q >> 1) * 2 + h) * 12 + (k - 5)) * 2 + (q & 1)) * 8;
+    }
     if (k < 23) return OFF_INSTRV + ((k - 17) * R + lr) * 8;
     return OFF_GLOBV + lr * 8;
+}
+// instrumental column j of home lane lr
+__host__ __device__ inline int icol_offset(int j, int lr) {
+    return OFF_ICOL + ((j >> 1) * R + lr) * 4 + (j & 1) * 2;
 }
 
 constexpr int64_t SEG = 1 << 22;             // rows per ingest segment

@@ -154,10 +154,10 @@ __global__ void __launch_bounds__(BLK) k_seg_scatter(
     perm[dst] = (uint32_t)(row_base_ext + r);
     ((int32_t*)(T + OFF_STAR))[lr] = star[r];
     const int a0 = bin * bin_width;
-    ((uint16_t*)(T + OFF_AOFF))[lr] = (uint16_t)(bin == 0 && (a < 0 || a > D - 4) ? 0 : a - a0);
+    (T + OFF_AOFF)[att_slot(lr)] = (unsigned char)(bin == 0 && (a < 0 || a > D - 4) ? 0 : a - a0);
     *(int32_t*)(T + OFF_A0) = a0;   // same value from every row of the tile
 #pragma unroll
-    for (int j = 0; j < 6; ++j) ((uint16_t*)(T + OFF_ICOL))[j * R + lr] = (uint16_t)instr[6 * r + j];
+    for (int j = 0; j < 6; ++j) *(uint16_t*)(T + icol_offset(j, lr)) = (uint16_t)instr[6 * r + j];
 #pragma unroll
     for (int k = 0; k < NPAR; ++k) *(double*)(T + val_offset(k, lr)) = vals[NPAR * r + k];
 }
@@ -168,7 +168,9 @@ __global__ void k_save_last_star(const int32_t* __restrict__ star, int64_t ns, i
 
 // Padding rows (they round every bin up to whole tiles and trail the bin's real rows): zero
 // coefficients, window offset 0 and instrumental column 0 (tiles are memset to 0); star = the
-// star of the last real row of the tile, so that they open no new star segment.
+// star of the last real row of the tile, so that they open no new star segment.  Also writes
+// the tile's overlap mask: bit q is set when the windows of attitude slots (0, q) and (1, q)
+// overlap, i.e. when aprod2 must not add the two in one instruction.
 // One warp per tile.
 __global__ void __launch_bounds__(256) k_fix_padding(unsigned char* __restrict__ tiles,
                                                      const uint32_t* __restrict__ perm,
@@ -180,6 +182,9 @@ __global__ void __launch_bounds__(256) k_fix_padding(unsigned char* __restrict__
     const bool real = perm[t * R + lane] != PERM_PAD;
     const int nreal = __popc(__ballot_sync(0xffffffffu, real));
     if (!real) ((int32_t*)(T + OFF_STAR))[lane] = nreal > 0 ? ((const int32_t*)(T + OFF_STAR))[nreal - 1] : 0;
+    const int da = (int)(T + OFF_AOFF)[lane & 15] - (int)(T + OFF_AOFF)[16 + (lane & 15)];
+    const unsigned cmask = __ballot_sync(0xffffffffu, lane < 16 && da > -4 && da < 4);
+    if (lane == 0) *(uint32_t*)(T + OFF_CMASK) = cmask;
 }
 
 // Caller-order dump of rows [row0, row0+nrows): every internal row whose caller row falls in
@@ -196,13 +201,13 @@ __global__ void k_expand_rows(const unsigned char* __restrict__ tiles, const uin
     const unsigned char* T = tiles + (ri / R) * (int64_t)TILE_BYTES;
     const int lr = (int)(ri % R);
     const int64_t s = ((const int32_t*)(T + OFF_STAR))[lr];
-    const int64_t a = (int64_t)(*(const int32_t*)(T + OFF_A0)) + ((const uint16_t*)(T + OFF_AOFF))[lr];
+    const int64_t a = (int64_t)(*(const int32_t*)(T + OFF_A0)) + (T + OFF_AOFF)[att_slot(lr)];
     const int64_t off_att = 5 * S, off_instr = off_att + 3 * D, off_glob = off_instr + I;
     for (int k = 0; k < NPAR; ++k) {
         int64_t c;
         if (k < 5) c = 5 * s + k;
         else if (k < 17) c = off_att + ((k - 5) / 4) * D + a + (k - 5) % 4;
-        else if (k < 23) c = off_instr + ((const uint16_t*)(T + OFF_ICOL))[(k - 17) * R + lr];
+        else if (k < 23) c = off_instr + *(const uint16_t*)(T + icol_offset(k - 17, lr));
         else c = off_glob;
         cols[NPAR * r + k] = c;
         vals[NPAR * r + k] = *(const double*)(T + val_offset(k, lr));
@@ -226,7 +231,7 @@ __global__ void __launch_bounds__(256) k_scale_values(unsigned char* __restrict_
     unsigned char* T = tiles + t * TILE_BYTES;
     const int lr = threadIdx.x & 31;
     const int64_t s = ((const int32_t*)(T + OFF_STAR))[lr];
-    const int64_t a = (int64_t)(*(const int32_t*)(T + OFF_A0)) + ((const uint16_t*)(T + OFF_AOFF))[lr];
+    const int64_t a = (int64_t)(*(const int32_t*)(T + OFF_A0)) + (T + OFF_AOFF)[att_slot(lr)];
     const double* pa = p + 5 * s;
     const double* pt = p + 5 * S + a;
     const double* pi = p + 5 * S + 3 * D;
@@ -238,7 +243,7 @@ __global__ void __launch_bounds__(256) k_scale_values(unsigned char* __restrict_
         for (int j = 0; j < 4; ++j) *(double*)(T + val_offset(5 + 4 * ax + j, lr)) *= pt[ax * D + j];
 #pragma unroll
     for (int j = 0; j < 6; ++j) {
-        const int c = ((const uint16_t*)(T + OFF_ICOL))[j * R + lr];
+        const int c = *(const uint16_t*)(T + icol_offset(j, lr));
         *(double*)(T + val_offset(17 + j, lr)) *= pi[c];
     }
     *(double*)(T + val_offset(23, lr)) *= pi[I];
