@@ -41,8 +41,8 @@ __device__ __forceinline__ double warp_sum(double v) {
 // D(8x8) += A(8x4) B(4x8), fp64 (DMMA).  Fragments: lane l holds A[l>>2][l&3], B[l&3][l>>2] and
 // D[l>>2][2(l&3) + {0,1}].
 __device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+        : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
 // Lane (h, j) = 16h + j holds p[q], its term of attitude slot (h, q), q < 16 (lanes j >= 12
@@ -52,24 +52,26 @@ __device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b)
 //   stage 2, four MMAs:      S[i][q'] = sum over the 4 lane groups of half (i&1) of D1_b[q'][.]
 //            with b = (i>>1)&1; rows i and i+4 are duplicates, so that every lane finds one slot
 //            sum in its own D fragment: lanes 0-15 take column 2(l&3), lanes 16-31 the next.
-// The MMAs run on the fp64 tensor pipe (4 cycles each per SM, measured), which is otherwise idle;
-// the 15-shuffle butterfly this replaces cost 30 LSU wavefronts per tile.
+// Four independent accumulator chains in stage 1 and two in stage 2 keep the dependent depth at
+// 4 + 2 MMAs.  The MMAs run on the fp64 tensor pipe (4 cycles each per SM, measured), which is
+// otherwise idle; the 15-shuffle butterfly this replaces cost 30 LSU wavefronts per tile.
 __device__ __forceinline__ double reduce_slots(const double (&p)[16], int lane) {
     const int grp = lane >> 2;
-    double d1[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+    double d1[4][2] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};   // [b + 2 * (q & 1)]
 #pragma unroll
     for (int q = 0; q < 16; ++q) {
         const double sel = __hiloint2double(grp == (q & 7) ? 0x3FF00000 : 0, 0);
-        dmma(d1[q >> 3][0], d1[q >> 3][1], sel, p[q]);
+        const int c = (q >> 3) + 2 * (q & 1);
+        dmma(d1[c][0], d1[c][1], sel, p[q]);
     }
-    double s0 = 0.0, s1 = 0.0;
+    double s[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
 #pragma unroll
     for (int b = 0; b < 2; ++b) {
         const double a2 = __hiloint2double((grp & 3) == 2 * b + ((lane & 3) >> 1) ? 0x3FF00000 : 0, 0);
-        dmma(s0, s1, a2, d1[b][0]);
-        dmma(s0, s1, a2, d1[b][1]);
+        dmma(s[b][0], s[b][1], a2, d1[b][0] + d1[b + 2][0]);
+        dmma(s[b][0], s[b][1], a2, d1[b][1] + d1[b + 2][1]);
     }
-    return (lane >> 4) ? s1 : s0;
+    return (lane >> 4) ? s[0][1] + s[1][1] : s[0][0] + s[1][0];
 }
 
 // A tile is consumed in two phases so that the loads of one phase are in flight while the
@@ -164,6 +166,15 @@ __device__ __forceinline__ void smem_add_f64(double* addr, double v) {
     } while (assumed != old);
 }
 
+// Bulk L2 prefetch (TMA unit, one instruction from one lane, nothing on the LSU pipe): the
+// tile PF_TILES ahead and its slice of the m-sized vector are on their way to L2 while the warp
+// works, so that the register loads issued one tile ahead find their lines there (about 300
+// cycles away instead of HBM's 800+).  Bytes in flight no longer depend on registers.
+constexpr int PF_TILES = 2;
+__device__ __forceinline__ void prefetch_l2(const void* p, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
 __device__ __forceinline__ int fetch_unit(int* counter, int lane) {
     int u = 0;
     if (lane == 0) u = atomicAdd(counter, 1);
@@ -180,15 +191,16 @@ __device__ __forceinline__ double att_mode1(const RegsA& ra, const double* xw, i
 
 // attitude part of aprod2 for one slot pair: slot (0, q) through lanes 0-11,
 // slot (1, q) through lanes 16-27, one slot per half and step; the two slots of a step go in
-// one instruction unless their windows overlap (cmask; then one after the other).
-// SQUARE: add the squared coefficients instead.
-template <bool SQUARE>
+// one instruction unless their windows overlap (cmask; then one after the other).  CHECK =
+// false: the tile has no overlapping pair (cmask == 0, about half of all tiles), no test per
+// step.  SQUARE: add the squared coefficients instead.
+template <bool SQUARE, bool CHECK>
 __device__ __forceinline__ void att_mode2_step(const RegsA& ra, int q, double yy, double* tw, int axo,
                                                bool lo12, bool hi12, int ws_dbg) {
     double* pa = tw + aoff_of(ra.aw, q) + axo;
     GSR_ASSERT((int)aoff_of(ra.aw, q) + 3 < ws_dbg);
     const double c = ra.at[q];
-    if ((ra.cmask >> q) & 1u) {
+    if (CHECK && ((ra.cmask >> q) & 1u)) {
         if (lo12) *pa = SQUARE ? fma(c, c, *pa) : fma(c, yy, *pa);
         __syncwarp();
         if (hi12) *pa = SQUARE ? fma(c, c, *pa) : fma(c, yy, *pa);
@@ -196,6 +208,34 @@ __device__ __forceinline__ void att_mode2_step(const RegsA& ra, int q, double yy
         if (lo12 || hi12) *pa = SQUARE ? fma(c, c, *pa) : fma(c, yy, *pa);
     }
     __syncwarp();
+}
+
+// the 16 steps of one tile; NEXT: reload the attitude coefficients of the next tile (Tn) pair by
+// pair as soon as their registers are dead (k_fused)
+template <bool SQUARE, bool CHECK, bool NEXT>
+__device__ __forceinline__ void att_mode2_tile(RegsA& ra, const double* ysm, double* tw, int axo, int lane,
+                                               const unsigned char* Tn, int ws_dbg) {
+    const int h = lane >> 4, jj = min(lane & 15, 11), act = (lane & 15) < 12;
+    const bool lo12 = lane < 12, hi12 = lane >= 16 && lane < 28;
+#pragma unroll
+    for (int g4 = 0; g4 < 4; ++g4) {
+        double yy4[4] = {0.0, 0.0, 0.0, 0.0};
+        if (!SQUARE) {
+            const double2 y01 = *(const double2*)(ysm + h * 16 + 4 * g4);
+            const double2 y23 = *(const double2*)(ysm + h * 16 + 4 * g4 + 2);
+            yy4[0] = y01.x; yy4[1] = y01.y; yy4[2] = y23.x; yy4[3] = y23.y;
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+            att_mode2_step<SQUARE, CHECK>(ra, 4 * g4 + i, yy4[i], tw, axo, lo12, hi12, ws_dbg);
+        if (NEXT) {
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const int ip = 2 * g4 + i;
+                ld_att_pair(Tn + OFF_ATTV + ((ip * 2 + h) * 12 + jj) * 16, act, ra.at[2 * ip], ra.at[2 * ip + 1]);
+            }
+        }
+    }
 }
 
 // astrometric part of aprod2 for one tile: segmented reduction over the
@@ -279,10 +319,15 @@ __global__ void __launch_bounds__(TPB) k_aprod1(const unsigned char* __restrict_
         double q = 0.0;
         const unsigned char* T = tiles + (int64_t)un.tile0 * TILE_BYTES;
         load_A(T, lane, ra);
+        if (lane == 0 && un.ntiles > 1) prefetch_l2(T + TILE_BYTES, TILE_BYTES);
         for (int t = 0; t < un.ntiles; ++t, T += TILE_BYTES) {
             RegsB r;
             load_B(T, lane, r);
             const int64_t ri = ((int64_t)un.tile0 + t) * R + lane;
+            if (lane == 0 && t + PF_TILES < un.ntiles) {
+                prefetch_l2(T + PF_TILES * TILE_BYTES, TILE_BYTES);
+                if (!PERM) prefetch_l2(y + ri + PF_TILES * R, R * 8);
+            }
             int64_t ry = ri;
             bool live = true;
             if (PERM) {
@@ -346,9 +391,8 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
     const double sy = SQUARE ? 1.0 : *sy_p;
     __syncthreads();
 
-    const int h = lane >> 4, jj = min(lane & 15, 11);
+    const int jj = min(lane & 15, 11);
     const int axo = (jj >> 2) * ws + (jj & 3);
-    const bool lo12 = lane < 12, hi12 = lane >= 16 && lane < 28;
     const int myslot = att_slot(lane);
     double* xatt = x + 5 * S;
     double g = 0.0;
@@ -363,10 +407,15 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
         __syncwarp();
         const unsigned char* T = tiles + (int64_t)un.tile0 * TILE_BYTES;
         load_A(T, lane, ra);
+        if (lane == 0 && un.ntiles > 1) prefetch_l2(T + TILE_BYTES, TILE_BYTES);
         for (int t = 0; t < un.ntiles; ++t, T += TILE_BYTES) {
             RegsB r;
             load_B(T, lane, r);
             const int64_t ri = ((int64_t)un.tile0 + t) * R + lane;
+            if (lane == 0 && t + PF_TILES < un.ntiles) {
+                prefetch_l2(T + PF_TILES * TILE_BYTES, TILE_BYTES);
+                if (!SQUARE && !PERM) prefetch_l2(y + ri + PF_TILES * R, R * 8);
+            }
             double yv = 1.0;
             if (!SQUARE) {
                 if (PERM) {
@@ -379,17 +428,8 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
                 __syncwarp();
             }
             // phase A -- attitude
-#pragma unroll
-            for (int g4 = 0; g4 < 4; ++g4) {
-                double yy4[4] = {0.0, 0.0, 0.0, 0.0};
-                if (!SQUARE) {
-                    const double2 y01 = *(const double2*)(ysm + h * 16 + 4 * g4);
-                    const double2 y23 = *(const double2*)(ysm + h * 16 + 4 * g4 + 2);
-                    yy4[0] = y01.x; yy4[1] = y01.y; yy4[2] = y23.x; yy4[3] = y23.y;
-                }
-#pragma unroll
-                for (int i = 0; i < 4; ++i) att_mode2_step<SQUARE>(ra, 4 * g4 + i, yy4[i], xw, axo, lo12, hi12, win);
-            }
+            if (ra.cmask == 0u) att_mode2_tile<SQUARE, false, false>(ra, ysm, xw, axo, lane, nullptr, win);
+            else att_mode2_tile<SQUARE, true, false>(ra, ysm, xw, axo, lane, nullptr, win);
             if (t + 1 < un.ntiles) load_A(T + TILE_BYTES, lane, ra);   // in flight during phase B
             // phase B
 #pragma unroll
@@ -461,9 +501,8 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
     const double ca = *ca_p;
     __syncthreads();
 
-    const int h = lane >> 4, jj = min(lane & 15, 11), act = (lane & 15) < 12;
+    const int h = lane >> 4, jj = min(lane & 15, 11);
     const int axo = (jj >> 2) * ws + (jj & 3);
-    const bool lo12 = lane < 12, hi12 = lane >= 16 && lane < 28;
     const int myslot = att_slot(lane);
     double g = 0.0;
     RegsA ra;
@@ -489,10 +528,15 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
         RegsB r;
         load_A(T, lane, ra);
         load_B_instr(T, lane, r);
+        if (lane == 0 && un.ntiles > 1) prefetch_l2(T + TILE_BYTES, TILE_BYTES);
         for (int t = 0; t < un.ntiles; ++t, T += TILE_BYTES) {
             const unsigned char* Tn = t + 1 < un.ntiles ? T + TILE_BYTES : T;   // (last: harmless reload)
             load_B_rest(T, lane, r);
             const int64_t ri = ((int64_t)un.tile0 + t) * R + lane;
+            if (lane == 0 && t + PF_TILES < un.ntiles) {
+                prefetch_l2(T + PF_TILES * TILE_BYTES, TILE_BYTES);
+                prefetch_l2(y + ri + PF_TILES * R, R * 8);
+            }
             const double yold = __ldcs(y + ri);
             // ---- mode 1 for this tile
             double sum = att_mode1(ra, xw, axo, lane);
@@ -512,19 +556,8 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
             load_B_instr(Tn, lane, r);
             __syncwarp();   // ysm visible to the whole warp
             // ---- mode 2 for this tile, attitude
-#pragma unroll
-            for (int g4 = 0; g4 < 4; ++g4) {
-                const double2 y01 = *(const double2*)(ysm + h * 16 + 4 * g4);
-                const double2 y23 = *(const double2*)(ysm + h * 16 + 4 * g4 + 2);
-                const double yy4[4] = {y01.x, y01.y, y23.x, y23.y};
-#pragma unroll
-                for (int i = 0; i < 4; ++i) att_mode2_step<false>(ra, 4 * g4 + i, yy4[i], tw, axo, lo12, hi12, win);
-#pragma unroll
-                for (int i = 0; i < 2; ++i) {
-                    const int ip = 2 * g4 + i;
-                    ld_att_pair(Tn + OFF_ATTV + ((ip * 2 + h) * 12 + jj) * 16, act, ra.at[2 * ip], ra.at[2 * ip + 1]);
-                }
-            }
+            if (ra.cmask == 0u) att_mode2_tile<false, false, true>(ra, ysm, tw, axo, lane, Tn, win);
+            else att_mode2_tile<false, true, true>(ra, ysm, tw, axo, lane, Tn, win);
 #pragma unroll
             for (int i = 0; i < 4; ++i) ra.aw[i] = awn[i];
             ra.cmask = cmaskn;

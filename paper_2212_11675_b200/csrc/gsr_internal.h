@@ -34,6 +34,11 @@ namespace gsr {
 //   a0    i32           first knot of the window (same for every tile of a unit)
 //   cmask u32           bit q: the windows of slots (0, q) and (1, q) overlap (|da| < 4), so
 //                       aprod2 must add them one after the other
+//   iperm [32] u16      instrumental slot code of home lane l: sum_e slot(e) 6^e, where the
+//                       caller's e-th instrumental entry sits in slot(e) of instr / icol.  The
+//                       entries of a row are permuted among the six slots at ingest so that the
+//                       16 rows of a half-warp spread over the shared-memory banks in every
+//                       slot (k_permute_instr); only gsr_debug_expand_rows reads the code
 //   padding up to                                                       6784 B = 212 B/row
 //
 // INTERNAL ROW ORDER.  LSQR only ever touches the m-sized vectors through A and A^T, so the
@@ -58,8 +63,9 @@ constexpr int OFF_STAR = OFF_GLOBV + R * 8;         // 6528
 constexpr int OFF_AOFF = OFF_STAR + R * 4;          // 6656
 constexpr int OFF_A0 = OFF_AOFF + R;                // 6688: i32 first knot of the tile's window
 constexpr int OFF_CMASK = OFF_A0 + 4;               // 6692
+constexpr int OFF_IPERM = OFF_CMASK + 4;            // 6696
 constexpr int TILE_BYTES = 6784;                    // 53 * 128
-static_assert(OFF_CMASK + 4 <= TILE_BYTES && TILE_BYTES % 128 == 0, "tile record");
+static_assert(OFF_IPERM + R * 2 <= TILE_BYTES && TILE_BYTES % 128 == 0, "tile record");
 // attitude slot 16*h + q of home lane l.  The mapping is the one the MMA reduction of aprod1
 // delivers its sums in (reduce_slots() in gsr_aprod.cu): lane l receives the sum of slot
 //   h = bit 2 of l,  q = 8 * (bit 3 of l) + 2 * (l & 3) + (bit 4 of l).
