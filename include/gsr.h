@@ -49,7 +49,8 @@ typedef enum {
     GSR_ENOMEM = -2,       /* cudaMalloc failed */
     GSR_ECUDA = -3,        /* a CUDA runtime call failed (sticky error is cleared) */
     GSR_ESTATE = -4,       /* call not legal in the handle's state */
-    GSR_EUNSUPPORTED = -5  /* device is not sm_100 */
+    GSR_EUNSUPPORTED = -5, /* device is not sm_100, size limit (see gsr_matrix_begin) or option */
+    GSR_ERANGE = -6        /* GSR_OPT_DETERMINISTIC: a pass left the range of its fixed-point sums */
 } gsr_status;
 
 typedef struct {
@@ -186,8 +187,19 @@ int gsr_lsqr_set_damp(gsr_matrix* A, double damp);
 enum {
     GSR_OPT_FORCE_ITNLIM = 1, /* 1: rules 1-6 are evaluated and recorded in *_natural but only
                                  the iteration limit stops the loop (fixed-count mode, A9)    */
-    GSR_OPT_DETERMINISTIC = 2, /* 1: aprod2 uses no floating-point atomics (bit-reproducible);
-                                 reserved: any value but 0 returns GSR_EUNSUPPORTED           */
+    GSR_OPT_DETERMINISTIC = 2, /* 1: gsr_lsqr_solve uses no floating-point atomics: every sum that
+                                 leaves a warp (astrometric runs, attitude windows, global column,
+                                 instrumental accumulators) is added to t = A^T u_hat as a 64-bit
+                                 fixed-point integer, so two solves on the same handle give
+                                 bit-identical x, norms and standard errors (the paper names its
+                                 atomics as a weakness).  Needs a preconditioned
+                                 matrix (the range of the sums rests on unit column norms), the
+                                 fused iteration, no constraint rows, no communicator, no damping:
+                                 otherwise gsr_lsqr_solve returns GSR_EUNSUPPORTED; GSR_ERANGE if a
+                                 pass exceeded its range (norm of u_hat grew more than 128-fold
+                                 beyond every earlier alpha and beta).  Each partial sum is rounded
+                                 once to 2^-54 of that range.  gsr_aprod2 and gsr_precondition keep
+                                 their fp64 atomics.  0 (default): fp64 atomics               */
     GSR_OPT_FUSED = 3,        /* 1 (default): one LSQR iteration reads the matrix ONCE -- u_hat =
                                  A v - (alpha/beta) u_hat and A^T u_hat are formed in the same
                                  pass, v = A^T u_hat / beta - beta v afterwards (same recurrences,
@@ -217,11 +229,28 @@ int gsr_debug_expand_rows(const gsr_matrix* A, int64_t row0, int64_t nrows, int6
  * Scratch vectors inside the handle are used; results are discarded.  Synchronous. */
 int gsr_time_product(gsr_matrix* A, int which, int reps, float* ms_avg, gsr_stream stream);
 
+/* One pass of the solver's fused iteration kernels (k_fused + its instrumental pass, with the
+ * handle's GSR_OPT_FIXED_POINT setting) on CALLER-ordered vectors, so that exactly the kernels
+ * of the timed loop can be compared with the oracle's two products at any size:
+ *     y <- A x + ca * y      (Algorithm 1; y_dev[m] in/out, caller row order)
+ *     t <- t + A^T y_new     (Algorithm 2; t_dev[n] in/out)
+ * x_dev[n], y_dev[m], t_dev[n] are device arrays owned by the caller.  Uses (and overwrites) the
+ * handle's LSQR work vectors: a previous solve's standard errors are lost.  Not available with
+ * constraint rows or a communicator (GSR_EUNSUPPORTED).  Asynchronous on `stream`. */
+int gsr_debug_fused_pass(gsr_matrix* A, const double* x_dev, double ca, double* y_dev,
+                         double* t_dev, gsr_stream stream);
+
 /* Device time (ms, CUDA events on the solve's stream) of the ITERATION LOOP of the last
  * gsr_lsqr_solve on this handle: from the first iteration's first kernel to the last iteration's
  * last one, without the initialisation (row a2) and the finalisation (row a12).  -1 before any
  * solve.  bench.py times "exactly K steps" with it. */
 double gsr_lsqr_last_loop_ms(const gsr_matrix* A);
+
+/* Number of iteration graphs captured on this handle so far.  Everything that is decided at
+ * capture time (iteration form, instrumental-pass variant, deterministic mode, constraint rows,
+ * communicator) is part of the graph's cache key; tests use this to check that changing such an
+ * option between two solves really re-captures. */
+int64_t gsr_debug_graph_builds(const gsr_matrix* A);
 
 /* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */
 int64_t gsr_launch_count(void);

@@ -27,6 +27,13 @@
  * augmented matrix (tests/test_constraints.py).
  * Standard errors (row f1): Paige & Saunders' var_j = sum_k (w_j/rho_k)^2, pinned by
  * diag((A^T A)^-1) on tiny systems run to finite termination.
+ * Timing-only OpenMP build (-DORC_OPENMP -fopenmp -> libgsr_oracle_omp.so): the same file with
+ * the paper's own CPU scheme: aprod1 as a `parallel for` over rows; aprod2 with
+ * one contiguous, star-aligned row range per thread, the astrometric columns owned by the range
+ * and thread-private accumulators for the replicated attitude + instrumental + global slice,
+ * combined in thread order.  Used by bench.py's all-core cpu_baseline and by the full-size
+ * parity legs; tests/test_oracle_omp.py checks it against the serial build (1e-13).  The
+ * serial build is the definition.
  * parity unpinned: the authors' own "modified" LSQR and their variance formula, covariances,
  * constraints (PAPER.md:27, 65, 67 give no formula) -- covariances / constraints not implemented.
  */
@@ -34,6 +41,18 @@
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
+#ifdef ORC_OPENMP
+#include <omp.h>
+#endif
+
+/* threads the build uses (1: the serial definition) */
+int orc_threads(void) {
+#ifdef ORC_OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
 
 #define N_ASTRO 5
 #define N_AXES 3
@@ -129,6 +148,9 @@ void orc_expand_rows(const orc_dims* d, const int32_t* star_idx, const int32_t* 
 void orc_aprod1(const orc_dims* d, const int32_t* star_idx, const int32_t* att_start,
                 const int32_t* instr_col, const double* A_d, const double* x, double* b,
                 double* scale) {
+#ifdef ORC_OPENMP
+#pragma omp parallel for schedule(static)
+#endif
     for (int64_t i = 0; i < d->n_rows; ++i) {
         double sum = 0.0, asum = 0.0;
         const int64_t k0 = i * N_PAR;
@@ -165,6 +187,48 @@ void orc_aprod2(const orc_dims* d, const int32_t* star_idx, const int32_t* att_s
         acc[j] = x[j];
         if (aacc) aacc[j] = fabs(x[j]);
     }
+#ifdef ORC_OPENMP
+    {   /* timing build: star-aligned row range per thread */
+        const int nt = omp_get_max_threads();
+        const int64_t n_astro = N_ASTRO * d->n_stars, n_rep = n - n_astro;
+        int64_t* lo = (int64_t*)malloc(sizeof(int64_t) * (size_t)(nt + 1));
+        for (int t = 0; t <= nt; ++t) {
+            int64_t r = d->n_rows * t / nt;
+            while (r > 0 && r < d->n_rows && star_idx[r] == star_idx[r - 1]) ++r;
+            lo[t] = r;
+        }
+        long double* priv = (long double*)calloc((size_t)(nt * n_rep), sizeof(long double));
+        long double* apriv = aacc ? (long double*)calloc((size_t)(nt * n_rep), sizeof(long double)) : NULL;
+#pragma omp parallel num_threads(nt)
+        {
+            const int t = omp_get_thread_num();
+            long double* pr = priv + (size_t)t * n_rep;
+            long double* apr = apriv ? apriv + (size_t)t * n_rep : NULL;
+            for (int64_t i = lo[t]; i < lo[t + 1]; ++i) {
+                const int64_t k0 = i * N_PAR;
+                for (int k = 0; k < N_PAR; ++k) {
+                    int64_t c = col_of(d, star_idx, att_start, instr_col, i, k);
+                    double tt = A_d[k0 + k] * b[i];
+                    if (c < n_astro) {          /* owned by this range: rows are star-aligned */
+                        acc[c] += tt;
+                        if (aacc) aacc[c] += fabs(tt);
+                    } else {
+                        pr[c - n_astro] += tt;
+                        if (apr) apr[c - n_astro] += fabs(tt);
+                    }
+                }
+            }
+        }
+        for (int t = 0; t < nt; ++t)            /* replicated slice, combined in thread order */
+            for (int64_t j = 0; j < n_rep; ++j) {
+                acc[n_astro + j] += priv[(size_t)t * n_rep + j];
+                if (aacc) aacc[n_astro + j] += apriv[(size_t)t * n_rep + j];
+            }
+        free(lo);
+        free(priv);
+        free(apriv);
+    }
+#else
     for (int64_t i = 0; i < d->n_rows; ++i) {
         const int64_t k0 = i * N_PAR;
         for (int k = 0; k < N_PAR; ++k) {
@@ -174,6 +238,7 @@ void orc_aprod2(const orc_dims* d, const int32_t* star_idx, const int32_t* att_s
             if (aacc) aacc[c] += fabs(t);
         }
     }
+#endif
     for (int64_t r = 0; r < g_con.n_con; ++r) /* constraints computation */
         for (int64_t e = g_con.row_ptr[r]; e < g_con.row_ptr[r + 1]; ++e) {
             double t = g_con.val[e] * b[d->n_rows + r];
@@ -193,11 +258,41 @@ void orc_colsumsq(const orc_dims* d, const int32_t* star_idx, const int32_t* att
                   const int32_t* instr_col, const double* A_d, double* q) {
     const int64_t n = n_cols(d);
     long double* acc = (long double*)calloc((size_t)n, sizeof(long double));
+#ifdef ORC_OPENMP
+    {   /* timing build: same partition as orc_aprod2 */
+        const int nt = omp_get_max_threads();
+        const int64_t n_astro = N_ASTRO * d->n_stars, n_rep = n - n_astro;
+        int64_t* lo = (int64_t*)malloc(sizeof(int64_t) * (size_t)(nt + 1));
+        for (int t = 0; t <= nt; ++t) {
+            int64_t r = d->n_rows * t / nt;
+            while (r > 0 && r < d->n_rows && star_idx[r] == star_idx[r - 1]) ++r;
+            lo[t] = r;
+        }
+        long double* priv = (long double*)calloc((size_t)(nt * n_rep), sizeof(long double));
+#pragma omp parallel num_threads(nt)
+        {
+            const int t = omp_get_thread_num();
+            long double* pr = priv + (size_t)t * n_rep;
+            for (int64_t i = lo[t]; i < lo[t + 1]; ++i)
+                for (int k = 0; k < N_PAR; ++k) {
+                    double a = A_d[i * N_PAR + k];
+                    int64_t c = col_of(d, star_idx, att_start, instr_col, i, k);
+                    if (c < n_astro) acc[c] += (long double)a * a;
+                    else pr[c - n_astro] += (long double)a * a;
+                }
+        }
+        for (int t = 0; t < nt; ++t)
+            for (int64_t j = 0; j < n_rep; ++j) acc[n_astro + j] += priv[(size_t)t * n_rep + j];
+        free(lo);
+        free(priv);
+    }
+#else
     for (int64_t i = 0; i < d->n_rows; ++i)
         for (int k = 0; k < N_PAR; ++k) {
             double a = A_d[i * N_PAR + k];
             acc[col_of(d, star_idx, att_start, instr_col, i, k)] += (long double)a * a;
         }
+#endif
     for (int64_t e = 0; g_con.n_con > 0 && e < g_con.row_ptr[g_con.n_con]; ++e)
         acc[g_con.col[e]] += (long double)g_con.val[e] * g_con.val[e];
     for (int64_t j = 0; j < n; ++j) q[j] = (double)acc[j];
@@ -211,6 +306,9 @@ void orc_precondition(const orc_dims* d, const int32_t* star_idx, const int32_t*
     const int64_t n = n_cols(d);
     orc_colsumsq(d, star_idx, att_start, instr_col, A_d, p);
     for (int64_t j = 0; j < n; ++j) p[j] = p[j] > 0.0 ? 1.0 / sqrt(p[j]) : 1.0;
+#ifdef ORC_OPENMP
+#pragma omp parallel for schedule(static)
+#endif
     for (int64_t i = 0; i < d->n_rows; ++i)
         for (int k = 0; k < N_PAR; ++k)
             A_d[i * N_PAR + k] = A_d[i * N_PAR + k] * p[col_of(d, star_idx, att_start, instr_col, i, k)];
@@ -218,17 +316,30 @@ void orc_precondition(const orc_dims* d, const int32_t* star_idx, const int32_t*
         g_con.val[e] = g_con.val[e] * p[g_con.col[e]];
 }
 
-static double nrm2(const double* v, int64_t len) {
-    long double s = 0.0L;
-    for (int64_t j = 0; j < len; ++j) s += (long double)v[j] * v[j];
-    return (double)sqrtl(s);
-}
 static double sumsq(const double* v, int64_t len) {
     long double s = 0.0L;
+#ifdef ORC_OPENMP
+#pragma omp parallel for schedule(static) reduction(+ : s)
+#endif
     for (int64_t j = 0; j < len; ++j) s += (long double)v[j] * v[j];
     return (double)s;
 }
+static double nrm2(const double* v, int64_t len) {
+    long double s = 0.0L;
+#ifdef ORC_OPENMP
+#pragma omp parallel for schedule(static) reduction(+ : s)
+#endif
+    for (int64_t j = 0; j < len; ++j) s += (long double)v[j] * v[j];
+    return (double)sqrtl(s);
+}
 static double hyp(double a, double b) { return sqrt(a * a + b * b); } /* reading A15 */
+/* v[i] = c * v[i] or v[i] / c, element-wise (same rounding in both builds) */
+static void scal(double* v, int64_t len, double c, int divide) {
+#ifdef ORC_OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int64_t i = 0; i < len; ++i) v[i] = divide ? v[i] / c : c * v[i];
+}
 
 /* Damping (row f4; Paige & Saunders 1982, section 2 of the algorithm paper): with damp > 0 LSQR
  * minimises || [A; damp I] x - [b; 0] ||.  The paper does not use it (damp = 0, the default);
@@ -267,7 +378,7 @@ int orc_lsqr_var(const orc_dims* d, const int32_t* star_idx, const int32_t* att_
     bnorm = beta;
     res->bnorm = bnorm;
     if (beta == 0.0) goto done_trivial; /* x = 0 is the exact solution: istop 0 */
-    for (int64_t i = 0; i < m; ++i) u[i] = u[i] / beta;
+    scal(u, m, beta, 1);
     /* "aprod 2 call (calculation of the initial solution)", Algorithm 3 line 6 */
     orc_aprod2(d, star_idx, att_start, instr_col, A_d, u, v, NULL);
     alpha = nrm2(v, n);
@@ -285,11 +396,11 @@ int orc_lsqr_var(const orc_dims* d, const int32_t* star_idx, const int32_t* att_
     while (1) {
         itn += 1;
         /* bidiagonalisation: u = A v - alpha u ; v = A^T u - beta v   (Alg. 3 lines 11, 15) */
-        for (int64_t i = 0; i < m; ++i) u[i] = -alpha * u[i];
+        scal(u, m, -alpha, 0);
         orc_aprod1(d, star_idx, att_start, instr_col, A_d, v, u, NULL);
         beta = nrm2(u, m);
         if (beta > 0.0) {
-            for (int64_t i = 0; i < m; ++i) u[i] = u[i] / beta;
+            scal(u, m, beta, 1);
             anorm = hyp(hyp(anorm, alpha), beta);
             if (damp > 0.0) anorm = hyp(anorm, damp);
             for (int64_t j = 0; j < n; ++j) v[j] = -beta * v[j];

@@ -17,16 +17,20 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "gsr_oracle.c")
 _LIB = os.path.join(_HERE, "libgsr_oracle.so")
+_LIB_OMP = os.path.join(_HERE, "libgsr_oracle_omp.so")
 
 
-def build(force: bool = False) -> str:
-    """Compile the oracle with gcc (no FMA contraction, reading A6)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        tmp = _LIB + f".tmp{os.getpid()}"
+def build(force: bool = False, omp: bool = False) -> str:
+    """Compile the oracle with gcc (no FMA contraction, reading A6).  omp=True: the timing-only
+    OpenMP build of the same file (-DORC_OPENMP, the paper's CPU scheme)."""
+    out = _LIB_OMP if omp else _LIB
+    if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(_SRC):
+        tmp = out + f".tmp{os.getpid()}"
+        extra = ["-fopenmp", "-DORC_OPENMP"] if omp else []
         subprocess.check_call(["gcc", "-O2", "-std=c99", "-ffp-contract=off", "-fPIC", "-shared",
-                               "-o", tmp, _SRC, "-lm"])
-        os.replace(tmp, _LIB)
-    return _LIB
+                               *extra, "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, out)
+    return out
 
 
 class _Dims(C.Structure):
@@ -59,17 +63,23 @@ class LsqrResult:
     se: np.ndarray | None = None       # standard errors of x (multiplied by p when scaled)
 
 
-_lib = None
+_libs = {}
 
 
-def lib():
-    global _lib
-    if _lib is None:
-        _lib = C.CDLL(build())
-        _lib.orc_validate.restype = C.c_int
-        _lib.orc_lsqr.restype = C.c_int
-        _lib.orc_lsqr_var.restype = C.c_int
-    return _lib
+def lib(omp: bool = False):
+    if omp not in _libs:
+        L = C.CDLL(build(omp=omp))
+        L.orc_validate.restype = C.c_int
+        L.orc_lsqr.restype = C.c_int
+        L.orc_lsqr_var.restype = C.c_int
+        L.orc_threads.restype = C.c_int
+        _libs[omp] = L
+    return _libs[omp]
+
+
+def omp_threads() -> int:
+    """Threads the OpenMP timing build uses (OMP_NUM_THREADS or all cores)."""
+    return int(lib(True).orc_threads())
 
 
 def _p(a, ct):
@@ -79,11 +89,14 @@ def _p(a, ct):
 class OracleSystem:
     """One system in caller form.  `values` is copied so precondition() can scale it."""
 
-    def __init__(self, n_stars, n_dfa, n_instr, star_idx, att_start, instr_col, values):
+    def __init__(self, n_stars, n_dfa, n_instr, star_idx, att_start, instr_col, values, omp=False,
+                 copy_values=True):
+        self.omp = bool(omp)   # route every call through the OpenMP timing build
         self.star_idx = np.ascontiguousarray(star_idx, dtype=np.int32)
         self.att_start = np.ascontiguousarray(att_start, dtype=np.int32)
         self.instr_col = np.ascontiguousarray(instr_col, dtype=np.int32).reshape(-1, 6)
-        self.values = np.array(values, dtype=np.float64, order="C", copy=True).reshape(-1, 24)
+        self.values = (np.array(values, dtype=np.float64, order="C", copy=True) if copy_values
+                       else np.ascontiguousarray(values, dtype=np.float64)).reshape(-1, 24)
         self.m = int(self.star_idx.shape[0])
         assert self.att_start.shape == (self.m,) and self.instr_col.shape == (self.m, 6)
         assert self.values.shape == (self.m, 24)
@@ -92,6 +105,9 @@ class OracleSystem:
         self.dims = _Dims(self.m, self.n_stars, self.n_dfa, self.n_instr)
         self.p = None
         self.n_con, self.con_ptr, self.con_col, self.con_val = 0, None, None, None
+
+    def _L(self):
+        return lib(self.omp)
 
     def set_constraints(self, row_ptr, col, val):
         """n_con extra rows in CSR form appended below the observations.
@@ -109,23 +125,23 @@ class OracleSystem:
 
     def _con(self, on=True):
         if self.n_con and on:
-            lib().orc_set_constraints(C.c_int64(self.n_con), _p(self.con_ptr, C.c_int64),
+            self._L().orc_set_constraints(C.c_int64(self.n_con), _p(self.con_ptr, C.c_int64),
                                       _p(self.con_col, C.c_int32), _p(self.con_val, C.c_double))
         else:
-            lib().orc_set_constraints(C.c_int64(0), None, None, None)
+            self._L().orc_set_constraints(C.c_int64(0), None, None, None)
 
     def _idx(self):
         return (C.byref(self.dims), _p(self.star_idx, C.c_int32), _p(self.att_start, C.c_int32),
                 _p(self.instr_col, C.c_int32))
 
     def validate(self) -> int:
-        return int(lib().orc_validate(*self._idx()))
+        return int(self._L().orc_validate(*self._idx()))
 
     def expand_rows(self, row0=0, nrows=None):
         nrows = self.m - row0 if nrows is None else nrows
         cols = np.empty((nrows, 24), dtype=np.int64)
         vals = np.empty((nrows, 24), dtype=np.float64)
-        lib().orc_expand_rows(*self._idx(), _p(self.values, C.c_double), C.c_int64(row0),
+        self._L().orc_expand_rows(*self._idx(), _p(self.values, C.c_double), C.c_int64(row0),
                               C.c_int64(nrows), _p(cols, C.c_int64), _p(vals, C.c_double))
         return cols, vals
 
@@ -136,7 +152,7 @@ class OracleSystem:
         assert x.shape == (self.n,) and y.shape == (self.m_total,)
         sc = np.empty(self.m_total) if want_scale else None
         self._con()
-        lib().orc_aprod1(*self._idx(), _p(self.values, C.c_double), _p(x, C.c_double),
+        self._L().orc_aprod1(*self._idx(), _p(self.values, C.c_double), _p(x, C.c_double),
                          _p(y, C.c_double), _p(sc, C.c_double))
         self._con(False)
         return (y, sc) if want_scale else y
@@ -148,7 +164,7 @@ class OracleSystem:
         assert x.shape == (self.n,) and y.shape == (self.m_total,)
         sc = np.empty(self.n) if want_scale else None
         self._con()
-        lib().orc_aprod2(*self._idx(), _p(self.values, C.c_double), _p(y, C.c_double),
+        self._L().orc_aprod2(*self._idx(), _p(self.values, C.c_double), _p(y, C.c_double),
                          _p(x, C.c_double), _p(sc, C.c_double))
         self._con(False)
         return (x, sc) if want_scale else x
@@ -156,7 +172,7 @@ class OracleSystem:
     def colsumsq(self):
         q = np.empty(self.n)
         self._con()
-        lib().orc_colsumsq(*self._idx(), _p(self.values, C.c_double), _p(q, C.c_double))
+        self._L().orc_colsumsq(*self._idx(), _p(self.values, C.c_double), _p(q, C.c_double))
         self._con(False)
         return q
 
@@ -165,7 +181,7 @@ class OracleSystem:
         assert self.p is None, "already preconditioned"
         p = np.empty(self.n)
         self._con()
-        lib().orc_precondition(*self._idx(), _p(self.values, C.c_double), _p(p, C.c_double))
+        self._L().orc_precondition(*self._idx(), _p(self.values, C.c_double), _p(p, C.c_double))
         self._con(False)
         self.p = p
         return p
@@ -180,29 +196,29 @@ class OracleSystem:
         hist = np.zeros((int(itnlim), 7)) if want_hist else None
         var = np.zeros(self.n) if want_se else None
         self._con()
-        lib().orc_set_damp(C.c_double(damp))
-        rc = lib().orc_lsqr_var(*self._idx(), _p(self.values, C.c_double), _p(b, C.c_double),
+        self._L().orc_set_damp(C.c_double(damp))
+        rc = self._L().orc_lsqr_var(*self._idx(), _p(self.values, C.c_double), _p(b, C.c_double),
                                 _p(x, C.c_double), C.c_int64(itnlim), C.c_double(atol),
                                 C.c_double(btol), C.c_double(conlim),
                                 C.c_int(1 if force_itnlim else 0), C.byref(res),
                                 _p(hist, C.c_double), _p(var, C.c_double))
         self._con(False)
-        lib().orc_set_damp(C.c_double(0.0))
+        self._L().orc_set_damp(C.c_double(0.0))
         assert rc == 0
         se = None
         if want_se:
             se = np.empty(self.n)
-            lib().orc_standard_errors(C.c_int64(self.m_total), C.c_int64(self.n), C.c_double(res.rnorm),
+            self._L().orc_standard_errors(C.c_int64(self.m_total), C.c_int64(self.n), C.c_double(res.rnorm),
                                       _p(var, C.c_double), _p(self.p, C.c_double), _p(se, C.c_double))
         if self.p is not None:
-            lib().orc_unscale(C.c_int64(self.n), _p(self.p, C.c_double), _p(x, C.c_double))
+            self._L().orc_unscale(C.c_int64(self.n), _p(self.p, C.c_double), _p(x, C.c_double))
         if hist is not None:
             hist = hist[:res.itn]
         return LsqrResult(x, res.istop, res.itn, res.istop_natural, res.itn_natural, res.rnorm,
                           res.arnorm, res.anorm, res.acond, res.xnorm, res.bnorm, hist, var, se)
 
 
-def from_torch(cfg, star, att, instr, vals) -> OracleSystem:
+def from_torch(cfg, star, att, instr, vals, omp=False) -> OracleSystem:
     """Build from the tensors of the shared input generator (host copies)."""
     return OracleSystem(cfg.n_stars, cfg.n_dfa, cfg.n_instr, star.cpu().numpy(), att.cpu().numpy(),
-                        instr.cpu().numpy(), vals.cpu().numpy())
+                        instr.cpu().numpy(), vals.cpu().numpy(), omp=omp)

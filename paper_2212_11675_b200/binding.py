@@ -13,7 +13,7 @@ from dataclasses import dataclass
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgsr_b200.so")
 
-GSR_OK, GSR_EINVAL, GSR_ENOMEM, GSR_ECUDA, GSR_ESTATE, GSR_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
+GSR_OK, GSR_EINVAL, GSR_ENOMEM, GSR_ECUDA, GSR_ESTATE, GSR_EUNSUPPORTED, GSR_ERANGE = 0, -1, -2, -3, -4, -5, -6
 GSR_OPT_FORCE_ITNLIM, GSR_OPT_DETERMINISTIC, GSR_OPT_FUSED, GSR_OPT_FIXED_POINT = 1, 2, 3, 4
 
 EXPORTS = [
@@ -21,14 +21,16 @@ EXPORTS = [
     "gsr_matrix_destroy", "gsr_matrix_dims", "gsr_matrix_device_bytes", "gsr_aprod1",
     "gsr_aprod2", "gsr_precondition", "gsr_lsqr_solve", "gsr_set_option", "gsr_strerror",
     "gsr_debug_expand_rows", "gsr_time_product", "gsr_launch_count", "gsr_lsqr_standard_errors", "gsr_lsqr_last_loop_ms", "gsr_lsqr_set_damp",
-    "gsr_matrix_set_constraints", "gsr_comm_unique_id", "gsr_comm_create", "gsr_comm_destroy", "gsr_matrix_set_comm",
+    "gsr_debug_fused_pass", "gsr_debug_graph_builds", "gsr_matrix_set_constraints", "gsr_comm_unique_id", "gsr_comm_create", "gsr_comm_destroy", "gsr_matrix_set_comm",
 ]
 
 
 class GsrError(RuntimeError):
     def __init__(self, code: int, what: str):
         self.code = code
-        super().__init__(f"{what}: {strerror(code)} ({code})")
+        # no strerror() lookup when the library itself is what is missing (it would recurse)
+        msg = strerror(code) if _lib is not None else "libgsr_b200.so not loaded"
+        super().__init__(f"{what}: {msg} ({code})")
 
 
 class gsr_dims(C.Structure):
@@ -98,6 +100,9 @@ def lib():
         L.gsr_time_product.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_float), vp]
         L.gsr_launch_count.argtypes = []
         L.gsr_launch_count.restype = i64
+        L.gsr_debug_fused_pass.argtypes = [vp, vp, dbl, vp, vp, vp]
+        L.gsr_debug_graph_builds.argtypes = [vp]
+        L.gsr_debug_graph_builds.restype = i64
         _lib = L
     return _lib
 
@@ -260,6 +265,16 @@ def gsr_time_product(h, which, reps, stream=None) -> float:
     _check(lib().gsr_time_product(h, int(which), int(reps), C.byref(ms), _stream(stream)),
            "gsr_time_product")
     return float(ms.value)
+
+
+def gsr_debug_fused_pass(h, x_dev, ca, y_dev, t_dev, stream=None):
+    """y <- A x + ca y ; t += A^T y_new through the solver's fused kernels (caller row order)."""
+    _check(lib().gsr_debug_fused_pass(h, _ptr(x_dev), float(ca), _ptr(y_dev), _ptr(t_dev),
+                                      _stream(stream)), "gsr_debug_fused_pass")
+
+
+def gsr_debug_graph_builds(h) -> int:
+    return int(lib().gsr_debug_graph_builds(h))
 
 
 def gsr_launch_count() -> int:

@@ -238,10 +238,29 @@ __device__ __forceinline__ void att_mode2_tile(RegsA& ra, const double* ysm, dou
     }
 }
 
+// GSR_OPT_DETERMINISTIC: every sum that leaves a warp goes to global memory as a 64-bit fixed-
+// point integer (native L2 integer atomics: integer addition is associative, so the result does
+// not depend on the order in which warps arrive).  On a column-scaled matrix every partial sum
+// of column j is bounded by sum_i |A_ij| |u_i| <= ||A_j|| ||u|| = ||u||; with 2^e >= ||u|| the
+// scale 2^(61-e) keeps it below 2^62.  What a warp adds is itself deterministic: a unit's rows
+// are processed in a fixed order by one warp.
+template <bool DET>
+__device__ __forceinline__ void add_out(double* addr, double v, double dscale) {
+    if (DET) atomicAdd((unsigned long long*)addr, (unsigned long long)__double2ll_rn(v * dscale));
+    else atomicAdd(addr, v);
+}
+// exponent e with 2^e > sqrt(ss) (the norm of the vector whose A^T product is accumulated)
+__device__ __forceinline__ int fixed_exp(double ss) {
+    const double ynorm = sqrt(ss);
+    int e = ynorm > 0.0 ? ilogb(ynorm) + 1 : 0;
+    return e < -900 ? -900 : e;   // keeps 2^(61-e) finite for a vanishing vector
+}
+
 // astrometric part of aprod2 for one tile: segmented reduction over the
 // star-sorted home lanes, one global atomic per (tile, star, coefficient).  vs[k] = A[l,k]*y[l].
+template <bool DET>
 __device__ __forceinline__ void astro_mode2(double (&vs)[5], int32_t s, int lane, double* __restrict__ x,
-                                            int64_t S) {
+                                            int64_t S, double dscale) {
     GSR_ASSERT(s >= 0 && s < S);
     const int32_t s_up = __shfl_up_sync(0xffffffffu, s, 1);
     const bool head = lane == 0 || s_up != s;
@@ -250,7 +269,7 @@ __device__ __forceinline__ void astro_mode2(double (&vs)[5], int32_t s, int lane
 #pragma unroll
         for (int k = 0; k < 5; ++k) {
             const double tsum = warp_sum(vs[k]);
-            if (lane == 0 && tsum != 0.0) atomicAdd(x + 5 * (int64_t)s + k, tsum);
+            if (lane == 0 && tsum != 0.0) add_out<DET>(x + 5 * (int64_t)s + k, tsum, dscale);
         }
     } else {
         // segmented inclusive scan; the last lane of each segment holds its sum.  A step of
@@ -274,7 +293,7 @@ __device__ __forceinline__ void astro_mode2(double (&vs)[5], int32_t s, int lane
         }
 #pragma unroll
         for (int k = 0; k < 5; ++k)
-            if (tail && vs[k] != 0.0) atomicAdd(x + 5 * (int64_t)s + k, vs[k]);
+            if (tail && vs[k] != 0.0) add_out<DET>(x + 5 * (int64_t)s + k, vs[k], dscale);
     }
 }
 
@@ -445,7 +464,7 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
             __syncwarp();
             // global
             g += SQUARE ? r.gl * r.gl : r.gl * yv;
-            astro_mode2(r.as, r.s, lane, x, S);
+            astro_mode2<false>(r.as, r.s, lane, x, S, 1.0);
         }
         // flush the unit's window
         __syncwarp();
@@ -475,6 +494,9 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
 // The instrumental block of A^T u_hat (a7) is left to k_aprod2_instr, because its CTA-shared
 // accumulator (I doubles) does not fit in shared memory beside x's instrumental block and the
 // two attitude windows per warp at I = 10 000.
+// DET (GSR_OPT_DETERMINISTIC): t is accumulated as 64-bit fixed-point integers with the scale
+// 2^(61 - *det_e) (see add_out), the global column once per unit instead of once per warp.
+template <bool DET>
 __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__ tiles,
                                               const Unit* __restrict__ units, int n_units,
                                               int* __restrict__ counter,
@@ -482,8 +504,9 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
                                               const double* __restrict__ ca_p,
                                               double* __restrict__ partials, double* __restrict__ tacc,
                                               int64_t S, int64_t D, int I, int win, int ws,
-                                              const int* __restrict__ stop) {
+                                              const int* __restrict__ stop, const int* __restrict__ det_e) {
     if (stop && *stop) return;
+    const double dscale = DET ? scalbn(1.0, 61 - *det_e) : 1.0;
     extern __shared__ double sm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double* xi = sm;
@@ -565,7 +588,7 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
             g = fma(r.gl, yv, g);
 #pragma unroll
             for (int k = 0; k < 5; ++k) r.as[k] *= yv;
-            astro_mode2(r.as, r.s, lane, tacc, S);
+            astro_mode2<DET>(r.as, r.s, lane, tacc, S, dscale);
         }
         q = warp_sum(q);
         if (lane == 0) partials[u] = q;
@@ -573,11 +596,18 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
         for (int i = lane; i < 3 * win; i += 32) {
             const int ax = i / win, k = i - ax * win;
             const double vacc = tw[ax * ws + k];
-            if (vacc != 0.0 && un.a0 + k < D) atomicAdd(tatt + ax * D + un.a0 + k, vacc);
+            if (vacc != 0.0 && un.a0 + k < D) add_out<DET>(tatt + ax * D + un.a0 + k, vacc, dscale);
+        }
+        if (DET) {   // the unit -> warp assignment is dynamic: one sum per unit, not per warp
+            g = warp_sum(g);
+            if (lane == 0 && g != 0.0) add_out<true>(tacc + 5 * S + 3 * D + I, g, dscale);
+            g = 0.0;
         }
     }
-    g = warp_sum(g);
-    if (lane == 0 && g != 0.0) atomicAdd(tacc + 5 * S + 3 * D + I, g);
+    if (!DET) {
+        g = warp_sum(g);
+        if (lane == 0 && g != 0.0) atomicAdd(tacc + 5 * S + 3 * D + I, g);
+    }
 }
 
 // Instrumental block of A^T u (row a7) over the instrumental planes only (1920 B per tile):
@@ -595,22 +625,19 @@ __global__ void __launch_bounds__(TPB) k_fused(const unsigned char* __restrict__
 //   multiple of 2^(e-61): an absolute error <= n_j 2^(e-62) per column, i.e. normwise
 //   ~1e-18 ||y|| per term (fp64 atomics are componentwise accurate instead; LSQR only needs
 //   the normwise bound).  ss_p points to sum y_i^2 over the rows of this launch (device).
+// det (FIXED only): leave the integer totals in xins (64-bit integer atomics, scale 2^(61-e)
+// with e = fixed_exp(*ss_p)); k_det_finish converts the vector afterwards.
 template <bool FIXED>
 __global__ void __launch_bounds__(TPB) k_aprod2_instr(const unsigned char* __restrict__ tiles,
                                                      int64_t n_tiles, const double* __restrict__ y,
                                                      double* __restrict__ xins, int I, int ncopy,
                                                      const double* __restrict__ ss_p,
-                                                     const int* __restrict__ stop) {
+                                                     const int* __restrict__ stop, int det) {
     if (stop && *stop) return;
     extern __shared__ double sm[];
     const int ipad = (I + 1) & ~1;
     for (int i = threadIdx.x; i < ipad * ncopy; i += TPB) sm[i] = 0.0;   // +0.0 = integer 0
-    int e = 0;
-    if (FIXED) {
-        const double ynorm = sqrt(*ss_p);
-        e = ynorm > 0.0 ? ilogb(ynorm) + 1 : 0;   // 2^e > ||y||
-        if (e < -900) e = -900;                   // keeps 2^(61-e) finite for a vanishing y
-    }
+    const int e = FIXED ? fixed_exp(*ss_p) : 0;   // 2^e > ||y||
     const double scale = FIXED ? scalbn(1.0, 61 - e) : 1.0;
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -651,12 +678,30 @@ __global__ void __launch_bounds__(TPB) k_aprod2_instr(const unsigned char* __res
         if (FIXED) {
             long long tot = 0;
             for (int w = 0; w < ncopy; ++w) tot += ((const long long*)sm)[w * ipad + i];
+            if (det) {
+                if (tot != 0) atomicAdd((unsigned long long*)(xins + i), (unsigned long long)tot);
+                continue;
+            }
             vacc = (double)tot * unscale;
         } else {
             vacc = 0.0;
             for (int w = 0; w < ncopy; ++w) vacc += sm[w * ipad + i];
         }
         if (vacc != 0.0) atomicAdd(xins + i, vacc);
+    }
+}
+
+// GSR_OPT_DETERMINISTIC: t holds 64-bit fixed-point integers after k_fused<true> (scale
+// 2^(61 - *det_e)) and the deterministic instrumental pass (scale from *ss_p); back to doubles.
+__global__ void __launch_bounds__(256) k_det_finish(double* __restrict__ t, int64_t n, int64_t off_instr,
+                                                    int64_t I, const int* __restrict__ det_e,
+                                                    const double* __restrict__ ss_p,
+                                                    const int* __restrict__ stop) {
+    if (stop && *stop) return;
+    const double ua = scalbn(1.0, *det_e - 61), ub = scalbn(1.0, fixed_exp(*ss_p) - 61);
+    for (int64_t j = (int64_t)blockIdx.x * 256 + threadIdx.x; j < n; j += (int64_t)gridDim.x * 256) {
+        const long long q = ((const long long*)t)[j];
+        t[j] = (double)q * (j >= off_instr && j < off_instr + I ? ub : ua);
     }
 }
 
@@ -691,12 +736,13 @@ int configure_product_kernels(gsr_matrix* A) {
     GSR_TRY(set_smem(k_aprod2<false, false>, b));
     GSR_TRY(set_smem(k_aprod2<false, true>, b));
     GSR_TRY(set_smem(k_aprod2<true, false>, b));
-    GSR_TRY(set_smem(k_fused, A->smem_fused));
+    GSR_TRY(set_smem(k_fused<false>, A->smem_fused));
+    GSR_TRY(set_smem(k_fused<true>, A->smem_fused));
     GSR_TRY(set_smem(k_aprod2_instr<false>, (int)instr_smem(A)));
     GSR_TRY(set_smem(k_aprod2_instr<true>, (int)instr_smem(A)));
     {
         int nb = 1;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_fused, TPB, A->smem_fused) != cudaSuccess || nb < 1) {
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_fused<false>, TPB, A->smem_fused) != cudaSuccess || nb < 1) {
             cudaGetLastError();
             nb = 1;
         }
@@ -762,27 +808,41 @@ int launch_aprod2(const gsr_matrix* A, const double* y, double* x, const double*
 }
 
 int launch_fused(const gsr_matrix* A, const double* v, double* u, const double* ca,
-                 double* partials, double* t, const int* stop, cudaStream_t s) {
+                 double* partials, double* t, const int* stop, const int* det_e, cudaStream_t s) {
     if (A->n_units == 0) return GSR_OK;
     GSR_TRY(reset_counter(A, s));
-    k_fused<<<A->grid_fused, TPB, A->smem_fused, s>>>(A->tiles, A->units, A->n_units, A->unit_counter, v, u,
-                                                     ca, partials, t, A->dims.n_stars, A->dims.n_dfa,
-                                                     (int)A->dims.n_instr, A->win, A->wstride, stop);
+    if (det_e)
+        k_fused<true><<<A->grid_fused, TPB, A->smem_fused, s>>>(
+            A->tiles, A->units, A->n_units, A->unit_counter, v, u, ca, partials, t, A->dims.n_stars,
+            A->dims.n_dfa, (int)A->dims.n_instr, A->win, A->wstride, stop, det_e);
+    else
+        k_fused<false><<<A->grid_fused, TPB, A->smem_fused, s>>>(
+            A->tiles, A->units, A->n_units, A->unit_counter, v, u, ca, partials, t, A->dims.n_stars,
+            A->dims.n_dfa, (int)A->dims.n_instr, A->win, A->wstride, stop, nullptr);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;
 }
 
 int launch_aprod2_instr(const gsr_matrix* A, const double* u, double* t, const double* ss,
-                        const int* stop, cudaStream_t s) {
+                        const int* stop, int det, cudaStream_t s) {
     if (A->n_tiles == 0) return GSR_OK;
+    if (det && (A->p == nullptr || ss == nullptr)) return GSR_ESTATE;
     // exact fixed-point accumulation needs unit column norms (see k_aprod2_instr) and ||u||^2
-    if (A->p != nullptr && ss != nullptr && !A->opt_no_fixed)
+    if (A->p != nullptr && ss != nullptr && (!A->opt_no_fixed || det))
         k_aprod2_instr<true><<<A->grid_instr, TPB, instr_smem(A), s>>>(
-            A->tiles, A->n_tiles, u, t + A->off_instr, (int)A->dims.n_instr, instr_copies(A), ss, stop);
+            A->tiles, A->n_tiles, u, t + A->off_instr, (int)A->dims.n_instr, instr_copies(A), ss, stop, det);
     else
         k_aprod2_instr<false><<<A->grid_instr, TPB, instr_smem(A), s>>>(
-            A->tiles, A->n_tiles, u, t + A->off_instr, (int)A->dims.n_instr, instr_copies(A), nullptr, stop);
+            A->tiles, A->n_tiles, u, t + A->off_instr, (int)A->dims.n_instr, instr_copies(A), nullptr, stop, 0);
+    count_launch();
+    GSR_CUDA_TRY(cudaGetLastError());
+    return GSR_OK;
+}
+
+int launch_det_finish(const gsr_matrix* A, double* t, const int* det_e, const double* ss,
+                      const int* stop, cudaStream_t s) {
+    k_det_finish<<<592, 256, 0, s>>>(t, A->n_cols, A->off_instr, A->dims.n_instr, det_e, ss, stop);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;

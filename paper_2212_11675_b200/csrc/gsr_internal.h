@@ -122,6 +122,11 @@ struct LsqrState {
     double atol, btol, ctol;
     long long itn, itnlim, itn_nat;
     int istop, istop_nat, stop, force, beta_pos, pad_;
+    // GSR_OPT_DETERMINISTIC: exponent of the fixed-point scale of the NEXT fused pass (2^det_e
+    // must exceed the norm of the u_hat that pass produces), its rigorous cap from ||A||_F,
+    // the largest alpha / beta seen so far, and the flag raised when a pass exceeded its range
+    int det, det_e, det_cap, det_fail;
+    double det_max;
 };
 
 struct Workspace {
@@ -148,8 +153,10 @@ struct Workspace {
     cudaGraphExec_t graph = nullptr;
     cudaStream_t graph_stream = nullptr;
     bool graph_valid = false;
-    int graph_two_pass = 0;
+    int graph_key = 0;          // options frozen into the captured graph (build_graph)
+    int64_t graph_ncon = 0;
     void* graph_comm = nullptr;
+    int graph_builds = 0;       // graphs captured so far (gsr_debug_graph_builds)
 };
 
 }  // namespace gsr
@@ -192,6 +199,7 @@ struct gsr_matrix {
     int opt_force_itnlim;
     int opt_two_pass;               // 1: aprod1 + aprod2 per iteration instead of the fused pass
     int opt_no_fixed;               // 1: fp64 atomics in the instrumental pass even when scaled
+    int opt_deterministic;          // 1: no floating-point atomics anywhere in the iteration
     double damp;                    // gsr_lsqr_set_damp (row f4); 0 = the paper's undamped LSQR
     int64_t n_con, con_nnz;         // row f3: constraint rows (CSR) appended below the observations
     int64_t* con_ptr;
@@ -258,10 +266,14 @@ int launch_colsumsq(const gsr_matrix* A, double* q, cudaStream_t s);
 //   t[col] += A[i,k] * u_new[i]                  for the astrometric, attitude and global blocks
 // followed by the instrumental pass  t[off_instr + c] += A[i,17+j] * u[i]  over the
 // instrumental planes only.  t must hold zeros (or the value to accumulate onto) on entry.
+// det_e != nullptr (GSR_OPT_DETERMINISTIC): t is accumulated as 64-bit fixed-point integers
+// with the scale 2^(61 - *det_e); launch_det_finish turns it back into doubles.
 int launch_fused(const gsr_matrix* A, const double* v, double* u, const double* ca,
-                 double* partials, double* t, const int* stop, cudaStream_t s);
+                 double* partials, double* t, const int* stop, const int* det_e, cudaStream_t s);
 int launch_aprod2_instr(const gsr_matrix* A, const double* u, double* t, const double* ss,
-                        const int* stop, cudaStream_t s);   // ss: device sum of u^2 (or nullptr)
+                        const int* stop, int det, cudaStream_t s);   // ss: device sum of u^2 (or nullptr)
+int launch_det_finish(const gsr_matrix* A, double* t, const int* det_e, const double* ss,
+                      const int* stop, cudaStream_t s);
 int configure_product_kernels(gsr_matrix* A);
 
 }  // namespace gsr

@@ -80,6 +80,16 @@ __global__ void __launch_bounds__(TB_N) k_gather_sumsq(const double* __restrict_
     if (threadIdx.x == 0) part[blockIdx.x] = q;
 }
 
+// dst[perm[i]] = src[i]: an internal-order m-vector back to the caller's row order
+__global__ void __launch_bounds__(TB_N) k_scatter_rows(const double* __restrict__ src,
+                                                       const uint32_t* __restrict__ perm,
+                                                       double* __restrict__ dst, int64_t len_int) {
+    for (int64_t i = (int64_t)blockIdx.x * TB_N + threadIdx.x; i < len_int; i += (int64_t)gridDim.x * TB_N) {
+        const uint32_t pe = perm[i];
+        if (pe != PERM_PAD) dst[pe] = src[i];
+    }
+}
+
 __global__ void __launch_bounds__(TB_N) k_sumsq(const double* __restrict__ v, int64_t len,
                                                 double* __restrict__ part, const int* __restrict__ stop,
                                                 int64_t split, double* __restrict__ parta) {
@@ -204,6 +214,7 @@ __global__ void __launch_bounds__(1024) k_scalar_init1(LsqrState* __restrict__ s
         st->inv_beta = 0.0;
     } else {
         st->inv_beta = 1.0 / beta;
+        st->det_e = ilogb(beta) + 2;   // deterministic init pass: u_hat = b, ||u_hat|| = beta_1 < 2^det_e
     }
 }
 
@@ -229,6 +240,9 @@ __global__ void __launch_bounds__(1024) k_scalar_init2(LsqrState* __restrict__ s
     st->phibar = st->beta;
     st->arnorm = alpha * st->beta;
     st->ca = -alpha / st->beta;
+    // range of the first fused pass (deterministic mode): ||u_hat_1|| = beta_2 <= ||A||_2
+    st->det_max = alpha;
+    st->det_e = min(ilogb(alpha) + 8, st->det_cap);
 }
 
 // beta_{k+1} = ||A v_k - alpha_k u_k||, anorm update
@@ -241,6 +255,12 @@ __global__ void __launch_bounds__(1024) k_scalar_beta(LsqrState* __restrict__ st
     st->itn += 1;
     double beta = sqrt(ss);
     st->beta = beta;
+    if (st->det && !(beta < scalbn(1.0, st->det_e))) {   // the pass left its fixed-point range
+        st->det_fail = 1;
+        st->stop = 1;
+        return;
+    }
+    if (beta > st->det_max) st->det_max = beta;
     if (beta > 0.0) {
         st->beta_pos = 1;
         st->anorm = hyp(hyp(st->anorm, st->alpha), beta);   // uses the OLD alpha
@@ -340,6 +360,11 @@ __global__ void __launch_bounds__(1024) k_scalar_main(LsqrState* __restrict__ st
     st->istop = istop;
     // coefficient of the next aprod1: u_hat <- A v - (alpha/beta) u_hat
     st->ca = st->beta_pos ? -alpha / beta : 0.0;
+    // deterministic mode: range of the next fused pass.  beta_{k+2} <= ||A||_2, of which the
+    // largest alpha / beta seen so far is a close lower estimate: 2^7 of headroom above it,
+    // never more than the rigorous cap 2 ||A||_F; k_scalar_beta checks the range afterwards.
+    if (alpha > st->det_max) st->det_max = alpha;
+    st->det_e = st->det_max > 0.0 ? min(ilogb(st->det_max) + 8, st->det_cap) : st->det_cap;
     // The update kernel of THIS iteration must still run; it checks `stop` first, so the
     // flag is raised by k_raise_stop after it.
 }
@@ -394,7 +419,7 @@ void free_workspace(gsr_matrix* A) {
 // together, k_aprod2_instr adds the instrumental block of t, k_vnew forms v = t/beta - beta v.
 // Two-pass form (GSR_OPT_FUSED = 0): aprod1, then aprod2 on the pre-scaled v.
 static int kernels_per_iteration(const gsr_matrix* A) {
-    return (A->opt_two_pass ? 8 : (A->comm ? 10 : 8)) + (A->n_con > 0 ? 2 : 0);
+    return (A->opt_two_pass ? 8 : (A->comm ? 10 : 8)) + (A->n_con > 0 ? 2 : 0) + (A->opt_deterministic ? 1 : 0);
 }
 
 static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
@@ -415,12 +440,14 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
         k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N, nullptr);
         k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, nullptr, W.var, 0, nullptr);
     } else if (!A->comm) {
-        GSR_TRY(launch_fused(A, W.v, W.u, &W.st->ca, W.part_u, W.t, &W.st->stop, s));
+        const int det = A->opt_deterministic;
+        GSR_TRY(launch_fused(A, W.v, W.u, &W.st->ca, W.part_u, W.t, &W.st->stop, det ? &W.st->det_e : nullptr, s));
         // constraint rows (row f3): same two steps on the CSR block, u_hat[m_int ..]
         GSR_TRY(launch_con_aprod1(A, W.v, W.u + A->m_int, &W.st->ca, W.part_u + A->n_units, &W.st->stop, s));
         GSR_TRY(launch_con_aprod2(A, W.u + A->m_int, W.t, A->coef_one, &W.st->stop, s));
         k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units + ncp, W.red + 3, &W.st->stop);
-        GSR_TRY(launch_aprod2_instr(A, W.u, W.t, W.red + 3, &W.st->stop, s));
+        GSR_TRY(launch_aprod2_instr(A, W.u, W.t, W.red + 3, &W.st->stop, det, s));
+        if (det) GSR_TRY(launch_det_finish(A, W.t, &W.st->det_e, W.red + 3, &W.st->stop, s));
         k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.red + 3, 1);
         k_vnew<<<NB_N, TB_N, 0, s>>>(W.v, W.t, n, W.st, W.part_v, 0, nullptr);
         k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N, nullptr);
@@ -429,9 +456,9 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
         // row-sharded: the same sequence with the paper's two reductions (Alg. 3 lines 12, 16)
         // as NCCL all-reduces inside the graph.  #1: replicated slice of t = A^T u_hat, with the
         // local sum of u_hat^2 riding in t[n]; #2: the distributed parts of ||v||^2 and ||w||^2.
-        GSR_TRY(launch_fused(A, W.v, W.u, &W.st->ca, W.part_u, W.t, &W.st->stop, s));
+        GSR_TRY(launch_fused(A, W.v, W.u, &W.st->ca, W.part_u, W.t, &W.st->stop, nullptr, s));
         k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units, W.t + n, &W.st->stop);
-        GSR_TRY(launch_aprod2_instr(A, W.u, W.t, W.t + n, &W.st->stop, s));   // local ||u_hat||^2
+        GSR_TRY(launch_aprod2_instr(A, W.u, W.t, W.t + n, &W.st->stop, 0, s));   // local ||u_hat||^2
         GSR_TRY(comm_allreduce_sum(A->comm, W.t + split, (size_t)(n - split + 1), s));
         k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.t + n, 1);
         k_vnew<<<NB_N, TB_N, 0, s>>>(W.v, W.t, n, W.st, W.part_v, split, W.part_va);
@@ -448,7 +475,13 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
 
 static int build_graph(gsr_matrix* A, cudaStream_t s) {
     Workspace& W = A->ws;
-    if (W.graph_valid && W.graph_stream == s && W.graph_two_pass == A->opt_two_pass && W.graph_comm == (void*)A->comm)
+    // everything enqueue_iteration() decides at capture time is part of the key: the iteration
+    // form, the communicator, the constraint rows, and the variant of the instrumental pass
+    // (fixed point needs a scaled matrix and GSR_OPT_FIXED_POINT)
+    const int key = (A->opt_two_pass ? 1 : 0) | (A->p != nullptr ? 2 : 0) | (A->opt_no_fixed ? 4 : 0) |
+                    (A->n_con > 0 ? 8 : 0) | (A->opt_deterministic ? 16 : 0);
+    if (W.graph_valid && W.graph_stream == s && W.graph_key == key && W.graph_comm == (void*)A->comm &&
+        W.graph_ncon == A->n_con)
         return GSR_OK;
     if (W.graph) {
         cudaGraphExecDestroy(W.graph);
@@ -484,8 +517,10 @@ static int build_graph(gsr_matrix* A, cudaStream_t s) {
     }
     W.graph_valid = true;
     W.graph_stream = s;
-    W.graph_two_pass = A->opt_two_pass;
+    W.graph_key = key;
+    W.graph_ncon = A->n_con;
     W.graph_comm = (void*)A->comm;
+    W.graph_builds += 1;
     return GSR_OK;
 }
 
@@ -505,6 +540,10 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     const int64_t m = A->dims.n_rows + A->n_con, n = A->n_cols;   // b: observations then constraints
     memset(result, 0, sizeof(*result));
     if (A->comm && A->n_con > 0) return GSR_EUNSUPPORTED;
+    // deterministic mode: fused iteration on a column-scaled matrix (the range bound of its
+    // fixed-point sums needs unit column norms), no constraint rows, one GPU
+    if (A->opt_deterministic && (!A->p || A->opt_two_pass || A->comm || A->n_con > 0 || A->damp > 0.0))
+        return GSR_EUNSUPPORTED;
 
     // b -> device
     const double* b_dev = b_hd;
@@ -524,6 +563,8 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     h.force = A->opt_force_itnlim;
     h.damp = A->damp;
     h.inv_alpha = 1.0;
+    h.det = A->opt_deterministic;
+    h.det_cap = ilogb(2.0 * sqrt((double)n)) + 1;   // ||A'||_2 <= ||A'||_F <= sqrt(n): unit columns
     GSR_CUDA_TRY(cudaMemcpyAsync(W.st, &h, sizeof(h), cudaMemcpyHostToDevice, s));
     GSR_CUDA_TRY(cudaMemsetAsync(W.v, 0, (size_t)n * 8, s));
     GSR_CUDA_TRY(cudaMemsetAsync(W.x, 0, (size_t)n * 8, s));
@@ -544,6 +585,17 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
         k_scalar_init1<<<1, 1024, 0, s>>>(W.st, W.part_u, NB_N + (A->n_con > 0 ? 1 : 0));
     }
     count_launch(2);
+    if (A->opt_deterministic) {
+        // v = A^T u_hat / beta_1 through the fused kernels: with v = 0 and ca = 1 the pass leaves
+        // u_hat = b as it is and accumulates t = A^T b in fixed point (range: ||b|| = beta_1)
+        GSR_CUDA_TRY(cudaMemsetAsync(W.t, 0, (size_t)n * 8, s));
+        GSR_TRY(launch_fused(A, W.v, W.u, A->coef_one, W.part_u, W.t, &W.st->stop, &W.st->det_e, s));
+        k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units, W.red + 3, &W.st->stop);
+        GSR_TRY(launch_aprod2_instr(A, W.u, W.t, W.red + 3, &W.st->stop, 1, s));
+        GSR_TRY(launch_det_finish(A, W.t, &W.st->det_e, W.red + 3, &W.st->stop, s));
+        k_vnew<<<NB_N, TB_N, 0, s>>>(W.v, W.t, n, W.st, W.part_v, 0, nullptr);   // v = t / beta_1
+        count_launch(2);
+    } else {
     GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s));
     GSR_TRY(launch_con_aprod2(A, W.u + A->m_int, W.v, &W.st->inv_beta, &W.st->stop, s));
     if (A->comm)     // replicated slice of v = A^T u: sum of the shards' contributions
@@ -553,6 +605,7 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
         k_sum_partials<<<1, 1024, 0, s>>>(W.part_va, NB_N, W.red, &W.st->stop);
         GSR_TRY(comm_allreduce_sum(A->comm, W.red, 1, s));
         count_launch();
+    }
     }
     k_scalar_init2<<<1, 1024, 0, s>>>(W.st, W.part_v, NB_N, A->comm ? W.red : nullptr);
     k_update<true><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, nullptr, nullptr, split, W.part_wa);
@@ -596,6 +649,7 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     if (!x_dev) GSR_CUDA_TRY(cudaMemcpyAsync(x_hd, xo, (size_t)n * 8, cudaMemcpyDeviceToHost, s));
     GSR_CUDA_TRY(cudaMemcpyAsync(&h, W.st, sizeof(h), cudaMemcpyDeviceToHost, s));
     GSR_CUDA_TRY(cudaStreamSynchronize(s));
+    if (h.det_fail) return GSR_ERANGE;
     result->istop = h.istop;
     result->istop_natural = h.istop_nat;
     result->itn = h.itn;
@@ -620,6 +674,8 @@ int gsr_lsqr_set_damp(gsr_matrix* A, double damp) {
     A->damp = damp;
     return GSR_OK;
 }
+
+int64_t gsr_debug_graph_builds(const gsr_matrix* A) { return A ? A->ws.graph_builds : 0; }
 
 double gsr_lsqr_last_loop_ms(const gsr_matrix* A) {
     return (A && A->ws.solved) ? A->ws.last_loop_ms : -1.0;
@@ -648,6 +704,29 @@ int gsr_lsqr_standard_errors(gsr_matrix* A, double* se_hd, gsr_stream stream) {
     return GSR_OK;
 }
 
+int gsr_debug_fused_pass(gsr_matrix* A, const double* x_dev, double ca, double* y_dev, double* t_dev,
+                         gsr_stream stream) {
+    if (!A || !x_dev || !t_dev || (!y_dev && A->dims.n_rows > 0)) return GSR_EINVAL;
+    if (A->state != 1) return GSR_ESTATE;
+    if (A->n_con > 0 || A->comm) return GSR_EUNSUPPORTED;
+    cudaStream_t s = (cudaStream_t)stream;
+    Workspace& W = A->ws;
+    GSR_TRY(ensure_workspace(A));
+    W.solved = false;
+    const double coef[2] = {ca, 0.0};
+    GSR_CUDA_TRY(cudaMemcpyAsync(W.red, coef, sizeof(coef), cudaMemcpyHostToDevice, s));
+    GSR_CUDA_TRY(cudaStreamSynchronize(s));   // `coef` lives on this stack frame
+    k_gather_sumsq<<<NB_N, TB_N, 0, s>>>(y_dev, A->perm, W.u, A->m_int, W.part_u);
+    count_launch();
+    GSR_TRY(launch_fused(A, x_dev, W.u, W.red, W.part_u, t_dev, nullptr, nullptr, s));
+    k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units, W.red + 3, nullptr);
+    GSR_TRY(launch_aprod2_instr(A, W.u, t_dev, W.red + 3, nullptr, 0, s));
+    k_scatter_rows<<<NB_N, TB_N, 0, s>>>(W.u, A->perm, y_dev, A->m_int);
+    count_launch(2);
+    GSR_CUDA_TRY(cudaGetLastError());
+    return GSR_OK;
+}
+
 int gsr_time_product(gsr_matrix* A, int which, int reps, float* ms_avg, gsr_stream stream) {
     if (!A || !ms_avg || reps < 1 || which < 1 || which > 4) return GSR_EINVAL;
     if (A->state != 1) return GSR_ESTATE;
@@ -659,7 +738,7 @@ int gsr_time_product(gsr_matrix* A, int which, int reps, float* ms_avg, gsr_stre
     GSR_CUDA_TRY(cudaEventCreate(&e1));
     int rc = GSR_OK;
     if (which == 4) {   // the instrumental pass needs a consistent u_hat and its sum of squares
-        rc = launch_fused(A, W.v, W.u, A->coef_one, W.part_u, W.t, nullptr, s);
+        rc = launch_fused(A, W.v, W.u, A->coef_one, W.part_u, W.t, nullptr, nullptr, s);
         k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units, W.red + 3, nullptr);
     }
     for (int pass = 0; pass < 2 && rc == GSR_OK; ++pass) {   // pass 0: warm-up
@@ -668,8 +747,8 @@ int gsr_time_product(gsr_matrix* A, int which, int reps, float* ms_avg, gsr_stre
         for (int i = 0; i < nrep && rc == GSR_OK; ++i) {
             if (which == 1) rc = launch_aprod1(A, W.v, W.u, A->coef_one, W.part_u, nullptr, nullptr, s);
             else if (which == 2) rc = launch_aprod2(A, W.u, W.v, A->coef_one, nullptr, nullptr, s);
-            else if (which == 3) rc = launch_fused(A, W.v, W.u, A->coef_one, W.part_u, W.t, nullptr, s);
-            else rc = launch_aprod2_instr(A, W.u, W.t, W.red + 3, nullptr, s);
+            else if (which == 3) rc = launch_fused(A, W.v, W.u, A->coef_one, W.part_u, W.t, nullptr, nullptr, s);
+            else rc = launch_aprod2_instr(A, W.u, W.t, W.red + 3, nullptr, 0, s);
         }
         cudaEventRecord(e1, s);
         if (cudaEventSynchronize(e1) != cudaSuccess) rc = GSR_ECUDA;

@@ -389,6 +389,7 @@ const char* gsr_strerror(int code) {
         case GSR_ECUDA: return "CUDA runtime error";
         case GSR_ESTATE: return "call not legal in this state";
         case GSR_EUNSUPPORTED: return "unsupported device (needs sm_100), size or option";
+        case GSR_ERANGE: return "deterministic mode: a pass left the range of its fixed-point sums";
         default: return "unknown gsr status";
     }
 }
@@ -589,7 +590,7 @@ int gsr_set_option(gsr_matrix* A, int key, int64_t value) {
     if (!A) return GSR_EINVAL;
     switch (key) {
         case GSR_OPT_FORCE_ITNLIM: A->opt_force_itnlim = value != 0; return GSR_OK;
-        case GSR_OPT_DETERMINISTIC: return value == 0 ? GSR_OK : GSR_EUNSUPPORTED;
+        case GSR_OPT_DETERMINISTIC: A->opt_deterministic = value != 0; return GSR_OK;
         case GSR_OPT_FUSED: A->opt_two_pass = value == 0; return GSR_OK;
         case GSR_OPT_FIXED_POINT: A->opt_no_fixed = value == 0; return GSR_OK;
         default: return GSR_EINVAL;

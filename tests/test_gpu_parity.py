@@ -344,13 +344,17 @@ def test_fixed_point_instrumental_pass_matches_fp64_atomics(name):
         k = 3
         ro = s.o.lsqr(rhs, k, force_itnlim=True)
         xs = []
-        for fixed in (1, 0):
+        for i, fixed in enumerate((1, 0, 0, 1)):
             b.gsr_set_option(s.A.h, b.GSR_OPT_FIXED_POINT, fixed)
             x = torch.empty(s.n, dtype=torch.float64, device="cuda")
             r = b.gsr_lsqr_solve(s.A.h, bd, x, k)
             assert (r.istop, r.itn) == (7, k)
             xs.append(x.cpu().numpy())
             assert np.linalg.norm(xs[-1] - ro.x) <= X_TOL * np.linalg.norm(ro.x)
+            # the variant of the instrumental pass is frozen into the captured graph: toggling
+            # the option must re-capture (1 -> 0 -> 0 -> 1: three graphs), or the second leg
+            # would replay the first one's kernels
+            assert b.gsr_debug_graph_builds(s.A.h) == (1, 2, 2, 3)[i]
         assert np.linalg.norm(xs[0] - xs[1]) <= 1e-12 * np.linalg.norm(ro.x)
     finally:
         s.A.close()
@@ -389,5 +393,56 @@ def test_damped_lsqr_parity(fused):
         r = b.gsr_lsqr_solve(s.A.h, bd, x, 500, 1e-10, 1e-10, 1e8)
         ro = s.o.lsqr(rhs, 500, 1e-10, 1e-10, 1e8)
         assert r.istop == ro.istop and np.linalg.norm(x.cpu().numpy() - ro.x) <= X_TOL * np.linalg.norm(ro.x)
+    finally:
+        s.A.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1", "skew_hot", "ragged_empty_stars"])
+def test_deterministic_mode_is_bit_reproducible(name):
+    """GSR_OPT_DETERMINISTIC (SURVEY 8(a) a5/a8, section 4 tier T4; the paper names its atomics
+    as a weakness): every sum that leaves a warp is a 64-bit fixed-point
+    integer add, so repeated solves on a handle are bit-identical -- x, the norms and the
+    standard errors -- and still match the oracle."""
+    b = _binding()
+    s = Sys(CASES[name])
+    try:
+        rhs = _rhs(s)
+        bd = torch.from_numpy(rhs).cuda()
+        b.gsr_set_option(s.A.h, b.GSR_OPT_DETERMINISTIC, 1)
+        x = torch.empty(s.n, dtype=torch.float64, device="cuda")
+        with pytest.raises(b.GsrError) as ei:      # needs unit column norms
+            b.gsr_lsqr_solve(s.A.h, bd, x, 3)
+        assert ei.value.code == b.GSR_EUNSUPPORTED
+        s.o.precondition()
+        b.gsr_precondition(s.A.h)
+        b.gsr_set_option(s.A.h, b.GSR_OPT_FORCE_ITNLIM, 1)
+        for k in (1, 8, 30):
+            ro = s.o.lsqr(rhs, k, force_itnlim=True)
+            runs = []
+            for rep in range(3):
+                x = torch.empty(s.n, dtype=torch.float64, device="cuda")
+                r = b.gsr_lsqr_solve(s.A.h, bd, x, k)
+                se = torch.empty(s.n, dtype=torch.float64, device="cuda")
+                b.gsr_lsqr_standard_errors(s.A.h, se)
+                runs.append((x.cpu().numpy(), se.cpu().numpy(), r))
+            for xx, se, r in runs[1:]:
+                assert np.array_equal(xx, runs[0][0]) and np.array_equal(se, runs[0][1])
+                assert r == runs[0][2]
+            assert (runs[0][2].istop, runs[0][2].itn) == (ro.istop, ro.itn) == (7, k)
+            assert np.linalg.norm(runs[0][0] - ro.x) <= X_TOL * np.linalg.norm(ro.x)
+        # standard mode with stopping rules: same stop, still bit-identical
+        ro = s.o.lsqr(rhs, 300, atol=1e-10, btol=1e-10, conlim=1e8)
+        b.gsr_set_option(s.A.h, b.GSR_OPT_FORCE_ITNLIM, 0)
+        xa = torch.empty(s.n, dtype=torch.float64, device="cuda")
+        xb = torch.empty(s.n, dtype=torch.float64, device="cuda")
+        ra = b.gsr_lsqr_solve(s.A.h, bd, xa, 300, 1e-10, 1e-10, 1e8)
+        rb = b.gsr_lsqr_solve(s.A.h, bd, xb, 300, 1e-10, 1e-10, 1e8)
+        assert ra == rb and torch.equal(xa, xb)
+        assert (ra.istop, ra.itn) == (ro.istop, ro.itn)
+        # back to fp64 atomics: same answer within the parity tolerance
+        b.gsr_set_option(s.A.h, b.GSR_OPT_DETERMINISTIC, 0)
+        rc = b.gsr_lsqr_solve(s.A.h, bd, xb, 300, 1e-10, 1e-10, 1e8)
+        assert (rc.istop, rc.itn) == (ro.istop, ro.itn)
+        assert float((xa - xb).norm() / xa.norm()) <= 1e-9
     finally:
         s.A.close()
