@@ -8,9 +8,11 @@ target is quoted on).  Inputs are seeded and synthetic (paper_2212_11675_b200/in
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg3] [--impl ours|reference]
 
-N > 1 (torchrun): every rank holds an independent system of the same config (weak scaling,
-no data-path collective).  `--impl reference` times the CPU oracle,
-as it stands, on a bounded sample of the workload (rank 0 only).
+N > 1 (torchrun): ONE system of N x the config's rows, row-sharded over the ranks by star-aligned
+blocks (the paper's MPI partition) with the replicated slice all-reduced by NCCL
+inside the CUDA graph; `--replicas` gives every rank an independent
+system instead (no data-path collective).  `--impl reference` times the CPU oracle, as it
+stands, on a bounded sample of the workload (rank 0 only).
 """
 from __future__ import annotations
 
@@ -33,11 +35,18 @@ TRAFFIC_APROD1, TRAFFIC_APROD2 = 228, 220      # bytes per row the 212 B/row lay
 # fused iteration (GSR_OPT_FUSED, default): k_fused does aprod1 and aprod2 minus the instrumental
 # block of A^T u (6 x (8+4) B of matrix + 8 B of u per row = 80 B), which k_aprod2_instr does
 BYTES_INSTR = 80
-BYTES_FUSED = BYTES_APROD1 + BYTES_APROD2 - BYTES_INSTR   # 392 algorithmic bytes per row
-# DRAM bytes per row measured by `ncu --set full` (dram__bytes_read.sum + dram__bytes_write.sum
-# over the rows of the launch; profiles/r1_v2_aprod_ncu_full.md); multiplied by the rows of the
-# timed launch to give roofline.traffic
-NCU_TRAFFIC_PER_ROW = {"aprod1": 228.2, "aprod2": 220.4, "fused": 229.1, "aprod2_instr": 68.1}
+# What ONE fused pass must move: the matrix once (224 B/row with int32 indices) +
+# u_hat read + u_hat write.  This is the roofline figure of k_fused.  The same work done as two
+# products would move 240 + 232 - 80 = 392 B/row; that "two-product equivalent" rate is reported
+# separately (products.fused_two_product_equiv_gbs) and is not a roofline fraction.
+BYTES_FUSED = 224 + 8 + 8
+BYTES_FUSED_2P = BYTES_APROD1 + BYTES_APROD2 - BYTES_INSTR
+BYTES_ITER_FUSED = BYTES_FUSED + BYTES_INSTR    # 320 B/row per fused iteration
+# DRAM bytes per row measured by `ncu --set full` at cfg3 (dram__bytes_read.sum +
+# dram__bytes_write.sum over the rows of the launch); multiplied by the rows of the timed launch
+# to give roofline.traffic.  Source files under profiles/ (NCU_TRAFFIC_SOURCE).
+NCU_TRAFFIC_PER_ROW = {"aprod1": 228.2, "aprod2": 220.4, "fused": 230.3, "aprod2_instr": 68.1}
+NCU_TRAFFIC_SOURCE = "profiles/r2_fused_ncu_full.md (k_fused), profiles/r1_v4_aprod_ncu_full.md (products), cfg3"
 GEN_ROWS = 1 << 23                              # rows generated and appended per chunk
 
 
@@ -49,12 +58,15 @@ def parse():
     ap.add_argument("--config", default="cfg3")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--oracle-rows", type=int, default=1 << 22)
+    ap.add_argument("--time-ordered", action="store_true",
+                    help="row f4(i): rows of a star in time order (att_start non-decreasing inside a star)")
+    ap.add_argument("--replicas", action="store_true",
+                    help="N > 1: N independent systems (no collective) instead of one row-sharded system")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--two-pass", action="store_true",
                     help="GSR_OPT_FUSED = 0: aprod1 + aprod2 per iteration (two reads of the matrix)")
     ap.add_argument("--sharded", action="store_true",
-                    help="N > 1: ONE system of N x the config's rows, row-sharded over the ranks "
-                         "(NCCL all-reduce of the replicated slice inside the graph) instead of N replicas")
+                    help="row-sharded form (the default for N > 1; at N = 1 a one-rank NCCL communicator)")
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE config 5: time aprod1/aprod2 alone from 1e6 to 3e8 rows")
     return ap.parse_args()
@@ -100,20 +112,50 @@ class ClockSampler(threading.Thread):
                 "reasons": reasons, "samples": len(self.rows)}
 
 
-def oracle_sample(cfg, rows, steps):
-    """The oracle, as it stands, on the first `rows` rows of the workload (own b, own p)."""
+def host_info():
+    """The box the oracle is timed on (nproc, CPU model, host RAM)."""
+    model, ram = "unknown", None
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.startswith("model name"):
+                model = ln.split(":", 1)[1].strip()
+                break
+        for ln in open("/proc/meminfo"):
+            if ln.startswith("MemTotal"):
+                ram = round(int(ln.split()[1]) / 1048576.0, 1)
+                break
+    except OSError:
+        pass
+    return {"nproc": os.cpu_count(), "cpu_model": model, "ram_gb": ram}
+
+
+def config_dict(cfg, args, world, sharded, m_total, n_total):
+    """`config` of the JSON line; the same function serves both arms (ours and --impl reference)."""
+    return {"workload": cfg.name + ("+time-ordered" if cfg.att_time_ordered else ""),
+            "rows": m_total, "cols": n_total, "stars": cfg.n_stars * (world if sharded else 1),
+            "knots_per_axis": cfg.n_dfa, "instr_cols": cfg.n_instr,
+            "preconditioned": True, "mode": "fixed-count (GSR_OPT_FORCE_ITNLIM)",
+            "iteration": "two-pass (aprod1 + aprod2)" if args.two_pass else
+                         "fused (one read of the matrix per iteration + instrumental pass)",
+            "l2": "matrix (%.1f GB) is far larger than L2; no flush needed" % (224e-9 * cfg.n_rows)
+                  if 224 * cfg.n_rows > 1e9 else "matrix fits in or near L2: L2-assisted numbers",
+            "parallelism": ("row-sharded x%d (NCCL all-reduce of the replicated slice)" % world
+                            if sharded else "replicas" if world > 1 else "single")}
+
+
+def oracle_sample(cfg, rows, steps, omp=False):
+    """The oracle, as it stands, on the first `rows` rows of the workload (own b, own p).
+    omp=True: its OpenMP timing build (same file, -DORC_OPENMP), all host cores."""
     import numpy as np
-    from dataclasses import replace
     from paper_2212_11675_b200 import inputs
     from oracle import gsr_oracle
     rows = min(rows, cfg.n_rows)
     sptr = inputs.star_ptr(cfg)
     star, att, instr, vals = inputs.gen_rows(cfg, 0, rows, "cpu", sptr=sptr)
     n_stars = int(star[-1]) + 1
-    sub = replace(cfg, name=cfg.name + "-sample", n_stars=n_stars, rows_per_star=0,
-                  n_rows_total=rows, counts=None)
     o = gsr_oracle.OracleSystem(n_stars, cfg.n_dfa, cfg.n_instr, star.numpy(), att.numpy(),
-                                instr.numpy(), vals.numpy())
+                                instr.numpy(), vals.numpy(), omp=omp)
+    del star, att, instr, vals
     xt = np.random.default_rng(cfg.seed).standard_normal(o.n)
     b = o.aprod1(xt, 1e-3 * np.random.default_rng(cfg.seed + 1).standard_normal(o.m))
     o.precondition()
@@ -122,28 +164,46 @@ def oracle_sample(cfg, rows, steps):
     dt = time.perf_counter() - t0
     assert r.itn == steps
     it_s_sample = steps / dt
-    return {"value": it_s_sample * rows / cfg.n_rows, "unit": UNIT, "cores": 1, "kind": "oracle",
+    cores = gsr_oracle.omp_threads() if omp else 1
+    return {"value": it_s_sample * rows / cfg.n_rows, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "build": "OpenMP timing build (aprod1 parallel for; aprod2 star-aligned ranges, thread-private "
+                     "replicated-slice accumulators combined in thread order, PAPER.md:103)" if omp
+                     else "serial",
             "sample": f"first {rows} rows ({n_stars} stars) of {cfg.name}, {steps} oracle LSQR "
                       f"iterations in {dt:.2f} s = {it_s_sample:.3f} it/s on the sample, scaled "
                       f"linearly by rows to the full {cfg.n_rows}-row system",
-            "seconds": dt}
+            "extrapolated": rows < cfg.n_rows, "seconds": dt}
+
+
+def cpu_baseline(cfg, rows, steps):
+    """`cpu_baseline` of the JSON line: the oracle on all host cores (value), and on one core."""
+    from oracle import gsr_oracle
+    gsr_oracle.build()
+    gsr_oracle.build(omp=True)
+    one = oracle_sample(cfg, rows, steps, omp=False)
+    allc = oracle_sample(cfg, rows, steps, omp=True)
+    allc["one_core"] = {k: one[k] for k in ("value", "unit", "cores", "sample", "seconds")}
+    allc["host"] = host_info()
+    return allc
 
 
 def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    from oracle import gsr_oracle
-    gsr_oracle.build()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    sharded = (world > 1 and not args.replicas) or args.sharded
     steps = max(1, min(args.steps, 20))
     for _ in range(min(args.warmup, 1)):
         oracle_sample(cfg, min(args.oracle_rows, 1 << 16), 1)
-    cb = oracle_sample(cfg, args.oracle_rows, steps)
+    cb = cpu_baseline(cfg, args.oracle_rows, steps)
+    m_total = cfg.n_rows * (world if sharded else 1)
+    n_total = cfg.n_cols + (5 * cfg.n_stars * (world - 1) if sharded else 0)
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT,
             "n_gpus": args.gpus, "steps": steps, "warmup": args.warmup,
             "ms_per_step": 1e3 / cb["value"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": cfg.name, "rows": cfg.n_rows, "cols": cfg.n_cols},
+            "config": config_dict(cfg, args, world, sharded, m_total, n_total),
             "cpu_baseline": cb,
             "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0,
                     "d2h_bytes_per_step": 0},
@@ -178,6 +238,9 @@ def run_sweep(args):
     sizes = [1_000_000 * 2 ** k for k in range(9)] + [300_000_000]
     for m in sizes:
         cfg = inputs.named_config(f"cfg5_{m}")
+        if args.time_ordered:
+            from dataclasses import replace
+            cfg = replace(cfg, att_time_ordered=True)
         h = build_system(cfg, g, inputs, torch, dev)
         ms1 = g.gsr_time_product(h, 1, 20)
         ms2 = g.gsr_time_product(h, 2, 20)
@@ -194,6 +257,7 @@ def run_sweep(args):
             torch.cuda.synchronize()
             api.append(e0.elapsed_time(e1) / 5)
         row = {"workload": cfg.name, "rows": m, "cols": cfg.n_cols,
+               "row_order": "time-ordered inside a star" if args.time_ordered else "uniform random knots",
                "l2": "L2-assisted" if 224 * m < 1e9 else "HBM",
                "aprod1_ms": ms1, "aprod2_ms": ms2,
                "aprod1_gbs": BYTES_APROD1 * m / ms1 * 1e-6, "aprod2_gbs": BYTES_APROD2 * m / ms2 * 1e-6,
@@ -214,6 +278,9 @@ def main():
     args = parse()
     from paper_2212_11675_b200 import inputs
     cfg0 = inputs.named_config(args.config)
+    if args.time_ordered:
+        from dataclasses import replace as _replace
+        cfg0 = _replace(cfg0, att_time_ordered=True)
     if args.impl == "reference":
         return run_reference(args, cfg0)
     if args.sweep:
@@ -231,7 +298,8 @@ def main():
     dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
-    cfg = replace(cfg0, seed=cfg0.seed + 1000 * rank) if rank else cfg0   # independent systems
+    sharded = (world > 1 and not args.replicas) or args.sharded
+    cfg = replace(cfg0, seed=cfg0.seed + 1000 * rank) if rank else cfg0   # rank's own rows
     m, n = cfg.n_rows, cfg.n_cols
 
     def barrier():
@@ -248,9 +316,9 @@ def main():
         nr = min(GEN_ROWS, m - r0)
         b[r0:r0 + nr] = inputs.noise(cfg, r0, nr, dev)
     comm = None
-    if args.sharded:
-        if os.environ.get("NCCL_DEBUG", "VERSION").upper() == "VERSION":
-            os.environ["NCCL_DEBUG"] = "WARN"    # keep stdout to the one JSON line
+    if sharded:
+        if "NCCL_DEBUG" not in os.environ:
+            os.environ["NCCL_DEBUG"] = "WARN"    # unset: keep stdout to the one JSON line
         # weak-scaled sharded system: rank r owns stars [r*S, (r+1)*S) of an N*S-star system; the
         # attitude + instrumental + global unknowns are shared, so their x_true comes from rank 0's seed
         xt0 = inputs.x_true(cfg0, dev)
@@ -329,19 +397,14 @@ def main():
             dom = ("fused", gb3, ms3, BYTES_FUSED)
         tpr = NCU_TRAFFIC_PER_ROW[dom[0]]
         traffic = tpr * m if tpr is not None else None
+        iter_bytes = (BYTES_APROD1 + BYTES_APROD2) if args.two_pass else BYTES_ITER_FUSED
+        m_total = m * (world if sharded else 1)
+        n_total = n + (5 * cfg.n_stars * (world - 1) if sharded else 0)
         line = {
             "metric": METRIC, "value": world * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
             "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": cfg0.name, "rows": m, "cols": n, "stars": cfg.n_stars,
-                       "knots_per_axis": cfg.n_dfa, "instr_cols": cfg.n_instr,
-                       "preconditioned": True, "mode": "fixed-count (GSR_OPT_FORCE_ITNLIM)",
-                       "iteration": "two-pass (aprod1 + aprod2)" if args.two_pass else
-                                    "fused (one read of the matrix per iteration + instrumental pass)",
-                       "l2": "matrix (%.1f GB) is far larger than L2; no flush needed" % (224e-9 * m)
-                             if 224 * m > 1e9 else "matrix fits in or near L2: L2-assisted numbers",
-                       "parallelism": ("row-sharded x%d (NCCL all-reduce of the replicated slice)" % world
-                                       if args.sharded else "replicas" if world > 1 else "single")},
+            "config": config_dict(cfg0, args, world, sharded, m_total, n_total),
             "e2e": {"value": world * K / (ms_e2e * 1e-3), "unit": UNIT,
                     "h2d_bytes_per_step": 8 * m / K, "d2h_bytes_per_step": (8 * n + 80) / K,
                     "note": "gsr_lsqr_solve with pinned host b and host x; matrix resident"},
@@ -349,37 +412,45 @@ def main():
             "clocks": clocks,
             "roofline": {"bound": "hbm", "kernel": dom[0], "achieved": dom[1], "peak": peak,
                          "unit": "GB/s", "frac": dom[1] / peak, "traffic": traffic,
-                         "traffic_note": "DRAM bytes per launch: ncu --set full bytes per row "
-                                         "(profiles/r1_v6_fused_ncu_full.md, r1_v4_aprod_ncu_full.md) x rows of this launch; the "
-                                         "layout stores 212 B/row, so traffic < algorithmic bytes",
+                         "dram_gbs": traffic / dom[2] * 1e-6, "dram_frac": traffic / dom[2] * 1e-6 / peak,
+                         "traffic_note": "DRAM bytes per launch = ncu --set full bytes per row ("
+                                         + NCU_TRAFFIC_SOURCE + ") x rows of this launch; the layout "
+                                         "stores 212 B/row (uint16 indices), so traffic < algorithmic bytes",
                          "peak_source": peak_src, "algorithmic_bytes_per_row": dom[3],
+                         "algorithmic_note": "k_fused: ONE read of the matrix (224 B/row, int32 indices) "
+                                             "+ u_hat read + write = 240 B/row; aprod1 240, aprod2 232",
                          "ms_per_launch": dom[2]},
             "products": {"aprod1_gbs": gb1, "aprod2_gbs": gb2, "aprod1_ms": ms1, "aprod2_ms": ms2,
                          "fused_ms": ms3, "fused_gbs": gb3, "instr_pass_ms": ms4, "instr_pass_gbs": gb4,
-                         "fused_plus_instr_gbs": (BYTES_APROD1 + BYTES_APROD2) * m / (ms3 + ms4) * 1e-6,
-                         "aprod1_actual_gbs": TRAFFIC_APROD1 * m / ms1 * 1e-6,
-                         "aprod2_actual_gbs": TRAFFIC_APROD2 * m / ms2 * 1e-6,
+                         "fused_two_product_equiv_gbs": BYTES_FUSED_2P * m / ms3 * 1e-6,
+                         "aprod1_frac_of_measured": gb1 / peak, "aprod2_frac_of_measured": gb2 / peak,
+                         "aprod1_dram_gbs": TRAFFIC_APROD1 * m / ms1 * 1e-6,
+                         "aprod2_dram_gbs": TRAFFIC_APROD2 * m / ms2 * 1e-6,
                          "combined_gbs": gb12, "combined_frac_of_measured": gb12 / peak,
                          "combined_frac_of_8tbs": gb12 / 8000.0,
-                         "iteration_gbs": 472 * m / (ms / K) * 1e-6,
-                         "iteration_frac_of_measured": 472 * m / (ms / K) * 1e-6 / peak,
-                         "iteration_frac_of_8tbs": 472 * m / (ms / K) * 1e-6 / 8000.0,
-                         "note": "GB/s are algorithmic (240 / 232 B per row per product, 472 per "
-                                 "iteration); the fused iteration reads the 212 B/row matrix once, so "
-                                 "its DRAM traffic is about 300 B/row"},
+                         "iteration_gbs": iter_bytes * m / (ms / K) * 1e-6,
+                         "iteration_frac_of_measured": iter_bytes * m / (ms / K) * 1e-6 / peak,
+                         "iteration_two_product_equiv_gbs": 472 * m / (ms / K) * 1e-6,
+                         "iteration_two_product_equiv_frac_of_8tbs": 472 * m / (ms / K) * 1e-6 / 8000.0,
+                         "note": "GB/s are algorithmic: aprod1 240, aprod2 232 B/row; fused pass 240 "
+                                 "(one matrix read), instrumental pass 80, fused iteration 320 B/row. "
+                                 "*_two_product_equiv_* divide the 472 B/row of an aprod1 + aprod2 "
+                                 "iteration by the fused time (what a two-product code would need to "
+                                 "sustain to be as fast); not a roofline fraction"},
             "lsqr": {"istop": res.istop, "itn": res.itn, "rnorm": res.rnorm, "anorm": res.anorm,
                      "acond": res.acond, "xnorm": res.xnorm, "istop_natural": res.istop_natural,
                      "itn_natural": res.itn_natural},
             "solve_call_ms": ms_solve,
-            "timing": "value = K / device time of the K iterations (CUDA events inside gsr_lsqr_solve on "
-                      "the launching stream); solve_call_ms also has the initialisation (one aprod2) "
-                      "and the finalisation; e2e is the wall clock of the whole call with host buffers",
+            "timing": "value = N x K / device time of the K iterations, timed by CUDA events that "
+                      "gsr_lsqr_solve records on the launching stream around its graph-launch loop (max "
+                      "over ranks; a row-sharded system has N x the config's rows, so one of its "
+                      "iterations counts as N config-sized ones); solve_call_ms also has the "
+                      "initialisation (one aprod2) and the finalisation; e2e is the wall clock of the "
+                      "whole call with host buffers",
             "setup_s": t_setup, "matrix_device_gb": g.gsr_matrix_device_bytes(h) * 1e-9,
         }
         if world == 1 and not args.no_cpu_baseline:
-            from oracle import gsr_oracle
-            gsr_oracle.build()
-            line["cpu_baseline"] = oracle_sample(cfg0, args.oracle_rows, 20)
+            line["cpu_baseline"] = cpu_baseline(cfg0, args.oracle_rows, 20)
         print(json.dumps(line), flush=True)
     g.gsr_matrix_destroy(h)
     if comm:

@@ -92,7 +92,23 @@ int gsr_matrix_create(gsr_matrix** out, const gsr_dims* dims,
 /* Chunked build for systems whose caller-form arrays do not fit beside the device copy
  * (config 3: 67 GB): begin, append consecutive row ranges in order, finalize.
  * append: row0 must equal the number of rows appended so far; arrays cover nrows rows.
- * finalize synchronises, reports validation errors (GSR_EINVAL) and makes the handle usable. */
+ * finalize synchronises, reports validation errors (GSR_EINVAL) and makes the handle usable.
+ *
+ * Size limits (checked by gsr_matrix_begin / gsr_matrix_create before any device work; tested in
+ * tests/test_abi.py):
+ *   GSR_EINVAL        n_rows < 0, n_stars < 1, n_dfa < 4, n_instr < 1, n_glob != 1;
+ *                     n_cols = 5 S + 3 D + I + 1 >= 2^31 (int32 column indices);
+ *                     n_rows >= 2^32 - 16 (uint32 row permutation; shard larger systems,
+ *                     gsr_matrix_set_comm, or stream them, gsr_stream_*)
+ *   GSR_EUNSUPPORTED  n_instr > 27 520: the product kernels keep the whole instrumental block of
+ *                     x (8 I bytes) in shared memory beside 32 attitude windows (227 KB per SM);
+ *                     more than 4096 attitude bins: n_dfa - 3 > 4096 * bw, where the bin width bw
+ *                     (knots) is what fits in the per-warp window, bw = 241 for I <= 3 328
+ *                     falling to 177 at I = 10 000 and 1 at I = 27 520, i.e. n_dfa <= 987 139 for
+ *                     I <= 3 328 and n_dfa <= 724 995 at I = 10 000;
+ *                     a device that is not sm_100.
+ * All product and solve calls on one handle must be stream-ordered with respect to each other
+ * (one stream, or events between streams): they share the handle's unit counter and workspace. */
 int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* dims, gsr_stream stream);
 int gsr_matrix_append_rows(gsr_matrix* A, int64_t row0, int64_t nrows,
                            const int32_t* star_idx_hd, const int32_t* att_start_hd,

@@ -49,6 +49,41 @@ def test_strerror_and_null_checks(lib):
     assert lib.gsr_launch_count() == 0
 
 
+@pytest.mark.parametrize("dims,code", [
+    ((10, 1, 8, 27521, 1), "GSR_EUNSUPPORTED"),           # I: x's instrumental block + windows > 227 KB
+    ((10, 1, 8, 70000, 1), "GSR_EUNSUPPORTED"),           # I > 65535 (uint16 instrumental columns)
+    ((10, 1, 987_140, 3328, 1), "GSR_EUNSUPPORTED"),  # more than 4096 attitude bins at bw = 241
+    ((10, 1, 724_996, 10_000, 1), "GSR_EUNSUPPORTED"),    # ... at bw = 177 (I = 10 000)
+    ((10, 429_496_800, 8, 1, 1), "GSR_EINVAL"),           # n_cols >= 2^31
+    ((0xFFFFFFF0, 1, 8, 1, 1), "GSR_EINVAL"),             # n_rows >= 2^32 - 16
+    ((-1, 1, 8, 1, 1), "GSR_EINVAL"),
+    ((10, 0, 8, 1, 1), "GSR_EINVAL"),
+    ((10, 1, 8, 0, 1), "GSR_EINVAL"),
+])
+def test_size_limits_documented_in_the_header(lib, dims, code):
+    """include/gsr.h "Size limits": each is refused before any device work."""
+    from paper_2212_11675_b200 import binding as b
+    h = C.c_void_p()
+    d = b.gsr_dims(*dims)
+    assert lib.gsr_matrix_begin(C.byref(h), C.byref(d), None) == getattr(b, code) and not h.value
+
+
+def test_sizes_just_inside_the_limits_pass_the_checks(lib):
+    """The same checks accept the largest sizes the header names (on a box without a GPU the call
+    then fails at the device query, which is not a size error)."""
+    import torch
+    from paper_2212_11675_b200 import binding as b
+    for dims in ((10, 1, 8, 27520, 1), (10, 1, 987_139, 3328, 1), (10, 1, 724_995, 10_000, 1)):
+        h = C.c_void_p()
+        d = b.gsr_dims(*dims)
+        rc = lib.gsr_matrix_begin(C.byref(h), C.byref(d), None)
+        if torch.cuda.is_available():
+            assert rc == b.GSR_OK
+            lib.gsr_matrix_destroy(h)
+        else:
+            assert rc == b.GSR_ECUDA
+
+
 def test_no_gpu_fails_loudly_not_silently(lib):
     """Without a CUDA device the product path reports an error; it never computes on the CPU."""
     import torch

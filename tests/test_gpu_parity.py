@@ -13,6 +13,9 @@ pytestmark = pytest.mark.gpu
 
 APROD_TOL = 1e-12
 X_TOL = 1e-9
+X_TOL_CAP = 1e-6      # upper bound of the sensitivity-relaxed tolerance (reading A20)
+SENS_LOG = []         # (case, fused, k, one-ulp sensitivity of the oracle's x): written to
+                      # gpurun_out/lsqr_sensitivity.json at the end of the module (A20)
 
 
 def _binding():
@@ -158,10 +161,17 @@ def test_precondition_and_lsqr_parity(name, fused):
             ru = s.o.lsqr(rhs_ulp, k, force_itnlim=True, want_se=True)
             sens = np.linalg.norm(ru.x - ro.x) / np.linalg.norm(ro.x)
             sens_se = np.linalg.norm(ru.se - ro.se) / np.linalg.norm(ro.se)
-            tol = max(X_TOL, 20.0 * sens)
+            # capped: no assert of this test has an unbounded tolerance (A20 lists the
+            # measured sensitivities; the largest, skew_hot k = 60, is far below the cap)
+            tol = min(max(X_TOL, 20.0 * sens), X_TOL_CAP)
+            SENS_LOG.append((name, fused, k, float(sens)))
             if k in STABLE_COUNTS[name]:
                 assert sens < 1e-10 and tol == X_TOL, (name, k, sens)
             assert np.linalg.norm(xg - ro.x) <= tol * np.linalg.norm(ro.x), (name, k, sens)
+            # the scaled iterate z = x / p as well (x spans 8 decades at cfg4-like
+            # column scales, so the 2-norm of x alone is blind to the small-scale unknowns)
+            zg, zo = xg / p_ref, ro.x / p_ref
+            assert np.linalg.norm(zg - zo) <= tol * np.linalg.norm(zo), (name, k, sens)
             assert abs(r.rnorm - ro.rnorm) <= tol * ro.rnorm
             # var is a sum of squares of the w vectors.  Before the first natural stop rule fires
             # it is as stable as x; past convergence the Lanczos vectors are rounding noise
@@ -172,7 +182,7 @@ def test_precondition_and_lsqr_parity(name, fused):
             nz = ro.se > 0
             assert np.all(np.isfinite(se_host)) and np.all(se_host[~nz] == 0.0)
             if not converged:
-                se_tol = max(2 * tol, 20.0 * sens_se)    # same rule as for x (reading A20)
+                se_tol = min(max(2 * tol, 20.0 * sens_se), 10 * X_TOL_CAP)   # same rule as for x (A20)
                 assert np.linalg.norm(se_host - ro.se) <= se_tol * np.linalg.norm(ro.se), (name, k, sens_se)
                 if tol == X_TOL:
                     assert np.all(np.abs(se_host[nz] - ro.se[nz]) <= 1e-7 * ro.se[nz])
@@ -446,3 +456,15 @@ def test_deterministic_mode_is_bit_reproducible(name):
         assert float((xa - xb).norm() / xa.norm()) <= 1e-9
     finally:
         s.A.close()
+
+
+def test_zz_write_sensitivity_log():
+    """Not a check of its own: records the oracle's one-ulp sensitivities that bounded the
+    tolerances of test_precondition_and_lsqr_parity (quoted in DESIGN.md, reading A20)."""
+    import json
+    import os
+    assert all(sn < X_TOL_CAP / 20.0 for _, _, _, sn in SENS_LOG), max(SENS_LOG, key=lambda t: t[3])
+    out = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    os.makedirs(out, exist_ok=True)
+    with open(os.path.join(out, "lsqr_sensitivity.json"), "w") as f:
+        json.dump([{"case": c, "fused": fu, "k": k, "sens": sn} for c, fu, k, sn in SENS_LOG], f, indent=1)

@@ -276,3 +276,85 @@ def test_damped_lsqr_solves_the_augmented_problem(damp):
     assert abs(r.rnorm - direct) <= 1e-11 * direct
     r0 = o.lsqr(b, 2000, 1e-15, 1e-15, 1e12)
     assert np.linalg.norm(r.x) < np.linalg.norm(r0.x)          # damping shrinks the solution
+
+
+@pytest.mark.parametrize("damp", [0.3, 2.5])
+@pytest.mark.parametrize("precond", [False, True])
+def test_damped_scipy_black_box(damp, precond):
+    """anorm, acond, xnorm, istop and itn under damping (the line anorm = hyp(anorm, damp), the
+    extra rotation, rnorm with the damping rows' share) against scipy.sparse.linalg.lsqr(damp=...)
+    used as a black box: an independent implementation of the same published algorithm."""
+    cfg = inputs.scaled(inputs.named_config("cfg1"), 10, "cfg1/10")
+    s, a, i, v = inputs.gen_all(cfg)
+    o = make_oracle(cfg, s.numpy(), a.numpy(), i.numpy(), v.numpy())
+    A, _ = csr_from_raw(cfg, s.numpy(), a.numpy(), i.numpy(), v.numpy())
+    b = A @ inputs.x_true(cfg).numpy() + inputs.noise(cfg, 0, cfg.n_rows).numpy()
+    p = None
+    if precond:
+        p = o.precondition()
+        A = A @ __import__("scipy.sparse").sparse.diags(p)
+    # fixed count, before any Ritz value has converged (reading A18): everything to 1e-10
+    k = 6
+    ref = spla.lsqr(A, b, damp=damp, atol=0.0, btol=0.0, conlim=0.0, iter_lim=k)
+    xk, istop, itn, r1norm, r2norm, anorm, acond, arnorm, xnorm = ref[:9]
+    r = o.lsqr(b, k, damp=damp, force_itnlim=True)
+    assert (r.istop, r.itn) == (7, k) and (istop, itn) == (7, k)
+    xs = p * xk if precond else xk
+    assert np.linalg.norm(r.x - xs) <= 1e-10 * np.linalg.norm(xs)
+    assert abs(r.rnorm - r2norm) <= 1e-10 * r2norm          # residual of the augmented system
+    assert abs(r.anorm - anorm) <= 1e-10 * anorm
+    assert abs(r.acond - acond) <= 1e-10 * acond
+    assert abs(r.xnorm - xnorm) <= 1e-10 * xnorm
+    assert abs(r.arnorm - arnorm) <= 1e-9 * arnorm
+    # natural stop: same rule, same iteration (+-1), estimates at the level reading A18 allows
+    ref = spla.lsqr(A, b, damp=damp, atol=1e-10, btol=1e-10, conlim=1e8, iter_lim=500)
+    r = o.lsqr(b, 500, 1e-10, 1e-10, 1e8, damp=damp)
+    assert r.istop == ref[1] and abs(r.itn - ref[2]) <= 1
+    xs = p * ref[0] if precond else ref[0]
+    assert np.linalg.norm(r.x - xs) <= 1e-9 * np.linalg.norm(xs)
+    if r.itn == ref[2]:
+        assert abs(r.rnorm - ref[4]) <= 1e-8 * ref[4]
+        assert abs(r.anorm - ref[5]) <= 1e-5 * ref[5]
+        assert abs(r.acond - ref[6]) <= 1e-5 * ref[6]
+        assert abs(r.xnorm - ref[8]) <= 1e-8 * ref[8]
+
+
+def test_stop_rules_4_and_5_are_told_apart():
+    """atol = btol = conlim = 0 leaves only the machine-precision rules.  A consistent system
+    drives rnorm to rounding level, so 1 + test1/(1 + anorm xnorm/bnorm) <= 1 fires (rule 4, which
+    wins over 5); with noise in b the residual stays O(1) and only test2 = ||A^T r||/(||A|| ||r||)
+    can reach rounding level (rule 5).  scipy's lsqr, as a black box, names the same rule."""
+    cfg, o, A = _sys(seed=7)
+    rng = np.random.default_rng(1)
+    xt = rng.standard_normal(A.shape[1])
+    for noise, rule in ((0.0, 4), (1e-3, 5)):
+        b = A @ xt + noise * rng.standard_normal(A.shape[0])
+        r = o.lsqr(b, 400, 0.0, 0.0, 0.0)
+        ref = spla.lsqr(A, b, atol=0.0, btol=0.0, conlim=0.0, iter_lim=400)
+        assert r.istop == rule == ref[1]
+        assert abs(r.itn - ref[2]) <= 2          # rounding-level quantities decide the exact step
+        assert r.itn < 400
+
+
+def test_stop_rule_6_is_shadowed_and_test3_underflow_gives_rule_3():
+    """Rule 6 (1 + 1/acond <= 1) is evaluated first and loses to every later rule.  With a finite
+    acond >= 1/eps the iterate has resolved a singular value below eps ||A||, and then either the
+    residual is at rounding level (rule 4) or A^T r is (rule 5); the one reachable state in which
+    test3 itself decides is acond = inf: rho^2 underflows to 0 on a matrix scaled by 1e-160,
+    ddnorm = ||w||^2 / 0 = inf, test3 = 0 <= ctol = 0, which is rule 3 -- at iteration 1, in the
+    oracle and in scipy alike.  (reading A25.)"""
+    cfg, star, att, instr, vals = small_system(seed=7)
+    o = make_oracle(cfg, star, att, instr, vals * 1e-160)
+    A, _ = csr_from_raw(cfg, star, att, instr, vals * 1e-160)
+    b = np.random.default_rng(1).standard_normal(A.shape[0])
+    r = o.lsqr(b, 50, 0.0, 0.0, 0.0)
+    with np.errstate(all="ignore"):
+        import warnings
+        with warnings.catch_warnings():
+            warnings.simplefilter("ignore")
+            ref = spla.lsqr(A, b, atol=0.0, btol=0.0, conlim=0.0, iter_lim=50)
+    assert (r.istop, r.itn) == (3, 1) == (ref[1], ref[2])
+    assert np.isinf(r.acond) and np.isinf(ref[6])
+    # in forced mode the same state is recorded as the natural stop and the loop goes on
+    rf = o.lsqr(b, 3, 0.0, 0.0, 0.0, force_itnlim=True)
+    assert (rf.istop, rf.itn, rf.istop_natural, rf.itn_natural) == (7, 3, 3, 1)
