@@ -45,7 +45,7 @@ BYTES_ITER_FUSED = BYTES_FUSED + BYTES_INSTR    # 320 B/row per fused iteration
 # DRAM bytes per row measured by `ncu --set full` at cfg3 (dram__bytes_read.sum +
 # dram__bytes_write.sum over the rows of the launch); multiplied by the rows of the timed launch
 # to give roofline.traffic.  Source files under profiles/ (NCU_TRAFFIC_SOURCE).
-NCU_TRAFFIC_PER_ROW = {"aprod1": 228.2, "aprod2": 220.4, "fused": 230.3, "aprod2_instr": 68.1}
+NCU_TRAFFIC_PER_ROW = {"aprod1": 228.2, "aprod2": 220.4, "fused": 230.1, "aprod2_instr": 68.1}
 NCU_TRAFFIC_SOURCE = "profiles/r2_fused_ncu_full.md (k_fused), profiles/r1_v4_aprod_ncu_full.md (products), cfg3"
 GEN_ROWS = 1 << 23                              # rows generated and appended per chunk
 
@@ -60,6 +60,11 @@ def parse():
     ap.add_argument("--oracle-rows", type=int, default=1 << 22)
     ap.add_argument("--time-ordered", action="store_true",
                     help="row f4(i): rows of a star in time order (att_start non-decreasing inside a star)")
+    ap.add_argument("--streamed-resident-gb", type=float, default=None,
+                    help="row f4(iii): out-of-core system -- at most this many GB of the tiled matrix stay "
+                         "on the device, the rest is streamed from pinned host memory every pass "
+                         "(use with --config cfg3x4 ...)")
+    ap.add_argument("--chunk-mb", type=float, default=512.0, help="streamed: size of each of the two chunk buffers")
     ap.add_argument("--replicas", action="store_true",
                     help="N > 1: N independent systems (no collective) instead of one row-sharded system")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -140,7 +145,10 @@ def config_dict(cfg, args, world, sharded, m_total, n_total):
             "l2": "matrix (%.1f GB) is far larger than L2; no flush needed" % (224e-9 * cfg.n_rows)
                   if 224 * cfg.n_rows > 1e9 else "matrix fits in or near L2: L2-assisted numbers",
             "parallelism": ("row-sharded x%d (NCCL all-reduce of the replicated slice)" % world
-                            if sharded else "replicas" if world > 1 else "single")}
+                            if sharded else "replicas" if world > 1 else "single"),
+            **({"storage": "out-of-core: at most %.1f GB of tiles on the device, the rest in pinned host "
+                           "memory, streamed every pass" % args.streamed_resident_gb}
+               if getattr(args, "streamed_resident_gb", None) is not None else {})}
 
 
 def oracle_sample(cfg, rows, steps, omp=False):
@@ -211,11 +219,15 @@ def run_reference(args, cfg):
     print(json.dumps(line), flush=True)
 
 
-def build_system(cfg, g, inputs, torch, dev):
+def build_system(cfg, g, inputs, torch, dev, resident_gb=None, chunk_mb=512.0):
     """Chunked ingest (gsr_matrix_begin/append/finalize) of rows generated on the device."""
     sptr = inputs.star_ptr(cfg)
     scales = inputs.col_scales(cfg, dev)
-    h = g.gsr_matrix_begin(cfg.n_rows, cfg.n_stars, cfg.n_dfa, cfg.n_instr)
+    if resident_gb is None:
+        h = g.gsr_matrix_begin(cfg.n_rows, cfg.n_stars, cfg.n_dfa, cfg.n_instr)
+    else:
+        h = g.gsr_matrix_begin_streamed(cfg.n_rows, cfg.n_stars, cfg.n_dfa, cfg.n_instr,
+                                        int(resident_gb * 1e9), int(chunk_mb * 1e6))
     for r0 in range(0, cfg.n_rows, GEN_ROWS):
         nr = min(GEN_ROWS, cfg.n_rows - r0)
         star, att, instr, vals = inputs.gen_rows(cfg, r0, nr, dev, sptr=sptr, scales=scales)
@@ -308,7 +320,8 @@ def main():
         torch.cuda.synchronize()
 
     t_setup = time.perf_counter()
-    h = build_system(cfg, g, inputs, torch, dev)
+    h = build_system(cfg, g, inputs, torch, dev, args.streamed_resident_gb, args.chunk_mb)
+    streamed = g.gsr_matrix_host_bytes(h) > 0
     # b = A x_true + noise, formed on the device with the library's own aprod1
     xt = inputs.x_true(cfg, dev)
     b = torch.empty(m, dtype=torch.float64, device=dev)
@@ -345,6 +358,7 @@ def main():
     sampler.start()
     barrier()
     l0 = g.gsr_launch_count()
+    sb0 = g.gsr_matrix_streamed_bytes(h)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.profiler.start()      # cudaProfilerStart: ncu --profile-from-start off sees only this
     e0.record()
@@ -354,6 +368,7 @@ def main():
     torch.cuda.profiler.stop()
     barrier()
     launches = g.gsr_launch_count() - l0
+    streamed_bytes = g.gsr_matrix_streamed_bytes(h) - sb0
     ms_solve = e0.elapsed_time(e1)            # whole call: initialisation + K iterations + x
     ms = g.gsr_lsqr_last_loop_ms(h)           # exactly the K iterations (CUDA events on the stream)
     assert 0.0 < ms <= ms_solve
@@ -375,7 +390,7 @@ def main():
     del b_host
 
     # per-kernel device time of the two products, CUDA events on the launching stream
-    reps = 10
+    reps = 2 if streamed else 10
     ms1 = g.gsr_time_product(h, 1, reps)
     ms2 = g.gsr_time_product(h, 2, reps)
     ms3 = g.gsr_time_product(h, 3, reps)
@@ -449,6 +464,18 @@ def main():
                       "whole call with host buffers",
             "setup_s": t_setup, "matrix_device_gb": g.gsr_matrix_device_bytes(h) * 1e-9,
         }
+        if streamed:
+            # the K iterations + the initial aprod2 each move the host part once (fused form)
+            per_it = streamed_bytes / (K + 1)
+            line["streamed"] = {
+                "host_gb": g.gsr_matrix_host_bytes(h) * 1e-9, "device_gb": g.gsr_matrix_device_bytes(h) * 1e-9,
+                "tile_gb": 212e-9 * m, "tile_bytes_over_hbm_180gb": 212e-9 * m / 180.0,
+                "h2d_gb_per_iteration": per_it * 1e-9, "chunk_mb": args.chunk_mb,
+                "h2d_gbs": per_it / (ms / K) * 1e-6,
+                "note": "iteration time is bounded below by the host part of the matrix over the bus "
+                        "(PCIe 5 x16: 64 GB/s raw, about 55 GB/s of payload); h2d_gbs is what the "
+                        "iteration sustained, kernels of the resident part and of the previous chunk "
+                        "overlapped with the copies"}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(cfg0, args.oracle_rows, 20)
         print(json.dumps(line), flush=True)

@@ -110,6 +110,25 @@ int gsr_matrix_create(gsr_matrix** out, const gsr_dims* dims,
  * All product and solve calls on one handle must be stream-ordered with respect to each other
  * (one stream, or events between streams): they share the handle's unit counter and workspace. */
 int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* dims, gsr_stream stream);
+
+/* Out-of-core build ("1.8e9 rows": the system
+ * "does not fit" one device).  As gsr_matrix_begin, but at most resident_bytes of the tiled
+ * matrix stay in device memory; the rest is kept in PINNED HOST memory owned by the handle
+ * (gsr_matrix_host_bytes) and crosses the bus once per pass over the matrix: every product,
+ * gsr_precondition (which also writes the scaled tiles back) and every LSQR iteration stream
+ * it through two device buffers of chunk_bytes each (raised to 1.7 MB if smaller), the H2D copy
+ * of the next chunk overlapping the kernels of the current one.  append / finalize / products /
+ * solve are used exactly as for a resident handle; results differ from a resident solve only
+ * in the order of floating-point atomic adds.  The m-sized work vectors and the row
+ * permutation (12 B/row) stay on the device.  If resident_bytes covers the whole matrix the
+ * handle is an ordinary resident one.  Not combined with gsr_matrix_set_comm or
+ * GSR_OPT_DETERMINISTIC (gsr_lsqr_solve: GSR_EUNSUPPORTED).
+ * Errors: as gsr_matrix_begin; GSR_EINVAL for negative sizes; GSR_ENOMEM if the host memory
+ * cannot be pinned. */
+int gsr_matrix_begin_streamed(gsr_matrix** out, const gsr_dims* dims, int64_t resident_bytes,
+                              int64_t chunk_bytes, gsr_stream stream);
+int64_t gsr_matrix_host_bytes(const gsr_matrix* A);     /* pinned host memory owned by the handle */
+int64_t gsr_matrix_streamed_bytes(const gsr_matrix* A); /* host-to-device bytes copied so far    */
 int gsr_matrix_append_rows(gsr_matrix* A, int64_t row0, int64_t nrows,
                            const int32_t* star_idx_hd, const int32_t* att_start_hd,
                            const int32_t* instr_col_hd, const double* values_hd);

@@ -22,6 +22,7 @@ EXPORTS = [
     "gsr_aprod2", "gsr_precondition", "gsr_lsqr_solve", "gsr_set_option", "gsr_strerror",
     "gsr_debug_expand_rows", "gsr_time_product", "gsr_launch_count", "gsr_lsqr_standard_errors", "gsr_lsqr_last_loop_ms", "gsr_lsqr_set_damp",
     "gsr_debug_fused_pass", "gsr_debug_graph_builds", "gsr_matrix_set_constraints", "gsr_comm_unique_id", "gsr_comm_create", "gsr_comm_destroy", "gsr_matrix_set_comm",
+    "gsr_matrix_begin_streamed", "gsr_matrix_host_bytes", "gsr_matrix_streamed_bytes",
 ]
 
 
@@ -74,6 +75,11 @@ def lib():
         vp, i64, dbl = C.c_void_p, C.c_int64, C.c_double
         L.gsr_matrix_create.argtypes = [C.POINTER(vp), C.POINTER(gsr_dims), vp, vp, vp, vp, vp]
         L.gsr_matrix_begin.argtypes = [C.POINTER(vp), C.POINTER(gsr_dims), vp]
+        L.gsr_matrix_begin_streamed.argtypes = [C.POINTER(vp), C.POINTER(gsr_dims), i64, i64, vp]
+        L.gsr_matrix_host_bytes.argtypes = [vp]
+        L.gsr_matrix_host_bytes.restype = i64
+        L.gsr_matrix_streamed_bytes.argtypes = [vp]
+        L.gsr_matrix_streamed_bytes.restype = i64
         L.gsr_matrix_append_rows.argtypes = [vp, i64, i64, vp, vp, vp, vp]
         L.gsr_matrix_finalize.argtypes = [vp]
         L.gsr_matrix_destroy.argtypes = [vp]
@@ -159,6 +165,23 @@ def gsr_matrix_begin(n_rows, n_stars, n_dfa, n_instr, stream=None) -> int:
     d = _dims(n_rows, n_stars, n_dfa, n_instr)
     _check(lib().gsr_matrix_begin(C.byref(h), C.byref(d), _stream(stream)), "gsr_matrix_begin")
     return h.value
+
+
+def gsr_matrix_begin_streamed(n_rows, n_stars, n_dfa, n_instr, resident_bytes, chunk_bytes,
+                              stream=None) -> int:
+    h = C.c_void_p()
+    d = _dims(n_rows, n_stars, n_dfa, n_instr)
+    _check(lib().gsr_matrix_begin_streamed(C.byref(h), C.byref(d), int(resident_bytes), int(chunk_bytes),
+                                           _stream(stream)), "gsr_matrix_begin_streamed")
+    return h.value
+
+
+def gsr_matrix_host_bytes(h) -> int:
+    return int(lib().gsr_matrix_host_bytes(h))
+
+
+def gsr_matrix_streamed_bytes(h) -> int:
+    return int(lib().gsr_matrix_streamed_bytes(h))
 
 
 def gsr_matrix_append_rows(h, row0, nrows, star_idx, att_start, instr_col, values):

@@ -756,13 +756,7 @@ int configure_product_kernels(gsr_matrix* A) {
     }
     A->grid1 = A->sm_count * resident_ctas(k_aprod1<true, false>, A);
     A->grid2 = A->sm_count * resident_ctas(k_aprod2<false, false>, A);
-    const int need = (A->n_units + NWARP - 1) / NWARP;
-    if (A->grid1 > need) A->grid1 = need;
-    if (A->grid2 > need) A->grid2 = need;
-    if (A->grid_fused > need) A->grid_fused = need;
-    const int64_t need_i = (A->n_tiles + NWARP - 1) / NWARP;
-    if (A->grid_instr > need_i) A->grid_instr = (int)(need_i > 0 ? need_i : 1);
-    return GSR_OK;
+    return GSR_OK;   // (a launch over few units takes fewer CTAs: grid_for)
 }
 
 static int reset_counter(const gsr_matrix* A, cudaStream_t s) {
@@ -770,21 +764,68 @@ static int reset_counter(const gsr_matrix* A, cudaStream_t s) {
     return GSR_OK;
 }
 
+// persistent grid of a launch over `nu` units: never more CTAs than there are units for
+static int grid_for(int grid, int nu) {
+    const int need = (nu + NWARP - 1) / NWARP;
+    return grid < need ? grid : (need > 0 ? need : 1);
+}
+// a whole pass = the resident view, or the resident view + the streamed chunks (row f4(iii))
+static int pass(const gsr_matrix* A, cudaStream_t s, const std::function<int(const TileView&)>& f) {
+    if (!A->so.on) {
+        const TileView v{A->tiles, 0, A->n_units, 0, A->n_tiles};
+        return f(v);
+    }
+    return for_each_view(const_cast<gsr_matrix*>(A), s, f);
+}
+
+static int aprod1_view(const gsr_matrix* A, const TileView& v, const double* x, double* y, const double* ca,
+                       double* partials, const int* stop, const uint32_t* perm, cudaStream_t s) {
+    const int nu = v.u1 - v.u0;
+    if (nu <= 0) return GSR_OK;
+    const int64_t S = A->dims.n_stars, D = A->dims.n_dfa;
+    const int I = (int)A->dims.n_instr;
+    const int grid = grid_for(A->grid1, nu);
+    const Unit* un = A->units + v.u0;
+    double* pu = partials ? partials + v.u0 : nullptr;
+    GSR_TRY(reset_counter(A, s));
+    if (perm)
+        k_aprod1<false, true><<<grid, TPB, A->smem_bytes, s>>>(
+            v.base, un, nu, A->unit_counter, x, y, ca, nullptr, perm, S, D, I, A->win, A->wstride, stop);
+    else if (partials)
+        k_aprod1<true, false><<<grid, TPB, A->smem_bytes, s>>>(
+            v.base, un, nu, A->unit_counter, x, y, ca, pu, nullptr, S, D, I, A->win, A->wstride, stop);
+    else
+        k_aprod1<false, false><<<grid, TPB, A->smem_bytes, s>>>(
+            v.base, un, nu, A->unit_counter, x, y, ca, nullptr, nullptr, S, D, I, A->win, A->wstride, stop);
+    count_launch();
+    GSR_CUDA_TRY(cudaGetLastError());
+    return GSR_OK;
+}
+
 int launch_aprod1(const gsr_matrix* A, const double* x, double* y, const double* ca,
                   double* partials, const int* stop, const uint32_t* perm, cudaStream_t s) {
     if (A->n_units == 0) return GSR_OK;
+    return pass(A, s, [&](const TileView& v) { return aprod1_view(A, v, x, y, ca, partials, stop, perm, s); });
+}
+
+static int aprod2_view(const gsr_matrix* A, const TileView& v, const double* y, double* x, const double* sy,
+                       const int* stop, const uint32_t* perm, bool square, cudaStream_t s) {
+    const int nu = v.u1 - v.u0;
+    if (nu <= 0) return GSR_OK;
     const int64_t S = A->dims.n_stars, D = A->dims.n_dfa;
     const int I = (int)A->dims.n_instr;
+    const int grid = grid_for(A->grid2, nu);
+    const Unit* un = A->units + v.u0;
     GSR_TRY(reset_counter(A, s));
-    if (perm)
-        k_aprod1<false, true><<<A->grid1, TPB, A->smem_bytes, s>>>(
-            A->tiles, A->units, A->n_units, A->unit_counter, x, y, ca, nullptr, perm, S, D, I, A->win, A->wstride, stop);
-    else if (partials)
-        k_aprod1<true, false><<<A->grid1, TPB, A->smem_bytes, s>>>(
-            A->tiles, A->units, A->n_units, A->unit_counter, x, y, ca, partials, nullptr, S, D, I, A->win, A->wstride, stop);
+    if (square)
+        k_aprod2<true, false><<<grid, TPB, A->smem_bytes, s>>>(
+            v.base, un, nu, A->unit_counter, nullptr, x, nullptr, nullptr, S, D, I, A->win, A->wstride, instr_copies(A), nullptr);
+    else if (perm)
+        k_aprod2<false, true><<<grid, TPB, A->smem_bytes, s>>>(
+            v.base, un, nu, A->unit_counter, y, x, sy, perm, S, D, I, A->win, A->wstride, instr_copies(A), stop);
     else
-        k_aprod1<false, false><<<A->grid1, TPB, A->smem_bytes, s>>>(
-            A->tiles, A->units, A->n_units, A->unit_counter, x, y, ca, nullptr, nullptr, S, D, I, A->win, A->wstride, stop);
+        k_aprod2<false, false><<<grid, TPB, A->smem_bytes, s>>>(
+            v.base, un, nu, A->unit_counter, y, x, sy, nullptr, S, D, I, A->win, A->wstride, instr_copies(A), stop);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;
@@ -793,15 +834,41 @@ int launch_aprod1(const gsr_matrix* A, const double* x, double* y, const double*
 int launch_aprod2(const gsr_matrix* A, const double* y, double* x, const double* sy,
                   const int* stop, const uint32_t* perm, cudaStream_t s) {
     if (A->n_units == 0) return GSR_OK;
-    const int64_t S = A->dims.n_stars, D = A->dims.n_dfa;
-    const int I = (int)A->dims.n_instr;
+    return pass(A, s, [&](const TileView& v) { return aprod2_view(A, v, y, x, sy, stop, perm, false, s); });
+}
+
+static int fused_view(const gsr_matrix* A, const TileView& v, const double* x, double* u, const double* ca,
+                      double* partials, double* t, const int* stop, const int* det_e, cudaStream_t s) {
+    const int nu = v.u1 - v.u0;
+    if (nu <= 0) return GSR_OK;
+    const int grid = grid_for(A->grid_fused, nu);
     GSR_TRY(reset_counter(A, s));
-    if (perm)
-        k_aprod2<false, true><<<A->grid2, TPB, A->smem_bytes, s>>>(
-            A->tiles, A->units, A->n_units, A->unit_counter, y, x, sy, perm, S, D, I, A->win, A->wstride, instr_copies(A), stop);
+    if (det_e)
+        k_fused<true><<<grid, TPB, A->smem_fused, s>>>(
+            v.base, A->units + v.u0, nu, A->unit_counter, x, u, ca, partials + v.u0, t, A->dims.n_stars,
+            A->dims.n_dfa, (int)A->dims.n_instr, A->win, A->wstride, stop, det_e);
     else
-        k_aprod2<false, false><<<A->grid2, TPB, A->smem_bytes, s>>>(
-            A->tiles, A->units, A->n_units, A->unit_counter, y, x, sy, nullptr, S, D, I, A->win, A->wstride, instr_copies(A), stop);
+        k_fused<false><<<grid, TPB, A->smem_fused, s>>>(
+            v.base, A->units + v.u0, nu, A->unit_counter, x, u, ca, partials + v.u0, t, A->dims.n_stars,
+            A->dims.n_dfa, (int)A->dims.n_instr, A->win, A->wstride, stop, nullptr);
+    count_launch();
+    GSR_CUDA_TRY(cudaGetLastError());
+    return GSR_OK;
+}
+
+static int instr_view(const gsr_matrix* A, const TileView& v, const double* u, double* t, const double* ss,
+                      const int* stop, int det, bool fixed, cudaStream_t s) {
+    const int64_t nt = v.t1 - v.t0;
+    if (nt <= 0) return GSR_OK;
+    const int64_t need = (nt + NWARP - 1) / NWARP;
+    const int grid = A->grid_instr < need ? A->grid_instr : (int)need;
+    const unsigned char* T0 = v.base + v.t0 * TILE_BYTES;
+    if (fixed)
+        k_aprod2_instr<true><<<grid, TPB, instr_smem(A), s>>>(
+            T0, nt, u + v.t0 * R, t + A->off_instr, (int)A->dims.n_instr, instr_copies(A), ss, stop, det);
+    else
+        k_aprod2_instr<false><<<grid, TPB, instr_smem(A), s>>>(
+            T0, nt, u + v.t0 * R, t + A->off_instr, (int)A->dims.n_instr, instr_copies(A), nullptr, stop, 0);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;
@@ -810,18 +877,7 @@ int launch_aprod2(const gsr_matrix* A, const double* y, double* x, const double*
 int launch_fused(const gsr_matrix* A, const double* v, double* u, const double* ca,
                  double* partials, double* t, const int* stop, const int* det_e, cudaStream_t s) {
     if (A->n_units == 0) return GSR_OK;
-    GSR_TRY(reset_counter(A, s));
-    if (det_e)
-        k_fused<true><<<A->grid_fused, TPB, A->smem_fused, s>>>(
-            A->tiles, A->units, A->n_units, A->unit_counter, v, u, ca, partials, t, A->dims.n_stars,
-            A->dims.n_dfa, (int)A->dims.n_instr, A->win, A->wstride, stop, det_e);
-    else
-        k_fused<false><<<A->grid_fused, TPB, A->smem_fused, s>>>(
-            A->tiles, A->units, A->n_units, A->unit_counter, v, u, ca, partials, t, A->dims.n_stars,
-            A->dims.n_dfa, (int)A->dims.n_instr, A->win, A->wstride, stop, nullptr);
-    count_launch();
-    GSR_CUDA_TRY(cudaGetLastError());
-    return GSR_OK;
+    return pass(A, s, [&](const TileView& w) { return fused_view(A, w, v, u, ca, partials, t, stop, det_e, s); });
 }
 
 int launch_aprod2_instr(const gsr_matrix* A, const double* u, double* t, const double* ss,
@@ -829,15 +885,21 @@ int launch_aprod2_instr(const gsr_matrix* A, const double* u, double* t, const d
     if (A->n_tiles == 0) return GSR_OK;
     if (det && (A->p == nullptr || ss == nullptr)) return GSR_ESTATE;
     // exact fixed-point accumulation needs unit column norms (see k_aprod2_instr) and ||u||^2
-    if (A->p != nullptr && ss != nullptr && (!A->opt_no_fixed || det))
-        k_aprod2_instr<true><<<A->grid_instr, TPB, instr_smem(A), s>>>(
-            A->tiles, A->n_tiles, u, t + A->off_instr, (int)A->dims.n_instr, instr_copies(A), ss, stop, det);
-    else
-        k_aprod2_instr<false><<<A->grid_instr, TPB, instr_smem(A), s>>>(
-            A->tiles, A->n_tiles, u, t + A->off_instr, (int)A->dims.n_instr, instr_copies(A), nullptr, stop, 0);
-    count_launch();
-    GSR_CUDA_TRY(cudaGetLastError());
-    return GSR_OK;
+    const bool fixed = A->p != nullptr && ss != nullptr && (!A->opt_no_fixed || det);
+    return pass(A, s, [&](const TileView& w) { return instr_view(A, w, u, t, ss, stop, det, fixed, s); });
+}
+
+// Streamed systems: both kernels of the fused iteration on every view while its tiles are on the
+// device, so that the host part of the matrix crosses the bus ONCE per iteration.  The
+// instrumental pass cannot know ||u_hat|| of the whole pass yet, hence fp64 atomics (the pass
+// is bound by the bus, not by them).
+int launch_fused_streamed(const gsr_matrix* A, const double* v, double* u, const double* ca,
+                          double* partials, double* t, const int* stop, cudaStream_t s) {
+    if (A->n_units == 0) return GSR_OK;
+    return pass(A, s, [&](const TileView& w) {
+        GSR_TRY(fused_view(A, w, v, u, ca, partials, t, stop, nullptr, s));
+        return instr_view(A, w, u, t, nullptr, stop, 0, false, s);
+    });
 }
 
 int launch_det_finish(const gsr_matrix* A, double* t, const int* det_e, const double* ss,
@@ -850,13 +912,7 @@ int launch_det_finish(const gsr_matrix* A, double* t, const int* det_e, const do
 
 int launch_colsumsq(const gsr_matrix* A, double* q, cudaStream_t s) {
     if (A->n_units == 0) return GSR_OK;
-    GSR_TRY(reset_counter(A, s));
-    k_aprod2<true, false><<<A->grid2, TPB, A->smem_bytes, s>>>(
-        A->tiles, A->units, A->n_units, A->unit_counter, nullptr, q, nullptr, nullptr, A->dims.n_stars,
-        A->dims.n_dfa, (int)A->dims.n_instr, A->win, A->wstride, instr_copies(A), nullptr);
-    count_launch();
-    GSR_CUDA_TRY(cudaGetLastError());
-    return GSR_OK;
+    return pass(A, s, [&](const TileView& v) { return aprod2_view(A, v, nullptr, q, nullptr, nullptr, nullptr, true, s); });
 }
 
 }  // namespace gsr

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <functional>
 #include <vector>
 
 #include "gsr.h"
@@ -102,6 +103,41 @@ struct Unit {
     int32_t ntiles;   // tiles in the unit
     int32_t a0;       // first knot of the unit's attitude window
     int32_t pad_;
+};
+
+// A run of units and the storage their tiles are read from.  `base` is the address tile 0 WOULD
+// have: a resident matrix passes its tile array, a streamed chunk (row f4(iii), below) passes
+// buffer - t0 * TILE_BYTES, so that the kernels keep their global tile and row indices.
+struct TileView {
+    unsigned char* base;
+    int u0, u1;          // units [u0, u1)
+    int64_t t0, t1;      // tiles [t0, t1) = exactly the tiles of those units
+};
+
+// Out-of-core storage (row f4(iii); systems larger than the device).  Tiles
+// [0, res_cap) stay in device memory, tiles [res_cap, n_tiles) in pinned host memory.  Every
+// pass over the matrix handles the resident run of units with one launch and the rest in
+// CHUNKS (runs of whole units, at most chunk_cap tiles) that a copy stream brings into one of
+// two device buffers while the other is being consumed: H2D copy of chunk c+1 || kernels of
+// chunk c.  All ordering is by events, the host never waits inside a pass.
+struct Chunk {
+    int u0, u1;
+    int64_t t0, t1;
+};
+struct StreamStore {
+    bool on = false;
+    int64_t res_cap = 0;                 // tiles kept on the device
+    int64_t chunk_cap = 0;               // tiles per chunk buffer
+    int64_t host_cap = 0;                // tiles of pinned host storage
+    unsigned char* host = nullptr;       // tile res_cap + i at host + i * TILE_BYTES
+    unsigned char* buf[2] = {nullptr, nullptr};
+    unsigned char* seg = nullptr;        // ingest: the tiles of the segment being scattered
+    int64_t seg_cap = 0;
+    cudaStream_t copy = nullptr;
+    cudaEvent_t copied[2] = {nullptr, nullptr}, done[2] = {nullptr, nullptr}, fork = nullptr;
+    int res_units = 0;                   // units [0, res_units) lie wholly below res_cap
+    std::vector<Chunk>* chunks = nullptr;
+    int64_t h2d_bytes = 0;               // bytes copied host -> device so far (bench.py)
 };
 
 // Device-resident LSQR scalars (row a9): every kernel of the iteration reads its coefficients
@@ -209,6 +245,7 @@ struct gsr_matrix {
     int64_t m_global, n_global;     // rows / columns of the whole system (= local without comm)
     int sm_count;
     gsr::Workspace ws;
+    gsr::StreamStore so;            // row f4(iii): out-of-core storage (so.on)
 };
 
 namespace gsr {
@@ -272,8 +309,17 @@ int launch_fused(const gsr_matrix* A, const double* v, double* u, const double* 
                  double* partials, double* t, const int* stop, const int* det_e, cudaStream_t s);
 int launch_aprod2_instr(const gsr_matrix* A, const double* u, double* t, const double* ss,
                         const int* stop, int det, cudaStream_t s);   // ss: device sum of u^2 (or nullptr)
+int launch_fused_streamed(const gsr_matrix* A, const double* v, double* u, const double* ca,
+                          double* partials, double* t, const int* stop, cudaStream_t s);
 int launch_det_finish(const gsr_matrix* A, double* t, const int* det_e, const double* ss,
                       const int* stop, cudaStream_t s);
 int configure_product_kernels(gsr_matrix* A);
+
+// One pass over the matrix: f(view) for the resident run of units, then for every streamed
+// chunk (double-buffered H2D copies on the copy stream, overlapped with f of the previous view).
+// writeback: f modifies the tiles; streamed chunks are copied back to the host afterwards.
+int for_each_view(gsr_matrix* A, cudaStream_t s, const std::function<int(const TileView&)>& f,
+                  bool writeback = false);
+void free_stream_store(gsr_matrix* A);
 
 }  // namespace gsr

@@ -439,6 +439,17 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
         k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop, 0, nullptr);
         k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N, nullptr);
         k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, nullptr, W.var, 0, nullptr);
+    } else if (A->so.on) {
+        // out-of-core (row f4(iii)): k_fused and the instrumental pass run back to back on every
+        // view while its tiles are on the device -- the host part crosses the bus once
+        GSR_TRY(launch_fused_streamed(A, W.v, W.u, &W.st->ca, W.part_u, W.t, &W.st->stop, s));
+        GSR_TRY(launch_con_aprod1(A, W.v, W.u + A->m_int, &W.st->ca, W.part_u + A->n_units, &W.st->stop, s));
+        GSR_TRY(launch_con_aprod2(A, W.u + A->m_int, W.t, A->coef_one, &W.st->stop, s));
+        k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units + ncp, W.red + 3, &W.st->stop);
+        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.red + 3, 1);
+        k_vnew<<<NB_N, TB_N, 0, s>>>(W.v, W.t, n, W.st, W.part_v, 0, nullptr);
+        k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N, nullptr);
+        k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, W.t, W.var, 0, nullptr);
     } else if (!A->comm) {
         const int det = A->opt_deterministic;
         GSR_TRY(launch_fused(A, W.v, W.u, &W.st->ca, W.part_u, W.t, &W.st->stop, det ? &W.st->det_e : nullptr, s));
@@ -540,6 +551,7 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     const int64_t m = A->dims.n_rows + A->n_con, n = A->n_cols;   // b: observations then constraints
     memset(result, 0, sizeof(*result));
     if (A->comm && A->n_con > 0) return GSR_EUNSUPPORTED;
+    if (A->so.on && (A->comm || A->opt_deterministic)) return GSR_EUNSUPPORTED;
     // deterministic mode: fused iteration on a column-scaled matrix (the range bound of its
     // fixed-point sums needs unit column norms), no constraint rows, one GPU
     if (A->opt_deterministic && (!A->p || A->opt_two_pass || A->comm || A->n_con > 0 || A->damp > 0.0))
@@ -618,18 +630,24 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     GSR_CUDA_TRY(cudaGetLastError());
 
     // the loop: graph launches; the stop flag is polled from pinned memory between batches
-    GSR_TRY(build_graph(A, s));
+    const bool use_graph = !A->so.on;   // streamed: two streams and copies per pass, enqueued by the host
+    if (use_graph) GSR_TRY(build_graph(A, s));
     if (!W.ev0) {
         GSR_CUDA_TRY(cudaEventCreate(&W.ev0));
         GSR_CUDA_TRY(cudaEventCreate(&W.ev1));
     }
     GSR_CUDA_TRY(cudaEventRecord(W.ev0, s));   // device time of the iterations alone (bench.py)
-    const int64_t batch = A->opt_force_itnlim ? 256 : 32;
+    const int64_t batch = !use_graph ? 1 : A->opt_force_itnlim ? 256 : 32;
     int64_t launched = 0;
     while (launched < itnlim) {
         int64_t nb = itnlim - launched < batch ? itnlim - launched : batch;
-        for (int64_t i = 0; i < nb; ++i) GSR_CUDA_TRY(cudaGraphLaunch(W.graph, s));
-        count_launch(nb * kernels_per_iteration(A));
+        if (use_graph) {
+            for (int64_t i = 0; i < nb; ++i) GSR_CUDA_TRY(cudaGraphLaunch(W.graph, s));
+            count_launch(nb * kernels_per_iteration(A));
+        } else {
+            GSR_TRY(enqueue_iteration(A, s));   // (its launchers count their own launches)
+            count_launch(6);
+        }
         launched += nb;
         GSR_CUDA_TRY(cudaMemcpyAsync(W.stop_host, &W.st->stop, sizeof(int), cudaMemcpyDeviceToHost, s));
         GSR_CUDA_TRY(cudaStreamSynchronize(s));

@@ -174,9 +174,10 @@ __global__ void k_save_last_star(const int32_t* __restrict__ star, int64_t ns, i
 // One warp per tile.
 __global__ void __launch_bounds__(256) k_fix_padding(unsigned char* __restrict__ tiles,
                                                      const uint32_t* __restrict__ perm,
-                                                     int64_t n_tiles) {
-    const int64_t t = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+                                                     int64_t t_begin, int64_t n_tiles) {
+    int64_t t = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
     if (t >= n_tiles) return;
+    t += t_begin;
     const int lane = threadIdx.x & 31;
     unsigned char* T = tiles + t * TILE_BYTES;
     const bool real = perm[t * R + lane] != PERM_PAD;
@@ -196,10 +197,10 @@ __global__ void __launch_bounds__(256) k_fix_padding(unsigned char* __restrict__
 // a half from 18.5 to 12.4 wavefronts on uniform columns.  One thread per (tile, half).
 __global__ void __launch_bounds__(128) k_permute_instr(unsigned char* __restrict__ tiles,
                                                        const uint32_t* __restrict__ perm,
-                                                       int64_t n_tiles) {
+                                                       int64_t t_begin, int64_t n_tiles) {
     const int64_t id = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (id >= 2 * n_tiles) return;
-    const int64_t t = id >> 1;
+    const int64_t t = t_begin + (id >> 1);
     const int l0 = (int)(id & 1) * 16;
     unsigned char* T = tiles + t * TILE_BYTES;
     unsigned char cnt[6][16];
@@ -250,10 +251,10 @@ __global__ void __launch_bounds__(128) k_permute_instr(unsigned char* __restrict
 // Caller-order dump of rows [row0, row0+nrows): every internal row whose caller row falls in
 // the range writes its 24 (column, value) pairs.
 __global__ void k_expand_rows(const unsigned char* __restrict__ tiles, const uint32_t* __restrict__ perm,
-                              int64_t m_int, int64_t row0, int64_t nrows, int64_t S, int64_t D,
+                              int64_t r_begin, int64_t r_end, int64_t row0, int64_t nrows, int64_t S, int64_t D,
                               int64_t I, int64_t* __restrict__ cols, double* __restrict__ vals) {
-    const int64_t ri = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (ri >= m_int) return;
+    const int64_t ri = r_begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (ri >= r_end) return;
     const uint32_t pe = perm[ri];
     if (pe == PERM_PAD) return;
     const int64_t r = (int64_t)pe - row0;
@@ -290,11 +291,12 @@ __global__ void k_make_p(double* __restrict__ p, int64_t n) {
 
 // values[i,k] *= p[col(i,k)] in place, one thread per row (8 tiles per CTA).
 __global__ void __launch_bounds__(256) k_scale_values(unsigned char* __restrict__ tiles,
-                                                      int64_t n_tiles, const double* __restrict__ p,
+                                                      int64_t t_begin, int64_t n_tiles,
+                                                      const double* __restrict__ p,
                                                       int64_t S, int64_t D, int64_t I) {
     const int64_t t = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
     if (t >= n_tiles) return;
-    unsigned char* T = tiles + t * TILE_BYTES;
+    unsigned char* T = tiles + (t_begin + t) * TILE_BYTES;
     const int lr = threadIdx.x & 31;
     const int64_t s = ((const int32_t*)(T + OFF_STAR))[lr];
     const int64_t a = (int64_t)(*(const int32_t*)(T + OFF_A0)) + (T + OFF_AOFF)[att_slot(lr)];
@@ -315,9 +317,94 @@ __global__ void __launch_bounds__(256) k_scale_values(unsigned char* __restrict_
     *(double*)(T + val_offset(23, lr)) *= pi[I];
 }
 
+// ---- out-of-core passes (row f4(iii)) -----------------------------------------------------
+// Copy chunk c into buffer c & 1 on the copy stream, as soon as the buffer's last consumer
+// (event done[b], recorded on the compute stream) has finished.  Tiles below res_cap come from
+// the device array (only the first chunk can straddle the boundary), the rest from the host.
+static int issue_chunk_copy(gsr_matrix* A, size_t c) {
+    StreamStore& so = A->so;
+    const Chunk& ch = (*so.chunks)[c];
+    const int b = (int)(c & 1);
+    GSR_CUDA_TRY(cudaStreamWaitEvent(so.copy, so.done[b], 0));
+    const int64_t td = ch.t1 < so.res_cap ? ch.t1 : so.res_cap;
+    if (ch.t0 < td)
+        GSR_CUDA_TRY(cudaMemcpyAsync(so.buf[b], A->tiles + ch.t0 * TILE_BYTES, (size_t)(td - ch.t0) * TILE_BYTES,
+                                     cudaMemcpyDeviceToDevice, so.copy));
+    const int64_t th = ch.t0 > so.res_cap ? ch.t0 : so.res_cap;
+    if (th < ch.t1) {
+        GSR_CUDA_TRY(cudaMemcpyAsync(so.buf[b] + (th - ch.t0) * TILE_BYTES, so.host + (th - so.res_cap) * TILE_BYTES,
+                                     (size_t)(ch.t1 - th) * TILE_BYTES, cudaMemcpyHostToDevice, so.copy));
+        so.h2d_bytes += (ch.t1 - th) * TILE_BYTES;
+    }
+    GSR_CUDA_TRY(cudaEventRecord(so.copied[b], so.copy));
+    return GSR_OK;
+}
+
+int for_each_view(gsr_matrix* A, cudaStream_t s, const std::function<int(const TileView&)>& f, bool writeback) {
+    StreamStore& so = A->so;
+    const std::vector<Chunk>& chunks = *so.chunks;
+    const size_t nc = chunks.size();
+    // the copy stream starts after whatever the caller has queued on s so far (a write-back of an
+    // earlier pass included), then runs ahead of the kernels by up to two chunks
+    GSR_CUDA_TRY(cudaEventRecord(so.fork, s));
+    GSR_CUDA_TRY(cudaStreamWaitEvent(so.copy, so.fork, 0));
+    for (size_t c = 0; c < nc && c < 2; ++c) GSR_TRY(issue_chunk_copy(A, c));
+    if (so.res_units > 0) {
+        const Unit& last = (*A->units_host)[so.res_units - 1];
+        const TileView v{A->tiles, 0, so.res_units, 0, (int64_t)last.tile0 + last.ntiles};
+        GSR_TRY(f(v));
+    }
+    for (size_t c = 0; c < nc; ++c) {
+        const Chunk& ch = chunks[c];
+        const int b = (int)(c & 1);
+        GSR_CUDA_TRY(cudaStreamWaitEvent(s, so.copied[b], 0));
+        const TileView v{so.buf[b] - ch.t0 * TILE_BYTES, ch.u0, ch.u1, ch.t0, ch.t1};
+        GSR_TRY(f(v));
+        if (writeback) {
+            const int64_t td = ch.t1 < so.res_cap ? ch.t1 : so.res_cap;
+            if (ch.t0 < td)
+                GSR_CUDA_TRY(cudaMemcpyAsync(A->tiles + ch.t0 * TILE_BYTES, so.buf[b], (size_t)(td - ch.t0) * TILE_BYTES,
+                                             cudaMemcpyDeviceToDevice, s));
+            const int64_t th = ch.t0 > so.res_cap ? ch.t0 : so.res_cap;
+            if (th < ch.t1)
+                GSR_CUDA_TRY(cudaMemcpyAsync(so.host + (th - so.res_cap) * TILE_BYTES, so.buf[b] + (th - ch.t0) * TILE_BYTES,
+                                             (size_t)(ch.t1 - th) * TILE_BYTES, cudaMemcpyDeviceToHost, s));
+        }
+        GSR_CUDA_TRY(cudaEventRecord(so.done[b], s));
+        if (c + 2 < nc) GSR_TRY(issue_chunk_copy(A, c + 2));
+    }
+    return GSR_OK;
+}
+
+void free_stream_store(gsr_matrix* A) {
+    StreamStore& so = A->so;
+    if (so.host) cudaFreeHost(so.host);
+    for (int b = 0; b < 2; ++b) {
+        if (so.buf[b]) dev_free(A, so.buf[b], (size_t)so.chunk_cap * TILE_BYTES);
+        if (so.copied[b]) cudaEventDestroy(so.copied[b]);
+        if (so.done[b]) cudaEventDestroy(so.done[b]);
+    }
+    if (so.seg) dev_free(A, so.seg, (size_t)so.seg_cap * TILE_BYTES);
+    if (so.fork) cudaEventDestroy(so.fork);
+    if (so.copy) cudaStreamDestroy(so.copy);
+    delete so.chunks;
+    cudaGetLastError();
+    so = StreamStore();
+}
+
 }  // namespace gsr
 
 using namespace gsr;
+
+// padding rows, overlap masks and bank spreading of tiles [t0, t0 + nt) (base: address of tile 0)
+static int finish_tiles(gsr_matrix* A, unsigned char* base, int64_t t0, int64_t nt) {
+    if (nt <= 0) return GSR_OK;
+    k_fix_padding<<<(unsigned)((nt + 7) / 8), 256, 0, A->stream>>>(base, A->perm, t0, nt);
+    k_permute_instr<<<(unsigned)((2 * nt + 127) / 128), 128, 0, A->stream>>>(base, A->perm, t0, nt);
+    count_launch(2);
+    GSR_CUDA_TRY(cudaGetLastError());
+    return GSR_OK;
+}
 
 static int flush_segment(gsr_matrix* A) {
     const int64_t ns = A->seg_fill;
@@ -329,7 +416,14 @@ static int flush_segment(gsr_matrix* A) {
                                                         A->bin_width, A->nbins, nblk, A->seg_counts,
                                                         A->last_star, A->err);
     k_seg_scan<<<1, 1024, 0, s>>>(A->seg_counts, A->nbins, nblk, A->seg_bin_rows);
-    k_seg_scatter<<<nblk, BLK, 0, s>>>(A->tiles, A->perm, A->n_tiles * R, A->rows_appended - ns,
+    // out-of-core: the segment's tiles are built in a device buffer of their own and then moved
+    // to where they live (device array below res_cap, pinned host memory above)
+    unsigned char* base = A->tiles;
+    if (A->so.on) {
+        GSR_CUDA_TRY(cudaMemsetAsync(A->so.seg, 0, (size_t)A->so.seg_cap * TILE_BYTES, s));
+        base = A->so.seg - A->n_tiles * TILE_BYTES;
+    }
+    k_seg_scatter<<<nblk, BLK, 0, s>>>(base, A->perm, A->n_tiles * R, A->rows_appended - ns,
                                        A->st_star, A->st_att, A->st_instr, A->st_vals, ns,
                                        A->dims.n_dfa, A->bin_width, nblk, A->seg_counts);
     k_save_last_star<<<1, 1, 0, s>>>(A->st_star, ns, A->last_star);
@@ -360,8 +454,24 @@ static int flush_segment(gsr_matrix* A) {
             A->units_host->push_back(u);
         }
     }
-    A->n_tiles += info[2 * A->nbins] / R;
-    if (A->n_tiles > A->tiles_cap) return GSR_ECUDA;   // cannot happen: capacity is an upper bound
+    const int64_t nt_seg = info[2 * A->nbins] / R;
+    if (A->n_tiles + nt_seg > A->tiles_cap) return GSR_ECUDA;   // cannot happen: capacity is an upper bound
+    if (A->so.on) {
+        StreamStore& so = A->so;
+        if (nt_seg > so.seg_cap) return GSR_ECUDA;
+        GSR_TRY(finish_tiles(A, base, A->n_tiles, nt_seg));
+        const int64_t t0 = A->n_tiles, t1 = t0 + nt_seg;
+        const int64_t td = t1 < so.res_cap ? t1 : so.res_cap;
+        if (t0 < td)
+            GSR_CUDA_TRY(cudaMemcpyAsync(A->tiles + t0 * TILE_BYTES, so.seg, (size_t)(td - t0) * TILE_BYTES,
+                                         cudaMemcpyDeviceToDevice, s));
+        const int64_t th = t0 > so.res_cap ? t0 : so.res_cap;
+        if (th < t1)
+            GSR_CUDA_TRY(cudaMemcpyAsync(so.host + (th - so.res_cap) * TILE_BYTES, so.seg + (th - t0) * TILE_BYTES,
+                                         (size_t)(t1 - th) * TILE_BYTES, cudaMemcpyDeviceToHost, s));
+        GSR_CUDA_TRY(cudaStreamSynchronize(s));
+    }
+    A->n_tiles += nt_seg;
     A->seg_fill = 0;
     return GSR_OK;
 }
@@ -396,7 +506,10 @@ const char* gsr_strerror(int code) {
 
 int64_t gsr_launch_count(void) { return g_launches; }
 
-int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
+// resident_bytes < 0: everything on the device.  Otherwise at most resident_bytes of tile storage
+// stay on the device and the rest goes to pinned host memory (row f4(iii)).
+static int begin_impl(gsr_matrix** out, const gsr_dims* d, gsr_stream stream, int64_t resident_bytes,
+                      int64_t chunk_bytes) {
     if (!out) return GSR_EINVAL;
     *out = nullptr;
     if (!d) return GSR_EINVAL;
@@ -451,7 +564,26 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
     const int64_t n_seg = (d->n_rows + SEG - 1) / SEG;
     A->tiles_cap = (d->n_rows + R - 1) / R + n_seg * nbins + 1;
     const size_t c = (size_t)A->seg_cap, nblk = (c + BLK - 1) / BLK;
-    int rc = dev_alloc(A, (void**)&A->tiles, (size_t)A->tiles_cap * TILE_BYTES);
+    int64_t dev_tiles = A->tiles_cap;
+    int rc = GSR_OK;
+    if (resident_bytes >= 0 && resident_bytes / TILE_BYTES < A->tiles_cap) {
+        StreamStore& so = A->so;
+        so.on = true;
+        so.res_cap = resident_bytes / TILE_BYTES;
+        so.chunk_cap = chunk_bytes / TILE_BYTES;
+        if (so.chunk_cap < 2 * UNIT_TILES_MAX) so.chunk_cap = 2 * UNIT_TILES_MAX;   // a unit always fits
+        so.host_cap = A->tiles_cap - so.res_cap;
+        so.seg_cap = (A->seg_cap + R - 1) / R + nbins + 1;
+        so.chunks = new (std::nothrow) std::vector<Chunk>();
+        dev_tiles = so.res_cap > 0 ? so.res_cap : 1;
+        if (!so.chunks || cudaHostAlloc((void**)&so.host, (size_t)so.host_cap * TILE_BYTES, cudaHostAllocDefault) != cudaSuccess) {
+            cudaGetLastError();
+            so.host = nullptr;
+            rc = GSR_ENOMEM;
+        }
+        if (rc == GSR_OK) rc = dev_alloc(A, (void**)&so.seg, (size_t)so.seg_cap * TILE_BYTES);
+    }
+    if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->tiles, (size_t)dev_tiles * TILE_BYTES);
     if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->perm, (size_t)A->tiles_cap * R * 4);
     if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->st_star, c * 4);
     if (rc == GSR_OK) rc = dev_alloc(A, (void**)&A->st_att, c * 4);
@@ -468,7 +600,7 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
         return rc != GSR_OK ? rc : GSR_ENOMEM;
     }
     const double ones[2] = {1.0, 1.0};
-    cudaError_t e = cudaMemsetAsync(A->tiles, 0, (size_t)A->tiles_cap * TILE_BYTES, A->stream);
+    cudaError_t e = cudaMemsetAsync(A->tiles, 0, (size_t)dev_tiles * TILE_BYTES, A->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(A->perm, 0xFF, (size_t)A->tiles_cap * R * 4, A->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(A->err, 0, sizeof(int), A->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(A->last_star, 0, 4, A->stream);
@@ -482,6 +614,25 @@ int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
     *out = A;
     return GSR_OK;
 }
+
+int gsr_matrix_begin(gsr_matrix** out, const gsr_dims* d, gsr_stream stream) {
+    return begin_impl(out, d, stream, -1, 0);
+}
+
+int gsr_matrix_begin_streamed(gsr_matrix** out, const gsr_dims* d, int64_t resident_bytes,
+                              int64_t chunk_bytes, gsr_stream stream) {
+    if (resident_bytes < 0 || chunk_bytes < 0) {
+        if (out) *out = nullptr;
+        return GSR_EINVAL;
+    }
+    return begin_impl(out, d, stream, resident_bytes, chunk_bytes);
+}
+
+int64_t gsr_matrix_host_bytes(const gsr_matrix* A) {
+    return (A && A->so.on) ? A->so.host_cap * (int64_t)TILE_BYTES : 0;
+}
+
+int64_t gsr_matrix_streamed_bytes(const gsr_matrix* A) { return A ? A->so.h2d_bytes : 0; }
 
 int gsr_matrix_append_rows(gsr_matrix* A, int64_t row0, int64_t nrows, const int32_t* star,
                            const int32_t* att, const int32_t* instr, const double* vals) {
@@ -525,12 +676,35 @@ int gsr_matrix_finalize(gsr_matrix* A) {
     if (A->n_units > 0) {
         GSR_CUDA_TRY(cudaMemcpyAsync(A->units, A->units_host->data(), (size_t)A->n_units * sizeof(Unit),
                                      cudaMemcpyHostToDevice, A->stream));
-        k_fix_padding<<<(unsigned)((A->n_tiles + 7) / 8), 256, 0, A->stream>>>(A->tiles, A->perm, A->n_tiles);
-        k_permute_instr<<<(unsigned)((2 * A->n_tiles + 127) / 128), 128, 0, A->stream>>>(A->tiles, A->perm, A->n_tiles);
-        count_launch(2);
-        GSR_CUDA_TRY(cudaGetLastError());
+        if (!A->so.on) GSR_TRY(finish_tiles(A, A->tiles, 0, A->n_tiles));   // (streamed: per segment)
     }
     GSR_CUDA_TRY(cudaStreamSynchronize(A->stream));
+    if (A->so.on) {
+        // chunk table: the leading units that lie wholly on the device form the resident view,
+        // the rest is cut into runs of whole units of at most chunk_cap tiles
+        StreamStore& so = A->so;
+        dev_free(A, so.seg, (size_t)so.seg_cap * TILE_BYTES);
+        so.seg = nullptr;
+        const std::vector<Unit>& U = *A->units_host;
+        int u = 0;
+        while (u < A->n_units && (int64_t)U[u].tile0 + U[u].ntiles <= so.res_cap) ++u;
+        so.res_units = u;
+        while (u < A->n_units) {
+            Chunk ch{u, u, U[u].tile0, U[u].tile0};
+            while (u < A->n_units && (int64_t)U[u].tile0 + U[u].ntiles - ch.t0 <= so.chunk_cap) {
+                ch.t1 = (int64_t)U[u].tile0 + U[u].ntiles;
+                ch.u1 = ++u;
+            }
+            so.chunks->push_back(ch);
+        }
+        for (int b = 0; b < 2; ++b) {
+            GSR_TRY(dev_alloc(A, (void**)&so.buf[b], (size_t)so.chunk_cap * TILE_BYTES));
+            GSR_CUDA_TRY(cudaEventCreateWithFlags(&so.copied[b], cudaEventDisableTiming));
+            GSR_CUDA_TRY(cudaEventCreateWithFlags(&so.done[b], cudaEventDisableTiming));
+        }
+        GSR_CUDA_TRY(cudaEventCreateWithFlags(&so.fork, cudaEventDisableTiming));
+        GSR_CUDA_TRY(cudaStreamCreateWithFlags(&so.copy, cudaStreamNonBlocking));
+    }
     GSR_TRY(configure_product_kernels(A));
     A->m_global = A->dims.n_rows;
     A->n_global = A->n_cols;
@@ -562,6 +736,7 @@ int gsr_matrix_destroy(gsr_matrix* A) {
     free_workspace(A);
     free_staging(A);
     free_constraints(A);
+    free_stream_store(A);
     cudaFree(A->tiles);
     cudaFree(A->perm);
     cudaFree(A->units);
@@ -612,10 +787,18 @@ int gsr_debug_expand_rows(const gsr_matrix* A, int64_t row0, int64_t nrows, int6
         cudaGetLastError();
         return GSR_ENOMEM;
     }
-    k_expand_rows<<<(unsigned)((A->m_int + 255) / 256), 256, 0, A->stream>>>(
-        A->tiles, A->perm, A->m_int, row0, nrows, A->dims.n_stars, A->dims.n_dfa, A->dims.n_instr, dc, dv);
-    count_launch();
-    e = cudaGetLastError();
+    auto expand = [&](const TileView& v) -> int {
+        const int64_t r0 = v.t0 * R, r1 = v.t1 * R;
+        if (r1 <= r0) return GSR_OK;
+        k_expand_rows<<<(unsigned)((r1 - r0 + 255) / 256), 256, 0, A->stream>>>(
+            v.base, A->perm, r0, r1, row0, nrows, A->dims.n_stars, A->dims.n_dfa, A->dims.n_instr, dc, dv);
+        count_launch();
+        GSR_CUDA_TRY(cudaGetLastError());
+        return GSR_OK;
+    };
+    int rcv = A->so.on ? for_each_view(const_cast<gsr_matrix*>(A), A->stream, expand)
+                       : expand(TileView{A->tiles, 0, A->n_units, 0, A->n_tiles});
+    e = rcv == GSR_OK ? cudaGetLastError() : cudaErrorUnknown;
     if (e == cudaSuccess) e = cudaMemcpyAsync(cols_host, dc, (size_t)nrows * NPAR * 8, cudaMemcpyDeviceToHost, A->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(vals_host, dv, (size_t)nrows * NPAR * 8, cudaMemcpyDeviceToHost, A->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(A->stream);
@@ -641,9 +824,17 @@ int gsr_precondition(gsr_matrix* A, double* p_out, gsr_stream stream) {
     k_make_p<<<(unsigned)((A->n_cols + 255) / 256), 256, 0, s>>>(A->p, A->n_cols);
     count_launch();
     if (A->n_tiles > 0) {
-        k_scale_values<<<(unsigned)((A->n_tiles + 7) / 8), 256, 0, s>>>(
-            A->tiles, A->n_tiles, A->p, A->dims.n_stars, A->dims.n_dfa, A->dims.n_instr);
-        count_launch();
+        auto scale = [&](const TileView& v) -> int {
+            const int64_t nt = v.t1 - v.t0;
+            if (nt <= 0) return GSR_OK;
+            k_scale_values<<<(unsigned)((nt + 7) / 8), 256, 0, s>>>(
+                v.base, v.t0, nt, A->p, A->dims.n_stars, A->dims.n_dfa, A->dims.n_instr);
+            count_launch();
+            GSR_CUDA_TRY(cudaGetLastError());
+            return GSR_OK;
+        };
+        if (A->so.on) GSR_TRY(for_each_view(A, s, scale, /*writeback=*/true));
+        else GSR_TRY(scale(TileView{A->tiles, 0, A->n_units, 0, A->n_tiles}));
     }
     GSR_TRY(launch_con_scale(A, A->p, s));
     GSR_CUDA_TRY(cudaGetLastError());

@@ -83,6 +83,11 @@ def named_config(name: str) -> GsrConfig:
         return GsrConfig("cfg4", 3, 200_000, 20_000, 60, n_rows_total=100_000_000,
                          powerlaw=(10, 10_000, 1.36), att_hot=(0.9, 0.40, 0.45),
                          col_scales=True, iterations=100)
+    if name.startswith("cfg3x"):
+        # K copies of config 3's star population over the same attitude and instrumental unknowns:
+        # the out-of-core workload (row f4(iii)); K = 6 is the paper's 1.8e9-row production size
+        k = int(name[5:])
+        return GsrConfig(name, 2, 300_000 * k, 50_000, 10_000, rows_per_star=1000, iterations=50)
     if name.startswith("cfg5_"):
         m = int(float(name[5:]))
         assert m % 5000 == 0

@@ -13,7 +13,10 @@ pytestmark = pytest.mark.gpu
 
 APROD_TOL = 1e-12
 X_TOL = 1e-9
-X_TOL_CAP = 1e-6      # upper bound of the sensitivity-relaxed tolerance (reading A20)
+X_TOL_CAP = 1e-4      # upper bound of the sensitivity-relaxed tolerance (reading A20): 20 x the
+                      # oracle's own one-ulp sensitivity, whose maximum over all cases is 1.6e-6
+                      # (skew_hot, k = 60: measured 4e-16 at k = 20, 5e-12 at 40, 1e-8 at 50,
+                      # 1.6e-6 at 60, 5e-11 at 70, 2e-15 at 200)
 SENS_LOG = []         # (case, fused, k, one-ulp sensitivity of the oracle's x): written to
                       # gpurun_out/lsqr_sensitivity.json at the end of the module (A20)
 
@@ -41,9 +44,9 @@ def _cases():
 CASES = _cases()
 # fixed iteration counts compared per case; STABLE ones must meet the plain 1e-9 bar
 FIXED_COUNTS = {"cfg1": (1, 3, 200), "ragged_empty_stars": (1, 3, 60), "one_instr_col": (1, 3, 60),
-                "skew_hot": (1, 3, 20, 60, 400)}
+                "skew_hot": (1, 3, 20, 60, 200, 400)}
 STABLE_COUNTS = {"cfg1": (1, 3, 200), "ragged_empty_stars": (1, 3, 60), "one_instr_col": (1, 3, 60),
-                 "skew_hot": (1, 3, 20, 400)}
+                 "skew_hot": (1, 3, 20, 200, 400)}
 
 
 class Sys:
@@ -184,7 +187,9 @@ def test_precondition_and_lsqr_parity(name, fused):
             if not converged:
                 se_tol = min(max(2 * tol, 20.0 * sens_se), 10 * X_TOL_CAP)   # same rule as for x (A20)
                 assert np.linalg.norm(se_host - ro.se) <= se_tol * np.linalg.norm(ro.se), (name, k, sens_se)
-                if tol == X_TOL:
+                # element-wise where the oracle's own se is stable too (var is a running sum: at
+                # skew_hot k = 200 it still carries the terms of the unstable stage around k = 60)
+                if tol == X_TOL and sens_se < 1e-10:
                     assert np.all(np.abs(se_host[nz] - ro.se[nz]) <= 1e-7 * ro.se[nz])
             assert abs(r.xnorm - ro.xnorm) <= tol * ro.xnorm
             assert abs(r.bnorm - ro.bnorm) <= 1e-12 * ro.bnorm
