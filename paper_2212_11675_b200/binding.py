@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libgsr_b200.so")
 
 GSR_OK, GSR_EINVAL, GSR_ENOMEM, GSR_ECUDA, GSR_ESTATE, GSR_EUNSUPPORTED, GSR_ERANGE = 0, -1, -2, -3, -4, -5, -6
 GSR_OPT_FORCE_ITNLIM, GSR_OPT_DETERMINISTIC, GSR_OPT_FUSED, GSR_OPT_FIXED_POINT = 1, 2, 3, 4
+GSR_OPT_APROD2_SPLIT = 5
 
 EXPORTS = [
     "gsr_matrix_create", "gsr_matrix_begin", "gsr_matrix_append_rows", "gsr_matrix_finalize",

@@ -51,7 +51,8 @@ __device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b)
 //            B = the terms; n = lane group = (h, axis), k = knot: the sum over the 4 knots)
 //   stage 2, four MMAs:      S[i][q'] = sum over the 4 lane groups of half (i&1) of D1_b[q'][.]
 //            with b = (i>>1)&1; rows i and i+4 are duplicates, so that every lane finds one slot
-//            sum in its own D fragment: lanes 0-15 take column 2(l&3), lanes 16-31 the next.
+//            sum in its own D fragment: of the lanes l, l ^ 16 one takes column 2(l&3), the other the
+//            next (att_slot() in gsr_internal.h says which).
 // Four independent accumulator chains in stage 1 and two in stage 2 keep the dependent depth at
 // 4 + 2 MMAs.  The MMAs run on the fp64 tensor pipe (4 cycles each per SM, measured), which is
 // otherwise idle; the 15-shuffle butterfly this replaces cost 30 LSU wavefronts per tile.
@@ -71,7 +72,7 @@ __device__ __forceinline__ double reduce_slots(const double (&p)[16], int lane) 
         dmma(s[b][0], s[b][1], a2, d1[b][0] + d1[b + 2][0]);
         dmma(s[b][0], s[b][1], a2, d1[b][1] + d1[b + 2][1]);
     }
-    return (lane >> 4) ? s[0][1] + s[1][1] : s[0][0] + s[1][0];
+    return ((lane >> 4) ^ ((lane >> 2) & 1)) ? s[0][1] + s[1][1] : s[0][0] + s[1][0];   // see att_slot()
 }
 
 // A tile is consumed in two phases so that the loads of one phase are in flight while the
@@ -383,7 +384,13 @@ __global__ void __launch_bounds__(TPB) k_aprod1(const unsigned char* __restrict_
 // CTA; astrometric block: segmented warp reduction over the star-sorted rows, one global atomic
 // per (warp, star, column); global column: register accumulation, one atomic per warp.
 // SQUARE: accumulate A[i,k]^2 instead (column sums of squares for the preconditioner).
-template <bool SQUARE, bool PERM>
+// INSTR = false: the instrumental block is left to k_aprod2_instr, which reads only the 1920
+// instrumental bytes of every tile (the split the fused iteration uses, section 5.4 of DESIGN.md):
+// the six compare-and-swap adds per row no longer share the LSU data pipe with the attitude
+// read-modify-writes, and this kernel streams 152 instead of 212 bytes per row.  With PERM the
+// scaled y of every internal row is also written to yint, so that the instrumental pass reads it
+// contiguously instead of gathering it a second time.
+template <bool SQUARE, bool PERM, bool INSTR>
 __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict__ tiles,
                                                const Unit* __restrict__ units, int n_units,
                                                int* __restrict__ counter,
@@ -391,22 +398,24 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
                                                const double* __restrict__ sy_p,
                                                const uint32_t* __restrict__ perm, int64_t S,
                                                int64_t D, int I, int win, int ws, int ncopy,
-                                               const int* __restrict__ stop) {
+                                               const int* __restrict__ stop, double* __restrict__ yint) {
     if (stop && *stop) return;
     extern __shared__ double sm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int ipad = INSTR ? (I + 1) & ~1 : 0;
     double* xi = sm;
-    double* xw = sm + ((I + 1) & ~1) + warp * 3 * ws;
-    double* ysm = sm + ((I + 1) & ~1) + NWARP * 3 * ws + warp * 32;   // y of the current tile by
+    double* xw = sm + ipad + warp * 3 * ws;
+    double* ysm = sm + ipad + NWARP * 3 * ws + warp * 32;   // y of the current tile by
                                                   // attitude slot: wide shared-memory broadcasts
                                                   // cost the LSU pipe less than shuffles
     // small I: one private copy of the instrumental accumulator per warp (copies 1.. behind the
     // y tiles), so that only lanes of the same instruction contend for an address (config 4)
-    const int ipad = (I + 1) & ~1;
     double* xcopies = sm + ipad + NWARP * 3 * ws + NWARP * 32;
-    for (int i = threadIdx.x; i < I; i += TPB) xi[i] = 0.0;
-    for (int i = threadIdx.x; i < (ncopy - 1) * ipad; i += TPB) xcopies[i] = 0.0;
-    if (ncopy > 1 && warp > 0) xi = xcopies + (warp - 1) * ipad;
+    if (INSTR) {
+        for (int i = threadIdx.x; i < I; i += TPB) xi[i] = 0.0;
+        for (int i = threadIdx.x; i < (ncopy - 1) * ipad; i += TPB) xcopies[i] = 0.0;
+        if (ncopy > 1 && warp > 0) xi = xcopies + (warp - 1) * ipad;
+    }
     const double sy = SQUARE ? 1.0 : *sy_p;
     __syncthreads();
 
@@ -429,10 +438,17 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
         if (lane == 0 && un.ntiles > 1) prefetch_l2(T + TILE_BYTES, TILE_BYTES);
         for (int t = 0; t < un.ntiles; ++t, T += TILE_BYTES) {
             RegsB r;
-            load_B(T, lane, r);
+            if (INSTR) load_B(T, lane, r);
+            else load_B_rest(T, lane, r);
             const int64_t ri = ((int64_t)un.tile0 + t) * R + lane;
             if (lane == 0 && t + PF_TILES < un.ntiles) {
-                prefetch_l2(T + PF_TILES * TILE_BYTES, TILE_BYTES);
+                // (!INSTR: the two halves of the record this kernel reads, not the instrumental part)
+                if (INSTR) {
+                    prefetch_l2(T + PF_TILES * TILE_BYTES, TILE_BYTES);
+                } else {
+                    prefetch_l2(T + PF_TILES * TILE_BYTES, OFF_INSTRV);
+                    prefetch_l2(T + PF_TILES * TILE_BYTES + OFF_GLOBV, TILE_BYTES - OFF_GLOBV);
+                }
                 if (!SQUARE && !PERM) prefetch_l2(y + ri + PF_TILES * R, R * 8);
             }
             double yv = 1.0;
@@ -440,6 +456,7 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
                 if (PERM) {
                     const uint32_t pe = __ldcs(perm + ri);
                     yv = pe != PERM_PAD ? y[pe] * sy : 0.0;
+                    if (!INSTR) yint[ri] = yv;
                 } else {
                     yv = __ldcs(y + ri) * sy;
                 }
@@ -453,15 +470,17 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
             // phase B
 #pragma unroll
             for (int k = 0; k < 5; ++k) r.as[k] = SQUARE ? r.as[k] * r.as[k] : r.as[k] * yv;
-#pragma unroll
-            for (int k = 0; k < 6; ++k) r.in[k] = SQUARE ? r.in[k] * r.in[k] : r.in[k] * yv;
             // instrumental
+            if (INSTR) {
 #pragma unroll
-            for (int k = 0; k < 6; ++k) {
-                GSR_ASSERT((int)icol_of(r.cw, k) < I);
-                smem_add_f64(xi + icol_of(r.cw, k), r.in[k]);
+                for (int k = 0; k < 6; ++k) r.in[k] = SQUARE ? r.in[k] * r.in[k] : r.in[k] * yv;
+#pragma unroll
+                for (int k = 0; k < 6; ++k) {
+                    GSR_ASSERT((int)icol_of(r.cw, k) < I);
+                    smem_add_f64(xi + icol_of(r.cw, k), r.in[k]);
+                }
+                __syncwarp();
             }
-            __syncwarp();
             // global
             g += SQUARE ? r.gl * r.gl : r.gl * yv;
             astro_mode2<false>(r.as, r.s, lane, x, S, 1.0);
@@ -478,12 +497,14 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
     g = warp_sum(g);
     if (lane == 0 && g != 0.0) atomicAdd(x + 5 * S + 3 * D + I, g);
     // flush the CTA's instrumental accumulators
-    __syncthreads();
-    double* xins = x + 5 * S + 3 * D;
-    for (int i = threadIdx.x; i < I; i += TPB) {
-        double vacc = sm[i];
-        for (int w = 1; w < ncopy; ++w) vacc += xcopies[(w - 1) * ipad + i];
-        if (vacc != 0.0) atomicAdd(xins + i, vacc);
+    if (INSTR) {
+        __syncthreads();
+        double* xins = x + 5 * S + 3 * D;
+        for (int i = threadIdx.x; i < I; i += TPB) {
+            double vacc = sm[i];
+            for (int w = 1; w < ncopy; ++w) vacc += xcopies[(w - 1) * ipad + i];
+            if (vacc != 0.0) atomicAdd(xins + i, vacc);
+        }
     }
 }
 
@@ -632,13 +653,15 @@ __global__ void __launch_bounds__(TPB) k_aprod2_instr(const unsigned char* __res
                                                      int64_t n_tiles, const double* __restrict__ y,
                                                      double* __restrict__ xins, int I, int ncopy,
                                                      const double* __restrict__ ss_p,
-                                                     const int* __restrict__ stop, int det) {
+                                                     const int* __restrict__ stop, int det,
+                                                     const double* __restrict__ sy_p) {
     if (stop && *stop) return;
     extern __shared__ double sm[];
     const int ipad = (I + 1) & ~1;
     for (int i = threadIdx.x; i < ipad * ncopy; i += TPB) sm[i] = 0.0;   // +0.0 = integer 0
     const int e = FIXED ? fixed_exp(*ss_p) : 0;   // 2^e > ||y||
-    const double scale = FIXED ? scalbn(1.0, 61 - e) : 1.0;
+    // sy_p (the stand-alone product only, never with FIXED): y is scaled by *sy_p first
+    const double scale = FIXED ? scalbn(1.0, 61 - e) : (sy_p ? *sy_p : 1.0);
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double* acc = sm + (ncopy > 1 ? warp * ipad : 0);
@@ -712,6 +735,9 @@ static size_t instr_smem(const gsr_matrix* A) {
     return (size_t)((A->dims.n_instr + 1) / 2 * 16) * instr_copies(A);
 }
 
+// shared memory of k_aprod2<., ., INSTR = false>: the windows and the y tiles only
+static int aprod2_main_smem(const gsr_matrix* A) { return NWARP * 3 * A->wstride * 8 + NWARP * 32 * 8; }
+
 template <typename K>
 static int set_smem(K kernel, int bytes) {
     GSR_CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
@@ -733,9 +759,11 @@ int configure_product_kernels(gsr_matrix* A) {
     GSR_TRY(set_smem(k_aprod1<true, false>, b));
     GSR_TRY(set_smem(k_aprod1<false, false>, b));
     GSR_TRY(set_smem(k_aprod1<false, true>, b));
-    GSR_TRY(set_smem(k_aprod2<false, false>, b));
-    GSR_TRY(set_smem(k_aprod2<false, true>, b));
-    GSR_TRY(set_smem(k_aprod2<true, false>, b));
+    GSR_TRY(set_smem(k_aprod2<false, false, true>, b));
+    GSR_TRY(set_smem(k_aprod2<false, true, true>, b));
+    GSR_TRY(set_smem(k_aprod2<true, false, true>, b));
+    GSR_TRY(set_smem(k_aprod2<false, false, false>, aprod2_main_smem(A)));
+    GSR_TRY(set_smem(k_aprod2<false, true, false>, aprod2_main_smem(A)));
     GSR_TRY(set_smem(k_fused<false>, A->smem_fused));
     GSR_TRY(set_smem(k_fused<true>, A->smem_fused));
     GSR_TRY(set_smem(k_aprod2_instr<false>, (int)instr_smem(A)));
@@ -755,7 +783,15 @@ int configure_product_kernels(gsr_matrix* A) {
         A->grid_instr = A->sm_count * nb;
     }
     A->grid1 = A->sm_count * resident_ctas(k_aprod1<true, false>, A);
-    A->grid2 = A->sm_count * resident_ctas(k_aprod2<false, false>, A);
+    A->grid2 = A->sm_count * resident_ctas(k_aprod2<false, false, true>, A);
+    {
+        int nb = 1;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_aprod2<false, false, false>, TPB, aprod2_main_smem(A)) != cudaSuccess || nb < 1) {
+            cudaGetLastError();
+            nb = 1;
+        }
+        A->grid2_main = A->sm_count * nb;
+    }
     return GSR_OK;   // (a launch over few units takes fewer CTAs: grid_for)
 }
 
@@ -814,18 +850,49 @@ static int aprod2_view(const gsr_matrix* A, const TileView& v, const double* y, 
     if (nu <= 0) return GSR_OK;
     const int64_t S = A->dims.n_stars, D = A->dims.n_dfa;
     const int I = (int)A->dims.n_instr;
-    const int grid = grid_for(A->grid2, nu);
     const Unit* un = A->units + v.u0;
     GSR_TRY(reset_counter(A, s));
-    if (square)
-        k_aprod2<true, false><<<grid, TPB, A->smem_bytes, s>>>(
-            v.base, un, nu, A->unit_counter, nullptr, x, nullptr, nullptr, S, D, I, A->win, A->wstride, instr_copies(A), nullptr);
-    else if (perm)
-        k_aprod2<false, true><<<grid, TPB, A->smem_bytes, s>>>(
-            v.base, un, nu, A->unit_counter, y, x, sy, perm, S, D, I, A->win, A->wstride, instr_copies(A), stop);
-    else
-        k_aprod2<false, false><<<grid, TPB, A->smem_bytes, s>>>(
-            v.base, un, nu, A->unit_counter, y, x, sy, nullptr, S, D, I, A->win, A->wstride, instr_copies(A), stop);
+    if (square) {
+        k_aprod2<true, false, true><<<grid_for(A->grid2, nu), TPB, A->smem_bytes, s>>>(
+            v.base, un, nu, A->unit_counter, nullptr, x, nullptr, nullptr, S, D, I, A->win, A->wstride, instr_copies(A), nullptr, nullptr);
+        count_launch();
+        GSR_CUDA_TRY(cudaGetLastError());
+        return GSR_OK;
+    }
+    if (!A->opt_aprod2_split) {
+        if (perm)
+            k_aprod2<false, true, true><<<grid_for(A->grid2, nu), TPB, A->smem_bytes, s>>>(
+                v.base, un, nu, A->unit_counter, y, x, sy, perm, S, D, I, A->win, A->wstride, instr_copies(A), stop, nullptr);
+        else
+            k_aprod2<false, false, true><<<grid_for(A->grid2, nu), TPB, A->smem_bytes, s>>>(
+                v.base, un, nu, A->unit_counter, y, x, sy, nullptr, S, D, I, A->win, A->wstride, instr_copies(A), stop, nullptr);
+        count_launch();
+        GSR_CUDA_TRY(cudaGetLastError());
+        return GSR_OK;
+    }
+    // two launches (default): everything but the instrumental block, then the instrumental pass
+    // over the instrumental planes alone (fp64 adds: a caller's y has no norm bound to scale by)
+    const int grid = grid_for(A->grid2_main, nu);
+    const int smem = aprod2_main_smem(A);
+    const double* yi = y + v.t0 * R;   // internal order: the view's slice of y
+    const double* syi = sy;
+    if (perm) {
+        if (!A->yint) return GSR_ESTATE;
+        k_aprod2<false, true, false><<<grid, TPB, smem, s>>>(
+            v.base, un, nu, A->unit_counter, y, x, sy, perm, S, D, I, A->win, A->wstride, 1, stop, A->yint);
+        yi = A->yint + v.t0 * R;       // already scaled
+        syi = nullptr;
+    } else {
+        k_aprod2<false, false, false><<<grid, TPB, smem, s>>>(
+            v.base, un, nu, A->unit_counter, y, x, sy, nullptr, S, D, I, A->win, A->wstride, 1, stop, nullptr);
+    }
+    count_launch();
+    GSR_CUDA_TRY(cudaGetLastError());
+    const int64_t nt = v.t1 - v.t0;
+    const int64_t need = (nt + NWARP - 1) / NWARP;
+    const int gi = A->grid_instr < need ? A->grid_instr : (int)need;
+    k_aprod2_instr<false><<<gi, TPB, instr_smem(A), s>>>(
+        v.base + v.t0 * TILE_BYTES, nt, yi, x + A->off_instr, I, instr_copies(A), nullptr, stop, 0, syi);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;
@@ -865,10 +932,10 @@ static int instr_view(const gsr_matrix* A, const TileView& v, const double* u, d
     const unsigned char* T0 = v.base + v.t0 * TILE_BYTES;
     if (fixed)
         k_aprod2_instr<true><<<grid, TPB, instr_smem(A), s>>>(
-            T0, nt, u + v.t0 * R, t + A->off_instr, (int)A->dims.n_instr, instr_copies(A), ss, stop, det);
+            T0, nt, u + v.t0 * R, t + A->off_instr, (int)A->dims.n_instr, instr_copies(A), ss, stop, det, nullptr);
     else
         k_aprod2_instr<false><<<grid, TPB, instr_smem(A), s>>>(
-            T0, nt, u + v.t0 * R, t + A->off_instr, (int)A->dims.n_instr, instr_copies(A), nullptr, stop, 0);
+            T0, nt, u + v.t0 * R, t + A->off_instr, (int)A->dims.n_instr, instr_copies(A), nullptr, stop, 0, nullptr);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;
@@ -931,6 +998,11 @@ int gsr_aprod1(const gsr_matrix* A, const double* x_dev, double* y_dev, gsr_stre
 int gsr_aprod2(const gsr_matrix* A, const double* y_dev, double* x_dev, gsr_stream stream) {
     if (!A || !x_dev || (!y_dev && A->dims.n_rows > 0)) return GSR_EINVAL;
     if (A->state != 1) return GSR_ESTATE;
+    if (A->opt_aprod2_split && !A->yint && A->m_int > 0) {
+        // scratch of the split form (a cache behind a logically const handle): y in internal order
+        gsr_matrix* Am = const_cast<gsr_matrix*>(A);
+        GSR_TRY(dev_alloc(Am, (void**)&Am->yint, (size_t)A->m_int * 8));
+    }
     GSR_TRY(launch_aprod2(A, y_dev, x_dev, A->coef_one, nullptr, A->perm, (cudaStream_t)stream));
     return launch_con_aprod2(A, y_dev + A->dims.n_rows, x_dev, A->coef_one, nullptr, (cudaStream_t)stream);
 }

@@ -91,10 +91,11 @@ int gsr_comm_destroy(gsr_comm* c) {
 int gsr_matrix_set_comm(gsr_matrix* A, gsr_comm* c, int64_t n_rows_global, int64_t n_cols_global) {
     if (!A) return GSR_EINVAL;
     if (A->state != 1 || A->p != nullptr || A->ws.st != nullptr) return GSR_ESTATE;   // before precondition / solve
-    if (c && A->n_con > 0) return GSR_EUNSUPPORTED;
-    if (c && (n_rows_global < A->dims.n_rows || n_cols_global < A->n_cols)) return GSR_EINVAL;
+    // constraint rows (row f3) stay with the rank whose handle they were given to, in LOCAL
+    // column numbering; n_rows_global counts them too (every rank's)
+    if (c && (n_rows_global < A->dims.n_rows + A->n_con || n_cols_global < A->n_cols)) return GSR_EINVAL;
     A->comm = c;
-    A->m_global = c ? n_rows_global : A->dims.n_rows;
+    A->m_global = c ? n_rows_global : A->dims.n_rows + A->n_con;
     A->n_global = c ? n_cols_global : A->n_cols;
     return GSR_OK;
 }

@@ -173,10 +173,9 @@ int gsr_matrix_set_constraints(gsr_matrix* A, int64_t n_con, const int64_t* row_
                                const int32_t* col_hd, const double* val_hd) {
     if (!A || n_con < 0) return GSR_EINVAL;
     if (A->state != 1 || A->p != nullptr || A->ws.st != nullptr) return GSR_ESTATE;   // before precondition / solve
-    if (A->comm) return GSR_EUNSUPPORTED;
     if (n_con > 0 && !row_ptr_hd) return GSR_EINVAL;
     free_constraints(A);
-    A->m_global = A->dims.n_rows;
+    if (!A->comm) A->m_global = A->dims.n_rows;   // (sharded: gsr_matrix_set_comm was told the total)
     if (n_con == 0) return GSR_OK;
     std::vector<int64_t> ptr((size_t)n_con + 1);
     GSR_CUDA_TRY(cudaMemcpy(ptr.data(), row_ptr_hd, ptr.size() * 8, cudaMemcpyDefault));
@@ -206,7 +205,7 @@ int gsr_matrix_set_constraints(gsr_matrix* A, int64_t n_con, const int64_t* row_
         free_constraints(A);
         return GSR_ECUDA;
     }
-    A->m_global = A->dims.n_rows + n_con;
+    if (!A->comm) A->m_global = A->dims.n_rows + n_con;
     return GSR_OK;
 }
 

@@ -69,9 +69,14 @@ constexpr int TILE_BYTES = 6784;                    // 53 * 128
 static_assert(OFF_IPERM + R * 2 <= TILE_BYTES && TILE_BYTES % 128 == 0, "tile record");
 // attitude slot 16*h + q of home lane l.  The mapping is the one the MMA reduction of aprod1
 // delivers its sums in (reduce_slots() in gsr_aprod.cu): lane l receives the sum of slot
-//   h = bit 2 of l,  q = 8 * (bit 3 of l) + 2 * (l & 3) + (bit 4 of l).
+//   h = bit 2 of l,  q = 8 * (bit 3 of l) + 2 * (l & 3) + (bit 4 of l XOR h).
+// (A lane's MMA fragment holds the sums of slots (h, q) and (h, q ^ 1); which of the two lanes l,
+// l ^ 16 takes which is free.  With the XOR the 16 lanes of a half-warp own slots 16h + q that
+// are distinct modulo 16, so that the per-tile store of u_hat by slot, ysm[att_slot(lane)], is
+// free of shared-memory bank conflicts.)
 __host__ __device__ inline int att_slot(int l) {
-    return 16 * ((l >> 2) & 1) + 8 * ((l >> 3) & 1) + 2 * (l & 3) + (l >> 4);
+    const int h = (l >> 2) & 1;
+    return 16 * h + 8 * ((l >> 3) & 1) + 2 * (l & 3) + ((l >> 4) ^ h);
 }
 // byte offset of coefficient k (paper order) of home lane lr inside a tile record
 __host__ __device__ inline int val_offset(int k, int lr) {
@@ -209,6 +214,7 @@ struct gsr_matrix {
     int smem_fused;                 // ... of the fused iteration kernel (two windows per warp)
     int ctas_per_sm;                // resident product CTAs per SM the shared-memory plan allows
     int grid1, grid2;               // persistent grids of aprod1 / aprod2
+    int grid2_main;                 // ... of aprod2 without its instrumental block (split form)
     int grid_fused, grid_instr;     // ... of the fused iteration kernel / its instrumental pass
     int64_t tiles_cap, n_tiles;     // allocated / used tiles
     int64_t m_int;                  // n_tiles * R, length of internal-order vectors
@@ -236,6 +242,9 @@ struct gsr_matrix {
     int opt_two_pass;               // 1: aprod1 + aprod2 per iteration instead of the fused pass
     int opt_no_fixed;               // 1: fp64 atomics in the instrumental pass even when scaled
     int opt_deterministic;          // 1: no floating-point atomics anywhere in the iteration
+    int opt_aprod2_split;           // 1: aprod2 = main launch + instrumental pass (default 0: one sweep)
+    double* yint;                   // [m_int] scaled y in internal order, written by the main
+                                    // launch of a caller-order gsr_aprod2 (allocated on first use)
     double damp;                    // gsr_lsqr_set_damp (row f4); 0 = the paper's undamped LSQR
     int64_t n_con, con_nnz;         // row f3: constraint rows (CSR) appended below the observations
     int64_t* con_ptr;

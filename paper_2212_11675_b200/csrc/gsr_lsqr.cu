@@ -419,7 +419,8 @@ void free_workspace(gsr_matrix* A) {
 // together, k_aprod2_instr adds the instrumental block of t, k_vnew forms v = t/beta - beta v.
 // Two-pass form (GSR_OPT_FUSED = 0): aprod1, then aprod2 on the pre-scaled v.
 static int kernels_per_iteration(const gsr_matrix* A) {
-    return (A->opt_two_pass ? 8 : (A->comm ? 10 : 8)) + (A->n_con > 0 ? 2 : 0) + (A->opt_deterministic ? 1 : 0);
+    return (A->opt_two_pass ? (A->opt_aprod2_split ? 9 : 8) : (A->comm ? 10 : 8)) + (A->n_con > 0 ? 2 : 0) +
+           (A->opt_deterministic ? 1 : 0);
 }
 
 static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
@@ -467,8 +468,12 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
         // row-sharded: the same sequence with the paper's two reductions (Alg. 3 lines 12, 16)
         // as NCCL all-reduces inside the graph.  #1: replicated slice of t = A^T u_hat, with the
         // local sum of u_hat^2 riding in t[n]; #2: the distributed parts of ||v||^2 and ||w||^2.
+        // Constraint rows belong to the rank that was given them (local column numbering): their
+        // part of u_hat^2 and of t joins the local sums before the all-reduce.
         GSR_TRY(launch_fused(A, W.v, W.u, &W.st->ca, W.part_u, W.t, &W.st->stop, nullptr, s));
-        k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units, W.t + n, &W.st->stop);
+        GSR_TRY(launch_con_aprod1(A, W.v, W.u + A->m_int, &W.st->ca, W.part_u + A->n_units, &W.st->stop, s));
+        GSR_TRY(launch_con_aprod2(A, W.u + A->m_int, W.t, A->coef_one, &W.st->stop, s));
+        k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units + ncp, W.t + n, &W.st->stop);
         GSR_TRY(launch_aprod2_instr(A, W.u, W.t, W.t + n, &W.st->stop, 0, s));   // local ||u_hat||^2
         GSR_TRY(comm_allreduce_sum(A->comm, W.t + split, (size_t)(n - split + 1), s));
         k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.t + n, 1);
@@ -490,7 +495,7 @@ static int build_graph(gsr_matrix* A, cudaStream_t s) {
     // form, the communicator, the constraint rows, and the variant of the instrumental pass
     // (fixed point needs a scaled matrix and GSR_OPT_FIXED_POINT)
     const int key = (A->opt_two_pass ? 1 : 0) | (A->p != nullptr ? 2 : 0) | (A->opt_no_fixed ? 4 : 0) |
-                    (A->n_con > 0 ? 8 : 0) | (A->opt_deterministic ? 16 : 0);
+                    (A->n_con > 0 ? 8 : 0) | (A->opt_deterministic ? 16 : 0) | (A->opt_aprod2_split ? 32 : 0);
     if (W.graph_valid && W.graph_stream == s && W.graph_key == key && W.graph_comm == (void*)A->comm &&
         W.graph_ncon == A->n_con)
         return GSR_OK;
@@ -550,7 +555,6 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     GSR_TRY(ensure_workspace(A));
     const int64_t m = A->dims.n_rows + A->n_con, n = A->n_cols;   // b: observations then constraints
     memset(result, 0, sizeof(*result));
-    if (A->comm && A->n_con > 0) return GSR_EUNSUPPORTED;
     if (A->so.on && (A->comm || A->opt_deterministic)) return GSR_EUNSUPPORTED;
     // deterministic mode: fused iteration on a column-scaled matrix (the range bound of its
     // fixed-point sums needs unit column norms), no constraint rows, one GPU
@@ -586,8 +590,10 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     if (A->comm && A->opt_two_pass) return GSR_EUNSUPPORTED;
     const int64_t split = A->comm ? A->off_att : 0;
     k_gather_sumsq<<<NB_N, TB_N, 0, s>>>(b_dev, A->perm, W.u, A->m_int, W.part_u);
-    if (A->comm) {   // ||b||^2 over all row shards
-        k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, NB_N, W.red + 2, nullptr);
+    if (A->comm) {   // ||b||^2 over all row shards (each with the constraint rows it owns)
+        if (A->n_con > 0)
+            GSR_TRY(launch_con_copy_sumsq(A, b_dev + A->dims.n_rows, W.u + A->m_int, W.part_u + NB_N, s));
+        k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, NB_N + (A->n_con > 0 ? 1 : 0), W.red + 2, nullptr);
         GSR_TRY(comm_allreduce_sum(A->comm, W.red + 2, 1, s));
         k_scalar_init1<<<1, 1024, 0, s>>>(W.st, W.red + 2, 1);
         count_launch();

@@ -744,6 +744,7 @@ int gsr_matrix_destroy(gsr_matrix* A) {
     cudaFree(A->seg_bin_rows);
     cudaFree(A->last_star);
     cudaFree(A->p);
+    cudaFree(A->yint);
     cudaFree(A->err);
     cudaFree(A->coef_one);
     cudaGetLastError();
@@ -768,6 +769,7 @@ int gsr_set_option(gsr_matrix* A, int key, int64_t value) {
         case GSR_OPT_DETERMINISTIC: A->opt_deterministic = value != 0; return GSR_OK;
         case GSR_OPT_FUSED: A->opt_two_pass = value == 0; return GSR_OK;
         case GSR_OPT_FIXED_POINT: A->opt_no_fixed = value == 0; return GSR_OK;
+        case GSR_OPT_APROD2_SPLIT: A->opt_aprod2_split = value != 0; return GSR_OK;
         default: return GSR_EINVAL;
     }
 }

@@ -118,6 +118,46 @@ def test_gpu_constraints_parity(fused, n_con, nnz_row):
 
 
 @pytest.mark.gpu
+def test_gpu_constraints_on_a_row_shard_world_1_nccl():
+    """Rows e + f3 together: constraint rows on a handle that carries a communicator (one rank:
+    the all-reduces are the identity, the sharded kernel sequence with the constraint launches
+    inside the graph is what runs).  The N > 1 algebra is tests/test_sharding_gloo.py's."""
+    import torch
+    from paper_2212_11675_b200 import binding as g
+    cfg = inputs.scaled(inputs.named_config("cfg1"), 10, "cfg1/10")
+    star, att, instr, vals = inputs.gen_all(cfg)
+    from oracle import gsr_oracle
+    o = gsr_oracle.from_torch(cfg, star, att, instr, vals)
+    n_con = 9
+    C, ptr, col, val = _constraints(o.n, n_con, 60, 5)
+    o.set_constraints(ptr, col, val)
+    A = g.GsrMatrix.create(cfg, star.cuda(), att.cuda(), instr.cuda(), vals.cuda())
+    try:
+        comm = g.gsr_comm_create(0, 1, g.gsr_comm_unique_id())
+        g.gsr_matrix_set_comm(A.h, comm, cfg.n_rows + n_con, cfg.n_cols)
+        g.gsr_matrix_set_constraints(A.h, n_con, ptr, col, val)       # after set_comm: both orders are legal
+        rng = np.random.default_rng(3)
+        b = o.aprod1(inputs.x_true(cfg).numpy(), 1e-3 * rng.standard_normal(o.m_total))
+        p_ref = o.precondition()
+        p = torch.empty(o.n, dtype=torch.float64, device="cuda")
+        g.gsr_precondition(A.h, p)
+        assert np.allclose(p.cpu().numpy(), p_ref, rtol=1e-13)
+        g.gsr_set_option(A.h, g.GSR_OPT_FORCE_ITNLIM, 1)
+        xs = torch.empty(o.n, dtype=torch.float64, device="cuda")
+        for k in (1, 10):
+            r = g.gsr_lsqr_solve(A.h, torch.from_numpy(b).cuda(), xs, k)
+            ro = o.lsqr(b, k, force_itnlim=True, want_se=True)
+            assert (r.istop, r.itn) == (ro.istop, ro.itn) == (7, k)
+            assert np.linalg.norm(xs.cpu().numpy() - ro.x) <= 1e-9 * np.linalg.norm(ro.x)
+            assert abs(r.rnorm - ro.rnorm) <= 1e-9 * ro.rnorm and abs(r.bnorm - ro.bnorm) <= 1e-12 * ro.bnorm
+            se = np.empty(o.n)
+            g.gsr_lsqr_standard_errors(A.h, se)
+            assert np.linalg.norm(se - ro.se) <= 1e-8 * np.linalg.norm(ro.se)
+    finally:
+        A.close()
+
+
+@pytest.mark.gpu
 def test_gpu_constraints_argument_errors():
     import torch
     from paper_2212_11675_b200 import binding as g

@@ -92,13 +92,23 @@ def test_aprod1_parity(sysm):
     assert np.all(err <= APROD_TOL * scale), float((err / scale).max())
 
 
-def test_aprod2_parity(sysm):
+@pytest.mark.parametrize("split", [1, 0])
+def test_aprod2_parity(sysm, split):
+    """Algorithm 2 through the C ABI, as one sweep over all four blocks (default)
+    and as two launches (GSR_OPT_APROD2_SPLIT = 1: the instrumental block in a pass of its own)."""
     b = _binding()
     y = inputs.random_vector(sysm.cfg, 3, sysm.m)
     x0 = inputs.random_vector(sysm.cfg, 4, sysm.n)
     x_ref, scale = sysm.o.aprod2(y.numpy(), x0.numpy(), want_scale=True)
     xd = x0.cuda()
-    b.gsr_aprod2(sysm.A.h, y.cuda(), xd)
+    b.gsr_set_option(sysm.A.h, b.GSR_OPT_APROD2_SPLIT, split)
+    try:
+        n0 = b.gsr_launch_count()
+        b.gsr_aprod2(sysm.A.h, y.cuda(), xd)
+        launches = b.gsr_launch_count() - n0
+    finally:
+        b.gsr_set_option(sysm.A.h, b.GSR_OPT_APROD2_SPLIT, 0)
+    assert launches == (2 if split else 1) or sysm.m == 0, launches   # the form asked for really ran
     err = np.abs(xd.cpu().numpy() - x_ref)
     assert np.all(err <= APROD_TOL * np.maximum(scale, 1e-300)), float((err / scale).max())
     # untouched columns (empty stars, unused instrumental columns) keep x0 exactly
@@ -194,8 +204,15 @@ def test_precondition_and_lsqr_parity(name, fused):
             assert abs(r.xnorm - ro.xnorm) <= tol * ro.xnorm
             assert abs(r.bnorm - ro.bnorm) <= 1e-12 * ro.bnorm
             if tol == X_TOL and (ro.itn_natural == 0 or k < ro.itn_natural):      # reading A18
-                assert abs(r.anorm - ro.anorm) <= 1e-9 * ro.anorm
-                assert abs(r.acond - ro.acond) <= 1e-9 * ro.acond
+                # anorm and acond are RUNNING sums over alpha_k, beta_k and ||w_k||/rho_k: like var
+                # they keep the terms of an unstable stage the iterate itself has left behind
+                # (skew_hot: around k = 60, still in the sums at k = 200), so they get the same rule
+                # as x -- 1e-9 where the oracle is that stable under a one-ulp change of b, else
+                # 20x its own sensitivity, capped at reading A18's post-convergence bound
+                sens_an = abs(ru.anorm - ro.anorm) / ro.anorm
+                sens_ac = abs(ru.acond - ro.acond) / ro.acond
+                assert abs(r.anorm - ro.anorm) <= min(max(1e-9, 20.0 * sens_an), 1e-2) * ro.anorm, (name, k, sens_an)
+                assert abs(r.acond - ro.acond) <= min(max(1e-9, 20.0 * sens_ac), 1e-2) * ro.acond, (name, k, sens_ac)
             else:   # past convergence alpha_k, beta_k are rounding noise: anorm loosely, acond not at all
                 assert abs(r.anorm - ro.anorm) <= 1e-2 * ro.anorm
             if ro.itn_natural:

@@ -59,7 +59,21 @@ def _allsum(a):
     return t.numpy().reshape(np.shape(a))
 
 
-def _sharded_lsqr(rank, world, port, k_fixed, fused, out):
+def _con_rows(cfg, n_con=4, nnz=9, seed=7):
+    """Constraint rows (row f3) on the replicated slice only -- attitude, instrumental and global
+    columns -- in GLOBAL column numbering: (row_ptr, col, val)."""
+    rng = np.random.default_rng(seed)
+    rep0 = 5 * cfg.n_stars
+    ptr, col, val = [0], [], []
+    for _ in range(n_con):
+        c = np.sort(rng.choice(cfg.n_cols - rep0, nnz, replace=False)) + rep0
+        col.extend(c.tolist())
+        val.extend(rng.standard_normal(nnz).tolist())
+        ptr.append(len(col))
+    return np.array(ptr, dtype=np.int64), np.array(col, dtype=np.int32), np.array(val)
+
+
+def _sharded_lsqr(rank, world, port, k_fixed, fused, out, with_con=False):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
@@ -76,13 +90,22 @@ def _sharded_lsqr(rank, world, port, k_fixed, fused, out):
         xt = inputs.x_true(cfg).numpy()
         xt_loc = np.concatenate([xt[sh.astro_offset_global:sh.astro_offset_global + 5 * sh.n_stars_local],
                                  np.zeros(ro - 5 * sh.n_stars_local), xt[sh.replicated_offset_global:]])
-        b = o.aprod1(xt_loc, inputs.noise(cfg, 0, cfg.n_rows).numpy()[rows])
+        noise = inputs.noise(cfg, 0, cfg.n_rows).numpy()[rows]
+        if with_con and rank == 0:
+            # rank 0 owns every constraint row (local numbering: replicated columns shift by the
+            # difference of the two astrometric blocks); its m-vectors get n_con more entries
+            ptr, col, val = _con_rows(cfg)
+            o.set_constraints(ptr, (col - 5 * cfg.n_stars + ro).astype(np.int32), val)
+            noise = np.concatenate([noise, np.zeros(len(ptr) - 1)])
+        b = o.aprod1(xt_loc, noise)
         # preconditioner: column sums of squares, replicated slice summed over the ranks
         q = o.colsumsq()
         q[ro:] = _allsum(q[ro:])
         p = np.where(q > 0, 1.0 / np.sqrt(np.where(q > 0, q, 1.0)), 1.0)
         cols, _ = o.expand_rows()
         o.values[:] = o.values * p[cols]
+        if o.n_con:
+            o.con_val[:] = o.con_val * p[o.con_col]
 
         def norm2(v_loc):        # distributed slice summed over ranks + replicated slice once
             return float(_allsum(np.array([np.dot(v_loc[:ro], v_loc[:ro])]))[0] + np.dot(v_loc[ro:], v_loc[ro:]))
@@ -140,17 +163,22 @@ def _free_port():
 
 
 @pytest.mark.timeout(300)
-@pytest.mark.parametrize("fused", [True, False])
-def test_sharded_lsqr_two_gloo_ranks_matches_single_process_oracle(fused):
+@pytest.mark.parametrize("fused,with_con", [(True, False), (False, False), (True, True)])
+def test_sharded_lsqr_two_gloo_ranks_matches_single_process_oracle(fused, with_con):
     k = 12
     world = 2
     mgr = mp.get_context("spawn").Manager()
     out = mgr.dict()
-    mp.spawn(_sharded_lsqr, args=(world, _free_port(), k, fused, out), nprocs=world, join=True)
+    mp.spawn(_sharded_lsqr, args=(world, _free_port(), k, fused, out, with_con), nprocs=world, join=True)
     cfg = _cfg()
     star, att, instr, vals = [t.numpy() for t in inputs.gen_all(cfg)]
     o = make_oracle(cfg, star, att, instr, vals)
-    b = o.aprod1(inputs.x_true(cfg).numpy(), inputs.noise(cfg, 0, cfg.n_rows).numpy())
+    noise = inputs.noise(cfg, 0, cfg.n_rows).numpy()
+    if with_con:      # the same rows below the observations of the unsharded system
+        ptr, col, val = _con_rows(cfg)
+        o.set_constraints(ptr, col, val)
+        noise = np.concatenate([noise, np.zeros(len(ptr) - 1)])
+    b = o.aprod1(inputs.x_true(cfg).numpy(), noise)
     o.precondition()
     ref = o.lsqr(b, k, force_itnlim=True)
     shards = [out[r][0] for r in range(world)]
