@@ -369,6 +369,7 @@ def main():
     barrier()
     launches = g.gsr_launch_count() - l0
     streamed_bytes = g.gsr_matrix_streamed_bytes(h) - sb0
+    while_graph = g.gsr_debug_while_graph(h)
     ms_solve = e0.elapsed_time(e1)            # whole call: initialisation + K iterations + x
     ms = g.gsr_lsqr_last_loop_ms(h)           # exactly the K iterations (CUDA events on the stream)
     assert 0.0 < ms <= ms_solve
@@ -424,6 +425,8 @@ def main():
                     "h2d_bytes_per_step": 8 * m / K, "d2h_bytes_per_step": (8 * n + 80) / K,
                     "note": "gsr_lsqr_solve with pinned host b and host x; matrix resident"},
             "gpu_launches": int(launches),
+            "loop": ("one launch of a conditional-WHILE CUDA graph for all K iterations"
+                     if while_graph else "one CUDA graph launch per iteration"),
             "clocks": clocks,
             "roofline": {"bound": "hbm", "kernel": dom[0], "achieved": dom[1], "peak": peak,
                          "unit": "GB/s", "frac": dom[1] / peak, "traffic": traffic,

@@ -246,7 +246,7 @@ enum {
                                  the fused iteration accumulates in exact 64-bit fixed point
                                  with native 32-bit shared atomics (order-independent sums,
                                  normwise error <= n_j 2^-62 ||u|| per column); 0: fp64 atomics  */
-    GSR_OPT_APROD2_SPLIT = 5  /* 0 (default): aprod2 (gsr_aprod2 and the two-pass iteration) is one
+    GSR_OPT_APROD2_SPLIT = 5, /* 0 (default): aprod2 (gsr_aprod2 and the two-pass iteration) is one
                                  launch that does all four blocks (Algorithm 2 as one sweep);
                                  1: two launches -- astrometric + attitude + global blocks over
                                  152 B of every row, then the instrumental block over the
@@ -254,6 +254,14 @@ enum {
                                  before).  Measured on B200: the sweep is 7 %
                                  faster at 10 000 instrumental columns in internal row order,
                                  the split 28 % faster through the caller-order API at 60        */
+    GSR_OPT_WHILE_GRAPH = 6   /* 1 (default): the whole iteration loop of gsr_lsqr_solve is ONE CUDA
+                                 graph launch -- a conditional WHILE node whose body is the
+                                 iteration and whose condition a device kernel sets from the
+                                 stop flag -- so neither the stop decision nor a launch crosses
+                                 to the host between iterations (matters for small systems:
+                                 config 1 is launch-bound); 0, with a communicator, or on a
+                                 streamed handle: one graph launch per iteration, the stop flag
+                                 polled from pinned memory every 32 (fixed-count mode: 256)    */
 };
 int gsr_set_option(gsr_matrix* A, int key, int64_t value);
 
@@ -297,6 +305,10 @@ double gsr_lsqr_last_loop_ms(const gsr_matrix* A);
  * communicator) is part of the graph's cache key; tests use this to check that changing such an
  * option between two solves really re-captures. */
 int64_t gsr_debug_graph_builds(const gsr_matrix* A);
+
+/* 1 if the iteration loop of the last gsr_lsqr_solve on this handle ran as ONE launch of the
+ * conditional-WHILE graph (GSR_OPT_WHILE_GRAPH), 0 if it ran as one graph launch per iteration. */
+int gsr_debug_while_graph(const gsr_matrix* A);
 
 /* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */
 int64_t gsr_launch_count(void);

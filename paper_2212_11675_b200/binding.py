@@ -15,14 +15,14 @@ LIB_PATH = os.path.join(_HERE, "libgsr_b200.so")
 
 GSR_OK, GSR_EINVAL, GSR_ENOMEM, GSR_ECUDA, GSR_ESTATE, GSR_EUNSUPPORTED, GSR_ERANGE = 0, -1, -2, -3, -4, -5, -6
 GSR_OPT_FORCE_ITNLIM, GSR_OPT_DETERMINISTIC, GSR_OPT_FUSED, GSR_OPT_FIXED_POINT = 1, 2, 3, 4
-GSR_OPT_APROD2_SPLIT = 5
+GSR_OPT_APROD2_SPLIT, GSR_OPT_WHILE_GRAPH = 5, 6
 
 EXPORTS = [
     "gsr_matrix_create", "gsr_matrix_begin", "gsr_matrix_append_rows", "gsr_matrix_finalize",
     "gsr_matrix_destroy", "gsr_matrix_dims", "gsr_matrix_device_bytes", "gsr_aprod1",
     "gsr_aprod2", "gsr_precondition", "gsr_lsqr_solve", "gsr_set_option", "gsr_strerror",
     "gsr_debug_expand_rows", "gsr_time_product", "gsr_launch_count", "gsr_lsqr_standard_errors", "gsr_lsqr_last_loop_ms", "gsr_lsqr_set_damp",
-    "gsr_debug_fused_pass", "gsr_debug_graph_builds", "gsr_matrix_set_constraints", "gsr_comm_unique_id", "gsr_comm_create", "gsr_comm_destroy", "gsr_matrix_set_comm",
+    "gsr_debug_fused_pass", "gsr_debug_graph_builds", "gsr_debug_while_graph", "gsr_matrix_set_constraints", "gsr_comm_unique_id", "gsr_comm_create", "gsr_comm_destroy", "gsr_matrix_set_comm",
     "gsr_matrix_begin_streamed", "gsr_matrix_host_bytes", "gsr_matrix_streamed_bytes",
 ]
 
@@ -110,6 +110,8 @@ def lib():
         L.gsr_debug_fused_pass.argtypes = [vp, vp, dbl, vp, vp, vp]
         L.gsr_debug_graph_builds.argtypes = [vp]
         L.gsr_debug_graph_builds.restype = i64
+        L.gsr_debug_while_graph.argtypes = [vp]
+        L.gsr_debug_while_graph.restype = C.c_int
         _lib = L
     return _lib
 
@@ -299,6 +301,10 @@ def gsr_debug_fused_pass(h, x_dev, ca, y_dev, t_dev, stream=None):
 
 def gsr_debug_graph_builds(h) -> int:
     return int(lib().gsr_debug_graph_builds(h))
+
+
+def gsr_debug_while_graph(h) -> int:
+    return int(lib().gsr_debug_while_graph(h))
 
 
 def gsr_launch_count() -> int:

@@ -30,6 +30,13 @@
 #define GSR_ASSERT(c) ((void)0)
 #endif
 
+#ifndef GSR_ASTRO_CAP
+#define GSR_ASTRO_CAP 0
+#endif
+#ifndef GSR_LDQ
+#define GSR_LDQ ".cs"
+#endif
+
 namespace gsr {
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -100,27 +107,27 @@ __device__ __forceinline__ uint32_t icol_of(const uint32_t (&cw)[3], int j) {
 // ahead of their first use).
 __device__ __forceinline__ double ld_stream_f64(const void* p) {
     double v;
-    asm volatile("ld.global.cs.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    asm volatile("ld.global" GSR_LDQ ".f64 %0, [%1];" : "=d"(v) : "l"(p));
     return v;
 }
 __device__ __forceinline__ int32_t ld_stream_s32(const void* p) {
     int32_t v;
-    asm volatile("ld.global.cs.s32 %0, [%1];" : "=r"(v) : "l"(p));
+    asm volatile("ld.global" GSR_LDQ ".s32 %0, [%1];" : "=r"(v) : "l"(p));
     return v;
 }
 __device__ __forceinline__ uint32_t ld_stream_u32(const void* p) {
     uint32_t v;
-    asm volatile("ld.global.cs.u32 %0, [%1];" : "=r"(v) : "l"(p));
+    asm volatile("ld.global" GSR_LDQ ".u32 %0, [%1];" : "=r"(v) : "l"(p));
     return v;
 }
 // two attitude coefficients (slots 2i, 2i+1); lanes j >= 12 keep their zeros
 __device__ __forceinline__ void ld_att_pair(const void* p, int active, double& a, double& b) {
     asm volatile("{\n\t.reg .pred pa;\n\tsetp.ne.s32 pa, %2, 0;\n\t"
-                 "@pa ld.global.cs.v2.f64 {%0, %1}, [%3];\n\t}"
+                 "@pa ld.global" GSR_LDQ ".v2.f64 {%0, %1}, [%3];\n\t}"
                  : "+d"(a), "+d"(b) : "r"(active), "l"(p));
 }
 __device__ __forceinline__ void ld_aoff(const unsigned char* T, int h, uint32_t (&aw)[4]) {
-    asm volatile("ld.global.cs.v4.u32 {%0, %1, %2, %3}, [%4];"
+    asm volatile("ld.global" GSR_LDQ ".v4.u32 {%0, %1, %2, %3}, [%4];"
                  : "=r"(aw[0]), "=r"(aw[1]), "=r"(aw[2]), "=r"(aw[3]) : "l"(T + OFF_AOFF + h * 16));
 }
 __device__ __forceinline__ void load_A(const unsigned char* __restrict__ T, int lane, RegsA& r) {
@@ -264,9 +271,19 @@ __device__ __forceinline__ void astro_mode2(double (&vs)[5], int32_t s, int lane
                                             int64_t S, double dscale) {
     GSR_ASSERT(s >= 0 && s < S);
     const int32_t s_up = __shfl_up_sync(0xffffffffu, s, 1);
-    const bool head = lane == 0 || s_up != s;
-    const unsigned heads = __ballot_sync(0xffffffffu, head);
-    if (heads == 1u) {   // the whole warp lies inside one star
+    bool head = lane == 0 || s_up != s;
+    unsigned heads = __ballot_sync(0xffffffffu, head);
+#if GSR_ASTRO_CAP > 0
+    // Runs longer than GSR_ASTRO_CAP rows are cut into pieces of that length, each flushed by its
+    // own atomic: the scan below then never needs a step beyond GSR_ASTRO_CAP / 2 (10 shuffles
+    // per step on the LSU pipe), at the price of a few more atomics for the stars with long runs.
+    {
+        const int run0 = 31 - __clz(heads & ((2u << lane) - 1u));
+        head = head || ((lane - run0) & (GSR_ASTRO_CAP - 1)) == 0;
+        heads = __ballot_sync(0xffffffffu, head);
+    }
+#endif
+    if (GSR_ASTRO_CAP == 0 && heads == 1u) {   // the whole warp lies inside one star
 #pragma unroll
         for (int k = 0; k < 5; ++k) {
             const double tsum = warp_sum(vs[k]);
@@ -283,7 +300,7 @@ __device__ __forceinline__ void astro_mode2(double (&vs)[5], int32_t s, int lane
                        n8 = n4 & (n4 >> 4), n16 = n8 & (n8 >> 8);
         const unsigned need = 1u | (n2 ? 2u : 0u) | (n4 ? 4u : 0u) | (n8 ? 8u : 0u) | (n16 ? 16u : 0u);
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
+        for (int o = 1; o < (GSR_ASTRO_CAP > 0 ? GSR_ASTRO_CAP : 32); o <<= 1) {
             if (need & o) {
 #pragma unroll
                 for (int k = 0; k < 5; ++k) {

@@ -198,6 +198,9 @@ struct Workspace {
     int64_t graph_ncon = 0;
     void* graph_comm = nullptr;
     int graph_builds = 0;       // graphs captured so far (gsr_debug_graph_builds)
+    cudaGraphExec_t wgraph = nullptr;   // the whole loop: a conditional WHILE node around the iteration
+    bool wgraph_tried = false;  // (same cache key as `graph`; built with it)
+    bool last_loop_while = false;   // the last solve ran as ONE launch of wgraph
 };
 
 }  // namespace gsr
@@ -242,6 +245,7 @@ struct gsr_matrix {
     int opt_two_pass;               // 1: aprod1 + aprod2 per iteration instead of the fused pass
     int opt_no_fixed;               // 1: fp64 atomics in the instrumental pass even when scaled
     int opt_deterministic;          // 1: no floating-point atomics anywhere in the iteration
+    int opt_no_while;               // 1: one graph launch per iteration instead of the WHILE graph
     int opt_aprod2_split;           // 1: aprod2 = main launch + instrumental pass (default 0: one sweep)
     double* yint;                   // [m_int] scaled y in internal order, written by the main
                                     // launch of a caller-order gsr_aprod2 (allocated on first use)

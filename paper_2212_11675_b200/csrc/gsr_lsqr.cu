@@ -246,12 +246,15 @@ __global__ void __launch_bounds__(1024) k_scalar_init2(LsqrState* __restrict__ s
 }
 
 // beta_{k+1} = ||A v_k - alpha_k u_k||, anorm update
+// (sum_out, if given, receives sum u_hat^2: the fixed-point scale of the instrumental pass)
 __global__ void __launch_bounds__(1024) k_scalar_beta(LsqrState* __restrict__ st,
-                                                      const double* __restrict__ part_u, int64_t np) {
+                                                      const double* __restrict__ part_u, int64_t np,
+                                                      double* __restrict__ sum_out) {
     if (st->stop) return;
     __shared__ double red[32];
     double ss = reduce_partials_1024(part_u, np, red);
     if (threadIdx.x != 0) return;
+    if (sum_out) *sum_out = ss;
     st->itn += 1;
     double beta = sqrt(ss);
     st->beta = beta;
@@ -373,6 +376,13 @@ __global__ void k_raise_stop(LsqrState* __restrict__ st) {
     if (st->istop != 0) st->stop = 1;
 }
 
+// Loop condition of the WHILE graph (row a11): run the body again unless the stop flag is up.
+// (It is also the body's k_raise_stop: one node less on the critical path of a small system.)
+__global__ void k_loop_cond(LsqrState* __restrict__ st, cudaGraphConditionalHandle h) {
+    if (st->istop != 0) st->stop = 1;
+    cudaGraphSetConditional(h, st->stop ? 0u : 1u);
+}
+
 // ---- host side ----------------------------------------------------------------------------
 
 int ensure_workspace(gsr_matrix* A) {
@@ -402,6 +412,7 @@ int ensure_workspace(gsr_matrix* A) {
 void free_workspace(gsr_matrix* A) {
     Workspace& W = A->ws;
     if (W.graph) cudaGraphExecDestroy(W.graph);
+    if (W.wgraph) cudaGraphExecDestroy(W.wgraph);
     cudaFree(W.u); cudaFree(W.v); cudaFree(W.w); cudaFree(W.x); cudaFree(W.t); cudaFree(W.var);
     cudaFree(W.part_u); cudaFree(W.part_v); cudaFree(W.part_w);
     cudaFree(W.part_va); cudaFree(W.part_wa); cudaFree(W.red);
@@ -419,11 +430,11 @@ void free_workspace(gsr_matrix* A) {
 // together, k_aprod2_instr adds the instrumental block of t, k_vnew forms v = t/beta - beta v.
 // Two-pass form (GSR_OPT_FUSED = 0): aprod1, then aprod2 on the pre-scaled v.
 static int kernels_per_iteration(const gsr_matrix* A) {
-    return (A->opt_two_pass ? (A->opt_aprod2_split ? 9 : 8) : (A->comm ? 10 : 8)) + (A->n_con > 0 ? 2 : 0) +
+    return (A->opt_two_pass ? (A->opt_aprod2_split ? 9 : 8) : (A->comm ? 10 : 7)) + (A->n_con > 0 ? 2 : 0) +
            (A->opt_deterministic ? 1 : 0);
 }
 
-static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
+static int enqueue_iteration(gsr_matrix* A, cudaStream_t s, const cudaGraphConditionalHandle* loop = nullptr) {
     Workspace& W = A->ws;
     const int64_t n = A->n_cols;
     const int64_t split = A->comm ? A->off_att : 0;   // sharded: [0, split) distributed slice
@@ -432,7 +443,7 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
         // bidiagonalisation, first half: u_hat <- A v - (alpha/beta) u_hat ; partials of u_hat^2
         GSR_TRY(launch_aprod1(A, W.v, W.u, &W.st->ca, W.part_u, &W.st->stop, nullptr, s));
         GSR_TRY(launch_con_aprod1(A, W.v, W.u + A->m_int, &W.st->ca, W.part_u + A->n_units, &W.st->stop, s));
-        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_units + ncp);
+        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_units + ncp, nullptr);
         // second half: v <- A^T (u_hat/beta) - beta v
         k_prescale<<<NB_N, TB_N, 0, s>>>(W.v, n, W.st);
         GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s));
@@ -446,8 +457,7 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
         GSR_TRY(launch_fused_streamed(A, W.v, W.u, &W.st->ca, W.part_u, W.t, &W.st->stop, s));
         GSR_TRY(launch_con_aprod1(A, W.v, W.u + A->m_int, &W.st->ca, W.part_u + A->n_units, &W.st->stop, s));
         GSR_TRY(launch_con_aprod2(A, W.u + A->m_int, W.t, A->coef_one, &W.st->stop, s));
-        k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units + ncp, W.red + 3, &W.st->stop);
-        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.red + 3, 1);
+        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_units + ncp, W.red + 3);
         k_vnew<<<NB_N, TB_N, 0, s>>>(W.v, W.t, n, W.st, W.part_v, 0, nullptr);
         k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N, nullptr);
         k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, W.t, W.var, 0, nullptr);
@@ -457,10 +467,10 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
         // constraint rows (row f3): same two steps on the CSR block, u_hat[m_int ..]
         GSR_TRY(launch_con_aprod1(A, W.v, W.u + A->m_int, &W.st->ca, W.part_u + A->n_units, &W.st->stop, s));
         GSR_TRY(launch_con_aprod2(A, W.u + A->m_int, W.t, A->coef_one, &W.st->stop, s));
-        k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units + ncp, W.red + 3, &W.st->stop);
+        // beta (and sum u_hat^2 for the fixed-point scale of the instrumental pass) in one kernel
+        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_units + ncp, W.red + 3);
         GSR_TRY(launch_aprod2_instr(A, W.u, W.t, W.red + 3, &W.st->stop, det, s));
         if (det) GSR_TRY(launch_det_finish(A, W.t, &W.st->det_e, W.red + 3, &W.st->stop, s));
-        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.red + 3, 1);
         k_vnew<<<NB_N, TB_N, 0, s>>>(W.v, W.t, n, W.st, W.part_v, 0, nullptr);
         k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N, nullptr);
         k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, W.t, W.var, 0, nullptr);
@@ -476,7 +486,7 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
         k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units + ncp, W.t + n, &W.st->stop);
         GSR_TRY(launch_aprod2_instr(A, W.u, W.t, W.t + n, &W.st->stop, 0, s));   // local ||u_hat||^2
         GSR_TRY(comm_allreduce_sum(A->comm, W.t + split, (size_t)(n - split + 1), s));
-        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.t + n, 1);
+        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.t + n, 1, nullptr);
         k_vnew<<<NB_N, TB_N, 0, s>>>(W.v, W.t, n, W.st, W.part_v, split, W.part_va);
         k_sum_partials<<<1, 1024, 0, s>>>(W.part_va, NB_N, W.red, &W.st->stop);
         GSR_TRY(comm_allreduce_sum(A->comm, W.red, 2, s));      // red[1]: from the last k_update
@@ -484,7 +494,8 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s) {
         k_update<false><<<NB_N, TB_N, 0, s>>>(W.v, W.w, W.x, n, W.st, W.part_w, W.t, W.var, split, W.part_wa);
         k_sum_partials<<<1, 1024, 0, s>>>(W.part_wa, NB_N, W.red + 1, &W.st->stop);
     }
-    k_raise_stop<<<1, 1, 0, s>>>(W.st);
+    if (loop) k_loop_cond<<<1, 1, 0, s>>>(W.st, *loop);   // body of the WHILE graph
+    else k_raise_stop<<<1, 1, 0, s>>>(W.st);
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;
 }
@@ -537,6 +548,49 @@ static int build_graph(gsr_matrix* A, cudaStream_t s) {
     W.graph_ncon = A->n_con;
     W.graph_comm = (void*)A->comm;
     W.graph_builds += 1;
+    // The whole loop as ONE graph: a conditional WHILE node whose body is the same iteration with
+    // k_loop_cond in the place of k_raise_stop.  One launch per solve, the stop decision never leaves the device.  Not with
+    // a communicator (NCCL kernels stay outside conditional bodies).  If the driver refuses any
+    // step the per-iteration graph above is what runs (gsr_debug_while_graph tells which).
+    if (W.wgraph) {
+        cudaGraphExecDestroy(W.wgraph);
+        W.wgraph = nullptr;
+    }
+    W.wgraph_tried = true;
+    if (!A->comm) {
+        cudaStream_t ws = nullptr;
+        cudaGraph_t wg = nullptr;
+        bool ok = cudaStreamCreateWithFlags(&ws, cudaStreamNonBlocking) == cudaSuccess;
+        ok = ok && cudaGraphCreate(&wg, 0) == cudaSuccess;
+        cudaGraphConditionalHandle ch;
+        ok = ok && cudaGraphConditionalHandleCreate(&ch, wg, 1, cudaGraphCondAssignDefault) == cudaSuccess;
+        cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+        cudaGraphNode_t node;
+        if (ok) {
+            np.conditional.handle = ch;
+            np.conditional.type = cudaGraphCondTypeWhile;
+            np.conditional.size = 1;
+            ok = cudaGraphAddNode(&node, wg, nullptr, 0, &np) == cudaSuccess;
+        }
+        if (ok) {
+            cudaGraph_t body = np.conditional.phGraph_out[0];
+            before = g_launches;
+            ok = cudaStreamBeginCaptureToGraph(ws, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+            if (ok) {
+                const int rcw = enqueue_iteration(A, ws, &ch);
+                cudaGraph_t got = nullptr;
+                ok = cudaStreamEndCapture(ws, &got) == cudaSuccess && rcw == GSR_OK;
+            }
+            g_launches = before;
+        }
+        ok = ok && cudaGraphInstantiate(&W.wgraph, wg, 0) == cudaSuccess;
+        if (!ok) {
+            cudaGetLastError();
+            W.wgraph = nullptr;
+        }
+        if (wg) cudaGraphDestroy(wg);
+        if (ws) cudaStreamDestroy(ws);
+    }
     return GSR_OK;
 }
 
@@ -645,6 +699,12 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     GSR_CUDA_TRY(cudaEventRecord(W.ev0, s));   // device time of the iterations alone (bench.py)
     const int64_t batch = !use_graph ? 1 : A->opt_force_itnlim ? 256 : 32;
     int64_t launched = 0;
+    W.last_loop_while = use_graph && W.wgraph != nullptr && !A->opt_no_while;
+    if (W.last_loop_while) {
+        // every iteration up to the stop (itn >= itnlim raises it too) in one launch
+        GSR_CUDA_TRY(cudaGraphLaunch(W.wgraph, s));
+        launched = itnlim;
+    }
     while (launched < itnlim) {
         int64_t nb = itnlim - launched < batch ? itnlim - launched : batch;
         if (use_graph) {
@@ -652,7 +712,7 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
             count_launch(nb * kernels_per_iteration(A));
         } else {
             GSR_TRY(enqueue_iteration(A, s));   // (its launchers count their own launches)
-            count_launch(6);
+            count_launch(5);
         }
         launched += nb;
         GSR_CUDA_TRY(cudaMemcpyAsync(W.stop_host, &W.st->stop, sizeof(int), cudaMemcpyDeviceToHost, s));
@@ -673,6 +733,7 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     if (!x_dev) GSR_CUDA_TRY(cudaMemcpyAsync(x_hd, xo, (size_t)n * 8, cudaMemcpyDeviceToHost, s));
     GSR_CUDA_TRY(cudaMemcpyAsync(&h, W.st, sizeof(h), cudaMemcpyDeviceToHost, s));
     GSR_CUDA_TRY(cudaStreamSynchronize(s));
+    if (W.last_loop_while) count_launch(h.itn * kernels_per_iteration(A));
     if (h.det_fail) return GSR_ERANGE;
     result->istop = h.istop;
     result->istop_natural = h.istop_nat;
@@ -700,6 +761,8 @@ int gsr_lsqr_set_damp(gsr_matrix* A, double damp) {
 }
 
 int64_t gsr_debug_graph_builds(const gsr_matrix* A) { return A ? A->ws.graph_builds : 0; }
+
+int gsr_debug_while_graph(const gsr_matrix* A) { return (A && A->ws.last_loop_while) ? 1 : 0; }
 
 double gsr_lsqr_last_loop_ms(const gsr_matrix* A) {
     return (A && A->ws.solved) ? A->ws.last_loop_ms : -1.0;

@@ -480,6 +480,54 @@ def test_deterministic_mode_is_bit_reproducible(name):
         s.A.close()
 
 
+@pytest.mark.parametrize("fused", [1, 0])
+def test_while_graph_loop_equals_one_launch_per_iteration(fused):
+    """Row a11, second form: the whole loop as one conditional-WHILE graph launch
+    (GSR_OPT_WHILE_GRAPH, default) against one graph launch per iteration with the stop flag
+    polled by the host.  Same kernels, same stop decision; in deterministic mode bit-identical."""
+    b = _binding()
+    s = Sys(CASES["cfg1"])
+    try:
+        rhs = _rhs(s)
+        bd = torch.from_numpy(rhs).cuda()
+        s.o.precondition()
+        b.gsr_precondition(s.A.h)
+        b.gsr_set_option(s.A.h, b.GSR_OPT_FUSED, fused)
+        if fused:
+            b.gsr_set_option(s.A.h, b.GSR_OPT_DETERMINISTIC, 1)
+        out = {}
+        for loop in (1, 0):
+            b.gsr_set_option(s.A.h, b.GSR_OPT_WHILE_GRAPH, loop)
+            # fixed count
+            b.gsr_set_option(s.A.h, b.GSR_OPT_FORCE_ITNLIM, 1)
+            x = torch.empty(s.n, dtype=torch.float64, device="cuda")
+            n0 = b.gsr_launch_count()
+            r = b.gsr_lsqr_solve(s.A.h, bd, x, 25)
+            launches = b.gsr_launch_count() - n0
+            assert b.gsr_debug_while_graph(s.A.h) == loop      # the loop form asked for really ran
+            assert (r.istop, r.itn) == (7, 25)
+            # natural stop
+            b.gsr_set_option(s.A.h, b.GSR_OPT_FORCE_ITNLIM, 0)
+            x2 = torch.empty(s.n, dtype=torch.float64, device="cuda")
+            r2 = b.gsr_lsqr_solve(s.A.h, bd, x2, 500, 1e-10, 1e-10, 1e8)
+            assert b.gsr_debug_while_graph(s.A.h) == loop
+            out[loop] = (x.cpu().numpy(), r, x2.cpu().numpy(), r2, launches)
+        ro = s.o.lsqr(rhs, 25, force_itnlim=True)
+        ro2 = s.o.lsqr(rhs, 500, 1e-10, 1e-10, 1e8)
+        for loop in (1, 0):
+            xx, r, xx2, r2, _ = out[loop]
+            assert np.linalg.norm(xx - ro.x) <= X_TOL * np.linalg.norm(ro.x)
+            assert r2.istop == ro2.istop and abs(r2.itn - ro2.itn) <= 1
+            assert np.linalg.norm(xx2 - ro2.x) <= X_TOL * np.linalg.norm(ro2.x)
+        assert out[1][3].itn == out[0][3].itn and out[1][3].istop == out[0][3].istop
+        assert out[1][4] == out[0][4], (out[1][4], out[0][4])      # same kernels per iteration
+        if fused:      # integer sums: the two loop forms agree to the last bit
+            assert np.array_equal(out[1][0], out[0][0]) and np.array_equal(out[1][2], out[0][2])
+            assert out[1][1] == out[0][1] and out[1][3] == out[0][3]
+    finally:
+        s.A.close()
+
+
 def test_zz_write_sensitivity_log():
     """Not a check of its own: records the oracle's one-ulp sensitivities that bounded the
     tolerances of test_precondition_and_lsqr_parity (quoted in DESIGN.md, reading A20)."""
