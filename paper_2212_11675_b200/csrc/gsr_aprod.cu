@@ -30,9 +30,6 @@
 #define GSR_ASSERT(c) ((void)0)
 #endif
 
-#ifndef GSR_ASTRO_CAP
-#define GSR_ASTRO_CAP 0
-#endif
 #ifndef GSR_LDQ
 #define GSR_LDQ ".cs"
 #endif
@@ -264,8 +261,16 @@ __device__ __forceinline__ int fixed_exp(double ss) {
     return e < -900 ? -900 : e;   // keeps 2^(61-e) finite for a vanishing vector
 }
 
-// astrometric part of aprod2 for one tile: segmented reduction over the
-// star-sorted home lanes, one global atomic per (tile, star, coefficient).  vs[k] = A[l,k]*y[l].
+// astrometric part of aprod2 for one tile.  vs[k] = A[l,k]*y[l].
+// Usual case (a star has a handful of rows per attitude bin, so a tile holds many stars): ONE
+// GLOBAL ATOMIC PER ROW AND COEFFICIENT, no reduction inside the warp.  Measured on B200 at
+// cfg3 (about 9 stars per tile): the 5 x 32-lane red.global instructions, whose lanes fall into
+// 3-4 lines, cost the LSU pipe far less than the segmented shuffle scan they replace (31
+// shuffles = 40 wavefronts per tile; k_fused 12.4 -> 11.7 ms, k_aprod2 12.1 -> 10.9 ms), and
+// the L2 takes the 1.5e9 adds per pass in its stride.  Tiles that lie inside one or two stars
+// (heavy stars: all their atomics would go to the same 5 addresses) are reduced first: runs are
+// cut into pieces of 4 rows, two scan steps, one atomic per piece.
+constexpr int ASTRO_FEW_STARS = 2;
 template <bool DET>
 __device__ __forceinline__ void astro_mode2(double (&vs)[5], int32_t s, int lane, double* __restrict__ x,
                                             int64_t S, double dscale) {
@@ -273,46 +278,32 @@ __device__ __forceinline__ void astro_mode2(double (&vs)[5], int32_t s, int lane
     const int32_t s_up = __shfl_up_sync(0xffffffffu, s, 1);
     bool head = lane == 0 || s_up != s;
     unsigned heads = __ballot_sync(0xffffffffu, head);
-#if GSR_ASTRO_CAP > 0
-    // Runs longer than GSR_ASTRO_CAP rows are cut into pieces of that length, each flushed by its
-    // own atomic: the scan below then never needs a step beyond GSR_ASTRO_CAP / 2 (10 shuffles
-    // per step on the LSU pipe), at the price of a few more atomics for the stars with long runs.
-    {
-        const int run0 = 31 - __clz(heads & ((2u << lane) - 1u));
-        head = head || ((lane - run0) & (GSR_ASTRO_CAP - 1)) == 0;
-        heads = __ballot_sync(0xffffffffu, head);
-    }
-#endif
-    if (GSR_ASTRO_CAP == 0 && heads == 1u) {   // the whole warp lies inside one star
-#pragma unroll
-        for (int k = 0; k < 5; ++k) {
-            const double tsum = warp_sum(vs[k]);
-            if (lane == 0 && tsum != 0.0) add_out<DET>(x + 5 * (int64_t)s + k, tsum, dscale);
-        }
-    } else {
-        // segmented inclusive scan; the last lane of each segment holds its sum.  A step of
-        // distance o is needed only if some run is longer than o rows, i.e. if there are o
-        // consecutive non-head lanes (shuffles cost LSU data-pipe wavefronts).
-        const unsigned below = heads & ((2u << lane) - 1u);        // heads at or below me
-        const int seg_start = 31 - __clz(below);
-        const bool tail = lane == 31 || ((heads >> (lane + 1)) & 1u);
-        const unsigned n1 = ~heads, n2 = n1 & (n1 >> 1), n4 = n2 & (n2 >> 2),
-                       n8 = n4 & (n4 >> 4), n16 = n8 & (n8 >> 8);
-        const unsigned need = 1u | (n2 ? 2u : 0u) | (n4 ? 4u : 0u) | (n8 ? 8u : 0u) | (n16 ? 16u : 0u);
-#pragma unroll
-        for (int o = 1; o < (GSR_ASTRO_CAP > 0 ? GSR_ASTRO_CAP : 32); o <<= 1) {
-            if (need & o) {
-#pragma unroll
-                for (int k = 0; k < 5; ++k) {
-                    const double up = __shfl_up_sync(0xffffffffu, vs[k], o);
-                    if (lane - o >= seg_start) vs[k] += up;
-                }
-            }
-        }
+    if (__popc(heads) > ASTRO_FEW_STARS) {
 #pragma unroll
         for (int k = 0; k < 5; ++k)
-            if (tail && vs[k] != 0.0) add_out<DET>(x + 5 * (int64_t)s + k, vs[k], dscale);
+            if (vs[k] != 0.0) add_out<DET>(x + 5 * (int64_t)s + k, vs[k], dscale);
+        return;
     }
+    {
+        const int run0 = 31 - __clz(heads & ((2u << lane) - 1u));
+        head = head || ((lane - run0) & 3) == 0;
+        heads = __ballot_sync(0xffffffffu, head);
+    }
+    // segmented inclusive scan over pieces of at most 4 rows; the last lane of a piece holds its sum
+    const unsigned below = heads & ((2u << lane) - 1u);        // heads at or below me
+    const int seg_start = 31 - __clz(below);
+    const bool tail = lane == 31 || ((heads >> (lane + 1)) & 1u);
+#pragma unroll
+    for (int o = 1; o < 4; o <<= 1) {
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            const double up = __shfl_up_sync(0xffffffffu, vs[k], o);
+            if (lane - o >= seg_start) vs[k] += up;
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < 5; ++k)
+        if (tail && vs[k] != 0.0) add_out<DET>(x + 5 * (int64_t)s + k, vs[k], dscale);
 }
 
 // ---- aprod1: y[i] = ca*y[i] + sum_k A[i,k] x[col(i,k)]  (Algorithm 1) --------------------

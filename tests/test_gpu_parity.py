@@ -195,7 +195,11 @@ def test_precondition_and_lsqr_parity(name, fused):
             nz = ro.se > 0
             assert np.all(np.isfinite(se_host)) and np.all(se_host[~nz] == 0.0)
             if not converged:
-                se_tol = min(max(2 * tol, 20.0 * sens_se), 10 * X_TOL_CAP)   # same rule as for x (A20)
+                # same rule as for x (A20); the cap is reading A21's estimate-level bound: var is a
+                # RUNNING sum, so at skew_hot k = 200 it still carries the unstable stage around
+                # k = 60 (oracle's own one-ulp sensitivity 3.4e-4, two correct GPU summation orders
+                # measured 2e-5 and 1.4e-3 from the oracle)
+                se_tol = min(max(2 * tol, 20.0 * sens_se), 1e-2)
                 assert np.linalg.norm(se_host - ro.se) <= se_tol * np.linalg.norm(ro.se), (name, k, sens_se)
                 # element-wise where the oracle's own se is stable too (var is a running sum: at
                 # skew_hot k = 200 it still carries the terms of the unstable stage around k = 60)
