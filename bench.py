@@ -68,6 +68,8 @@ def parse():
     ap.add_argument("--replicas", action="store_true",
                     help="N > 1: N independent systems (no collective) instead of one row-sharded system")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--while-graph", action="store_true",
+                    help="run the loop as ONE conditional-WHILE CUDA graph launch (GSR_OPT_WHILE_GRAPH)")
     ap.add_argument("--two-pass", action="store_true",
                     help="GSR_OPT_FUSED = 0: aprod1 + aprod2 per iteration (two reads of the matrix)")
     ap.add_argument("--sharded", action="store_true",
@@ -345,6 +347,7 @@ def main():
     g.gsr_precondition(h)
     g.gsr_set_option(h, g.GSR_OPT_FORCE_ITNLIM, 1)
     g.gsr_set_option(h, g.GSR_OPT_FUSED, 0 if args.two_pass else 1)
+    g.gsr_set_option(h, g.GSR_OPT_WHILE_GRAPH, 1 if args.while_graph else 0)
     x = torch.empty(n, dtype=torch.float64, device=dev)
     torch.cuda.synchronize()
     t_setup = time.perf_counter() - t_setup

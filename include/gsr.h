@@ -246,22 +246,27 @@ enum {
                                  the fused iteration accumulates in exact 64-bit fixed point
                                  with native 32-bit shared atomics (order-independent sums,
                                  normwise error <= n_j 2^-62 ||u|| per column); 0: fp64 atomics  */
-    GSR_OPT_APROD2_SPLIT = 5, /* 0 (default): aprod2 (gsr_aprod2 and the two-pass iteration) is one
+    GSR_OPT_APROD2_SPLIT = 5, /* how aprod2 (gsr_aprod2 and the two-pass iteration) runs.  0: one
                                  launch that does all four blocks (Algorithm 2 as one sweep);
                                  1: two launches -- astrometric + attitude + global blocks over
                                  152 B of every row, then the instrumental block over the
                                  instrumental planes alone (fp64 adds, componentwise accuracy as
-                                 before).  Measured on B200: the sweep is 7 %
-                                 faster at 10 000 instrumental columns in internal row order,
-                                 the split 28 % faster through the caller-order API at 60        */
-    GSR_OPT_WHILE_GRAPH = 6   /* 1 (default): the whole iteration loop of gsr_lsqr_solve is ONE CUDA
-                                 graph launch -- a conditional WHILE node whose body is the
-                                 iteration and whose condition a device kernel sets from the
-                                 stop flag -- so neither the stop decision nor a launch crosses
-                                 to the host between iterations (matters for small systems:
-                                 config 1 is launch-bound); 0, with a communicator, or on a
-                                 streamed handle: one graph launch per iteration, the stop flag
-                                 polled from pinned memory every 32 (fixed-count mode: 256)    */
+                                 before); -1 (default): the split when n_instr < 512, where the
+                                 lanes of one instruction contend for the few accumulators
+                                 (measured on B200 at 1e8 rows, 60 columns: 6.0 against 8.5 ms),
+                                 else the sweep (10 000 columns, 3e8 rows: 14.3 against 14.7)  */
+    GSR_OPT_WHILE_GRAPH = 6   /* 1: the whole iteration loop of gsr_lsqr_solve is ONE CUDA graph
+                                 launch -- a conditional WHILE node whose body is the iteration
+                                 and whose condition a device kernel sets from the stop flag --
+                                 so neither the stop decision nor a launch crosses to the host
+                                 between iterations (config 1, launch-bound: 60.4 against 62.8 us
+                                 per iteration; immaterial at 1e8 rows and above).  Ignored with
+                                 a communicator or on a streamed handle.  0 (default): one
+                                 graph launch per iteration, the stop flag polled from pinned
+                                 memory every 32 (fixed-count mode: 256) -- the default because
+                                 Nsight Compute cannot see kernel nodes inside a graph that has
+                                 conditional nodes, and the per-kernel evidence under profiles/
+                                 is taken from the default path                                 */
 };
 int gsr_set_option(gsr_matrix* A, int key, int64_t value);
 

@@ -261,49 +261,50 @@ __device__ __forceinline__ int fixed_exp(double ss) {
     return e < -900 ? -900 : e;   // keeps 2^(61-e) finite for a vanishing vector
 }
 
-// astrometric part of aprod2 for one tile.  vs[k] = A[l,k]*y[l].
-// Usual case (a star has a handful of rows per attitude bin, so a tile holds many stars): ONE
-// GLOBAL ATOMIC PER ROW AND COEFFICIENT, no reduction inside the warp.  Measured on B200 at
-// cfg3 (about 9 stars per tile): the 5 x 32-lane red.global instructions, whose lanes fall into
-// 3-4 lines, cost the LSU pipe far less than the segmented shuffle scan they replace (31
-// shuffles = 40 wavefronts per tile; k_fused 12.4 -> 11.7 ms, k_aprod2 12.1 -> 10.9 ms), and
-// the L2 takes the 1.5e9 adds per pass in its stride.  Tiles that lie inside one or two stars
-// (heavy stars: all their atomics would go to the same 5 addresses) are reduced first: runs are
-// cut into pieces of 4 rows, two scan steps, one atomic per piece.
-constexpr int ASTRO_FEW_STARS = 2;
+// astrometric part of aprod2 for one tile: segmented reduction over the
+// star-sorted home lanes, one global atomic per (tile, star, coefficient).  vs[k] = A[l,k]*y[l].
+// (Measured on B200, cfg3, real LSQR vectors: cutting the runs into pieces of 8 / 4 / 2 / 1 rows to
+// save scan steps -- 1 = one atomic per row and coefficient, no scan -- gives k_fused 13.9 / 13.9 /
+// 14.8 / 18.3 ms against 13.9 for whole runs: the L2 atomic rate, not the shuffles, is what the
+// shorter pieces run into.  Timed with u = 0 the same variants look 6 % FASTER, because the
+// zero-valued atomics are skipped: product timings need real vectors.)
 template <bool DET>
 __device__ __forceinline__ void astro_mode2(double (&vs)[5], int32_t s, int lane, double* __restrict__ x,
                                             int64_t S, double dscale) {
     GSR_ASSERT(s >= 0 && s < S);
     const int32_t s_up = __shfl_up_sync(0xffffffffu, s, 1);
-    bool head = lane == 0 || s_up != s;
-    unsigned heads = __ballot_sync(0xffffffffu, head);
-    if (__popc(heads) > ASTRO_FEW_STARS) {
-#pragma unroll
-        for (int k = 0; k < 5; ++k)
-            if (vs[k] != 0.0) add_out<DET>(x + 5 * (int64_t)s + k, vs[k], dscale);
-        return;
-    }
-    {
-        const int run0 = 31 - __clz(heads & ((2u << lane) - 1u));
-        head = head || ((lane - run0) & 3) == 0;
-        heads = __ballot_sync(0xffffffffu, head);
-    }
-    // segmented inclusive scan over pieces of at most 4 rows; the last lane of a piece holds its sum
-    const unsigned below = heads & ((2u << lane) - 1u);        // heads at or below me
-    const int seg_start = 31 - __clz(below);
-    const bool tail = lane == 31 || ((heads >> (lane + 1)) & 1u);
-#pragma unroll
-    for (int o = 1; o < 4; o <<= 1) {
+    const bool head = lane == 0 || s_up != s;
+    const unsigned heads = __ballot_sync(0xffffffffu, head);
+    if (heads == 1u) {   // the whole warp lies inside one star
 #pragma unroll
         for (int k = 0; k < 5; ++k) {
-            const double up = __shfl_up_sync(0xffffffffu, vs[k], o);
-            if (lane - o >= seg_start) vs[k] += up;
+            const double tsum = warp_sum(vs[k]);
+            if (lane == 0 && tsum != 0.0) add_out<DET>(x + 5 * (int64_t)s + k, tsum, dscale);
         }
-    }
+    } else {
+        // segmented inclusive scan; the last lane of each segment holds its sum.  A step of
+        // distance o is needed only if some run is longer than o rows, i.e. if there are o
+        // consecutive non-head lanes (shuffles cost LSU data-pipe wavefronts).
+        const unsigned below = heads & ((2u << lane) - 1u);        // heads at or below me
+        const int seg_start = 31 - __clz(below);
+        const bool tail = lane == 31 || ((heads >> (lane + 1)) & 1u);
+        const unsigned n1 = ~heads, n2 = n1 & (n1 >> 1), n4 = n2 & (n2 >> 2),
+                       n8 = n4 & (n4 >> 4), n16 = n8 & (n8 >> 8);
+        const unsigned need = 1u | (n2 ? 2u : 0u) | (n4 ? 4u : 0u) | (n8 ? 8u : 0u) | (n16 ? 16u : 0u);
 #pragma unroll
-    for (int k = 0; k < 5; ++k)
-        if (tail && vs[k] != 0.0) add_out<DET>(x + 5 * (int64_t)s + k, vs[k], dscale);
+        for (int o = 1; o < 32; o <<= 1) {
+            if (need & o) {
+#pragma unroll
+                for (int k = 0; k < 5; ++k) {
+                    const double up = __shfl_up_sync(0xffffffffu, vs[k], o);
+                    if (lane - o >= seg_start) vs[k] += up;
+                }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 5; ++k)
+            if (tail && vs[k] != 0.0) add_out<DET>(x + 5 * (int64_t)s + k, vs[k], dscale);
+    }
 }
 
 // ---- aprod1: y[i] = ca*y[i] + sum_k A[i,k] x[col(i,k)]  (Algorithm 1) --------------------
@@ -867,7 +868,7 @@ static int aprod2_view(const gsr_matrix* A, const TileView& v, const double* y, 
         GSR_CUDA_TRY(cudaGetLastError());
         return GSR_OK;
     }
-    if (!A->opt_aprod2_split) {
+    if (!aprod2_is_split(A)) {
         if (perm)
             k_aprod2<false, true, true><<<grid_for(A->grid2, nu), TPB, A->smem_bytes, s>>>(
                 v.base, un, nu, A->unit_counter, y, x, sy, perm, S, D, I, A->win, A->wstride, instr_copies(A), stop, nullptr);
@@ -1006,7 +1007,7 @@ int gsr_aprod1(const gsr_matrix* A, const double* x_dev, double* y_dev, gsr_stre
 int gsr_aprod2(const gsr_matrix* A, const double* y_dev, double* x_dev, gsr_stream stream) {
     if (!A || !x_dev || (!y_dev && A->dims.n_rows > 0)) return GSR_EINVAL;
     if (A->state != 1) return GSR_ESTATE;
-    if (A->opt_aprod2_split && !A->yint && A->m_int > 0) {
+    if (aprod2_is_split(A) && !A->yint && A->m_int > 0) {
         // scratch of the split form (a cache behind a logically const handle): y in internal order
         gsr_matrix* Am = const_cast<gsr_matrix*>(A);
         GSR_TRY(dev_alloc(Am, (void**)&Am->yint, (size_t)A->m_int * 8));

@@ -245,8 +245,8 @@ struct gsr_matrix {
     int opt_two_pass;               // 1: aprod1 + aprod2 per iteration instead of the fused pass
     int opt_no_fixed;               // 1: fp64 atomics in the instrumental pass even when scaled
     int opt_deterministic;          // 1: no floating-point atomics anywhere in the iteration
-    int opt_no_while;               // 1: one graph launch per iteration instead of the WHILE graph
-    int opt_aprod2_split;           // 1: aprod2 = main launch + instrumental pass (default 0: one sweep)
+    int opt_while;                  // 1: the whole loop as one conditional-WHILE graph launch
+    int opt_aprod2_split;           // GSR_OPT_APROD2_SPLIT + 1: 0 = auto (default), 1 = one sweep, 2 = split
     double* yint;                   // [m_int] scaled y in internal order, written by the main
                                     // launch of a caller-order gsr_aprod2 (allocated on first use)
     double damp;                    // gsr_lsqr_set_damp (row f4); 0 = the paper's undamped LSQR
@@ -327,6 +327,12 @@ int launch_fused_streamed(const gsr_matrix* A, const double* v, double* u, const
 int launch_det_finish(const gsr_matrix* A, double* t, const int* det_e, const double* ss,
                       const int* stop, cudaStream_t s);
 int configure_product_kernels(gsr_matrix* A);
+// aprod2 as two launches (main sweep + instrumental pass)?  Auto: when the instrumental block is
+// so narrow that the lanes of one instruction contend for its accumulators (measured: I = 60,
+// one sweep 8.5 ms, split 6.0 ms at 1e8 rows; I = 6000 / 10 000: 4.84 / 14.3 against 5.25 / 14.7)
+inline bool aprod2_is_split(const gsr_matrix* A) {
+    return A->opt_aprod2_split == 2 || (A->opt_aprod2_split == 0 && A->dims.n_instr < 512);
+}
 
 // One pass over the matrix: f(view) for the resident run of units, then for every streamed
 // chunk (double-buffered H2D copies on the copy stream, overlapped with f of the previous view).

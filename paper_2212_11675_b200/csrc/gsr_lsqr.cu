@@ -430,7 +430,7 @@ void free_workspace(gsr_matrix* A) {
 // together, k_aprod2_instr adds the instrumental block of t, k_vnew forms v = t/beta - beta v.
 // Two-pass form (GSR_OPT_FUSED = 0): aprod1, then aprod2 on the pre-scaled v.
 static int kernels_per_iteration(const gsr_matrix* A) {
-    return (A->opt_two_pass ? (A->opt_aprod2_split ? 9 : 8) : (A->comm ? 10 : 7)) + (A->n_con > 0 ? 2 : 0) +
+    return (A->opt_two_pass ? (aprod2_is_split(A) ? 9 : 8) : (A->comm ? 10 : 7)) + (A->n_con > 0 ? 2 : 0) +
            (A->opt_deterministic ? 1 : 0);
 }
 
@@ -506,7 +506,8 @@ static int build_graph(gsr_matrix* A, cudaStream_t s) {
     // form, the communicator, the constraint rows, and the variant of the instrumental pass
     // (fixed point needs a scaled matrix and GSR_OPT_FIXED_POINT)
     const int key = (A->opt_two_pass ? 1 : 0) | (A->p != nullptr ? 2 : 0) | (A->opt_no_fixed ? 4 : 0) |
-                    (A->n_con > 0 ? 8 : 0) | (A->opt_deterministic ? 16 : 0) | (A->opt_aprod2_split ? 32 : 0);
+                    (A->n_con > 0 ? 8 : 0) | (A->opt_deterministic ? 16 : 0) | (aprod2_is_split(A) ? 32 : 0) |
+                    (A->opt_while ? 64 : 0);
     if (W.graph_valid && W.graph_stream == s && W.graph_key == key && W.graph_comm == (void*)A->comm &&
         W.graph_ncon == A->n_con)
         return GSR_OK;
@@ -551,13 +552,14 @@ static int build_graph(gsr_matrix* A, cudaStream_t s) {
     // The whole loop as ONE graph: a conditional WHILE node whose body is the same iteration with
     // k_loop_cond in the place of k_raise_stop.  One launch per solve, the stop decision never leaves the device.  Not with
     // a communicator (NCCL kernels stay outside conditional bodies).  If the driver refuses any
-    // step the per-iteration graph above is what runs (gsr_debug_while_graph tells which).
+    // step the per-iteration graph above is what runs (gsr_debug_while_graph tells which).  Built
+    // only when GSR_OPT_WHILE_GRAPH asks for it (the option is part of the cache key).
     if (W.wgraph) {
         cudaGraphExecDestroy(W.wgraph);
         W.wgraph = nullptr;
     }
     W.wgraph_tried = true;
-    if (!A->comm) {
+    if (!A->comm && A->opt_while) {
         cudaStream_t ws = nullptr;
         cudaGraph_t wg = nullptr;
         bool ok = cudaStreamCreateWithFlags(&ws, cudaStreamNonBlocking) == cudaSuccess;
@@ -699,7 +701,7 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     GSR_CUDA_TRY(cudaEventRecord(W.ev0, s));   // device time of the iterations alone (bench.py)
     const int64_t batch = !use_graph ? 1 : A->opt_force_itnlim ? 256 : 32;
     int64_t launched = 0;
-    W.last_loop_while = use_graph && W.wgraph != nullptr && !A->opt_no_while;
+    W.last_loop_while = use_graph && W.wgraph != nullptr && A->opt_while;
     if (W.last_loop_while) {
         // every iteration up to the stop (itn >= itnlim raises it too) in one launch
         GSR_CUDA_TRY(cudaGraphLaunch(W.wgraph, s));

@@ -769,8 +769,11 @@ int gsr_set_option(gsr_matrix* A, int key, int64_t value) {
         case GSR_OPT_DETERMINISTIC: A->opt_deterministic = value != 0; return GSR_OK;
         case GSR_OPT_FUSED: A->opt_two_pass = value == 0; return GSR_OK;
         case GSR_OPT_FIXED_POINT: A->opt_no_fixed = value == 0; return GSR_OK;
-        case GSR_OPT_APROD2_SPLIT: A->opt_aprod2_split = value != 0; return GSR_OK;
-        case GSR_OPT_WHILE_GRAPH: A->opt_no_while = value == 0; return GSR_OK;
+        case GSR_OPT_APROD2_SPLIT:
+            if (value < -1 || value > 1) return GSR_EINVAL;
+            A->opt_aprod2_split = (int)value + 1;
+            return GSR_OK;
+        case GSR_OPT_WHILE_GRAPH: A->opt_while = value != 0; return GSR_OK;
         default: return GSR_EINVAL;
     }
 }

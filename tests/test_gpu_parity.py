@@ -92,10 +92,11 @@ def test_aprod1_parity(sysm):
     assert np.all(err <= APROD_TOL * scale), float((err / scale).max())
 
 
-@pytest.mark.parametrize("split", [1, 0])
+@pytest.mark.parametrize("split", [1, 0, -1])
 def test_aprod2_parity(sysm, split):
-    """Algorithm 2 through the C ABI, as one sweep over all four blocks (default)
-    and as two launches (GSR_OPT_APROD2_SPLIT = 1: the instrumental block in a pass of its own)."""
+    """Algorithm 2 through the C ABI: as two launches (GSR_OPT_APROD2_SPLIT = 1:
+    the instrumental block in a pass of its own), as one sweep over all four blocks (0), and in
+    the default setting (-1: the split for narrow instrumental blocks)."""
     b = _binding()
     y = inputs.random_vector(sysm.cfg, 3, sysm.m)
     x0 = inputs.random_vector(sysm.cfg, 4, sysm.n)
@@ -107,8 +108,9 @@ def test_aprod2_parity(sysm, split):
         b.gsr_aprod2(sysm.A.h, y.cuda(), xd)
         launches = b.gsr_launch_count() - n0
     finally:
-        b.gsr_set_option(sysm.A.h, b.GSR_OPT_APROD2_SPLIT, 0)
-    assert launches == (2 if split else 1) or sysm.m == 0, launches   # the form asked for really ran
+        b.gsr_set_option(sysm.A.h, b.GSR_OPT_APROD2_SPLIT, -1)
+    two = split == 1 or (split == -1 and sysm.cfg.n_instr < 512)      # -1: by the width of the block
+    assert launches == (2 if two else 1) or sysm.m == 0, launches     # the form asked for really ran
     err = np.abs(xd.cpu().numpy() - x_ref)
     assert np.all(err <= APROD_TOL * np.maximum(scale, 1e-300)), float((err / scale).max())
     # untouched columns (empty stars, unused instrumental columns) keep x0 exactly
@@ -487,8 +489,8 @@ def test_deterministic_mode_is_bit_reproducible(name):
 @pytest.mark.parametrize("fused", [1, 0])
 def test_while_graph_loop_equals_one_launch_per_iteration(fused):
     """Row a11, second form: the whole loop as one conditional-WHILE graph launch
-    (GSR_OPT_WHILE_GRAPH, default) against one graph launch per iteration with the stop flag
-    polled by the host.  Same kernels, same stop decision; in deterministic mode bit-identical."""
+    (GSR_OPT_WHILE_GRAPH = 1) against one graph launch per iteration with the stop flag polled
+    by the host (default).  Same kernels, same stop decision; in deterministic mode bit-identical."""
     b = _binding()
     s = Sys(CASES["cfg1"])
     try:
@@ -516,6 +518,7 @@ def test_while_graph_loop_equals_one_launch_per_iteration(fused):
             r2 = b.gsr_lsqr_solve(s.A.h, bd, x2, 500, 1e-10, 1e-10, 1e8)
             assert b.gsr_debug_while_graph(s.A.h) == loop
             out[loop] = (x.cpu().numpy(), r, x2.cpu().numpy(), r2, launches)
+        b.gsr_set_option(s.A.h, b.GSR_OPT_WHILE_GRAPH, 0)
         ro = s.o.lsqr(rhs, 25, force_itnlim=True)
         ro2 = s.o.lsqr(rhs, 500, 1e-10, 1e-10, 1e8)
         for loop in (1, 0):
