@@ -669,7 +669,8 @@ __global__ void __launch_bounds__(TPB) k_aprod2_instr(const unsigned char* __res
     const int ipad = (I + 1) & ~1;
     for (int i = threadIdx.x; i < ipad * ncopy; i += TPB) sm[i] = 0.0;   // +0.0 = integer 0
     const int e = FIXED ? fixed_exp(*ss_p) : 0;   // 2^e > ||y||
-    // sy_p (the stand-alone product only, never with FIXED): y is scaled by *sy_p first
+    // sy_p (the stand-alone product only): the product is A^T (y * *sy_p); FIXED applies the factor
+    // to the totals, so that the range bound stays ||y||
     const double scale = FIXED ? scalbn(1.0, 61 - e) : (sy_p ? *sy_p : 1.0);
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -704,7 +705,7 @@ __global__ void __launch_bounds__(TPB) k_aprod2_instr(const unsigned char* __res
         }
     }
     __syncthreads();
-    const double unscale = FIXED ? scalbn(1.0, e - 61) : 1.0;
+    const double unscale = FIXED ? scalbn(1.0, e - 61) * (sy_p ? *sy_p : 1.0) : 1.0;
     for (int i = threadIdx.x; i < I; i += TPB) {
         double vacc;
         if (FIXED) {
@@ -853,8 +854,12 @@ int launch_aprod1(const gsr_matrix* A, const double* x, double* y, const double*
     return pass(A, s, [&](const TileView& v) { return aprod1_view(A, v, x, y, ca, partials, stop, perm, s); });
 }
 
+// ss != nullptr (the solver's own calls): device sum of y^2 over ALL rows of the product.  On a
+// column-scaled matrix the instrumental block is then done by the exact fixed-point pass of the
+// fused iteration (reading A22: normwise accuracy, which is what LSQR needs) after a main launch
+// without it, instead of six fp64 compare-and-swap adds per row inside the sweep.
 static int aprod2_view(const gsr_matrix* A, const TileView& v, const double* y, double* x, const double* sy,
-                       const int* stop, const uint32_t* perm, bool square, cudaStream_t s) {
+                       const int* stop, const uint32_t* perm, bool square, const double* ss, cudaStream_t s) {
     const int nu = v.u1 - v.u0;
     if (nu <= 0) return GSR_OK;
     const int64_t S = A->dims.n_stars, D = A->dims.n_dfa;
@@ -868,7 +873,8 @@ static int aprod2_view(const gsr_matrix* A, const TileView& v, const double* y, 
         GSR_CUDA_TRY(cudaGetLastError());
         return GSR_OK;
     }
-    if (!aprod2_is_split(A)) {
+    const bool fixed = ss != nullptr && A->p != nullptr && !A->opt_no_fixed && perm == nullptr;
+    if (!fixed && !aprod2_is_split(A)) {
         if (perm)
             k_aprod2<false, true, true><<<grid_for(A->grid2, nu), TPB, A->smem_bytes, s>>>(
                 v.base, un, nu, A->unit_counter, y, x, sy, perm, S, D, I, A->win, A->wstride, instr_copies(A), stop, nullptr);
@@ -900,17 +906,21 @@ static int aprod2_view(const gsr_matrix* A, const TileView& v, const double* y, 
     const int64_t nt = v.t1 - v.t0;
     const int64_t need = (nt + NWARP - 1) / NWARP;
     const int gi = A->grid_instr < need ? A->grid_instr : (int)need;
-    k_aprod2_instr<false><<<gi, TPB, instr_smem(A), s>>>(
-        v.base + v.t0 * TILE_BYTES, nt, yi, x + A->off_instr, I, instr_copies(A), nullptr, stop, 0, syi);
+    if (fixed)
+        k_aprod2_instr<true><<<gi, TPB, instr_smem(A), s>>>(
+            v.base + v.t0 * TILE_BYTES, nt, yi, x + A->off_instr, I, instr_copies(A), ss, stop, 0, syi);
+    else
+        k_aprod2_instr<false><<<gi, TPB, instr_smem(A), s>>>(
+            v.base + v.t0 * TILE_BYTES, nt, yi, x + A->off_instr, I, instr_copies(A), nullptr, stop, 0, syi);
     count_launch();
     GSR_CUDA_TRY(cudaGetLastError());
     return GSR_OK;
 }
 
 int launch_aprod2(const gsr_matrix* A, const double* y, double* x, const double* sy,
-                  const int* stop, const uint32_t* perm, cudaStream_t s) {
+                  const int* stop, const uint32_t* perm, cudaStream_t s, const double* ss) {
     if (A->n_units == 0) return GSR_OK;
-    return pass(A, s, [&](const TileView& v) { return aprod2_view(A, v, y, x, sy, stop, perm, false, s); });
+    return pass(A, s, [&](const TileView& v) { return aprod2_view(A, v, y, x, sy, stop, perm, false, ss, s); });
 }
 
 static int fused_view(const gsr_matrix* A, const TileView& v, const double* x, double* u, const double* ca,
@@ -988,7 +998,7 @@ int launch_det_finish(const gsr_matrix* A, double* t, const int* det_e, const do
 
 int launch_colsumsq(const gsr_matrix* A, double* q, cudaStream_t s) {
     if (A->n_units == 0) return GSR_OK;
-    return pass(A, s, [&](const TileView& v) { return aprod2_view(A, v, nullptr, q, nullptr, nullptr, nullptr, true, s); });
+    return pass(A, s, [&](const TileView& v) { return aprod2_view(A, v, nullptr, q, nullptr, nullptr, nullptr, true, nullptr, s); });
 }
 
 }  // namespace gsr

@@ -307,8 +307,10 @@ void free_workspace(gsr_matrix* A);
 int launch_aprod1(const gsr_matrix* A, const double* x, double* y, const double* ca,
                   double* partials, const int* stop, const uint32_t* perm, cudaStream_t s);
 //   aprod2: x[col] += A[i,k] * (y[i] * (*sy))
+//   ss (optional): device sum of y^2 over all rows -- the solver's own calls; lets the instrumental
+//   block take the exact fixed-point pass on a column-scaled matrix (aprod2_two_launches)
 int launch_aprod2(const gsr_matrix* A, const double* y, double* x, const double* sy,
-                  const int* stop, const uint32_t* perm, cudaStream_t s);
+                  const int* stop, const uint32_t* perm, cudaStream_t s, const double* ss = nullptr);
 //   column sums of squares (preconditioner): q[col] += A[i,k]^2
 int launch_colsumsq(const gsr_matrix* A, double* q, cudaStream_t s);
 // fused LSQR pass (one read of the matrix per iteration):
@@ -330,6 +332,8 @@ int configure_product_kernels(gsr_matrix* A);
 // aprod2 as two launches (main sweep + instrumental pass)?  Auto: when the instrumental block is
 // so narrow that the lanes of one instruction contend for its accumulators (measured: I = 60,
 // one sweep 8.5 ms, split 6.0 ms at 1e8 rows; I = 6000 / 10 000: 4.84 / 14.3 against 5.25 / 14.7)
+// (the solver's aprod2 with a known norm: main launch + fixed-point instrumental pass)
+inline bool aprod2_fixed_split(const gsr_matrix* A) { return A->p != nullptr && !A->opt_no_fixed; }
 inline bool aprod2_is_split(const gsr_matrix* A) {
     return A->opt_aprod2_split == 2 || (A->opt_aprod2_split == 0 && A->dims.n_instr < 512);
 }

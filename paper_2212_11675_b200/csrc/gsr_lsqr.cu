@@ -199,10 +199,12 @@ __global__ void k_standard_errors(const double* __restrict__ var, const double* 
 
 // beta_1 = ||b||
 __global__ void __launch_bounds__(1024) k_scalar_init1(LsqrState* __restrict__ st,
-                                                       const double* __restrict__ part_u, int64_t np) {
+                                                       const double* __restrict__ part_u, int64_t np,
+                                                       double* __restrict__ sum_out) {
     __shared__ double red[32];
     double ss = reduce_partials_1024(part_u, np, red);
     if (threadIdx.x != 0) return;
+    if (sum_out) *sum_out = ss;   // ||b||^2: the range of the initial aprod2's fixed-point pass
     double beta = sqrt(ss);
     st->beta = beta;
     st->bnorm = beta;
@@ -430,7 +432,7 @@ void free_workspace(gsr_matrix* A) {
 // together, k_aprod2_instr adds the instrumental block of t, k_vnew forms v = t/beta - beta v.
 // Two-pass form (GSR_OPT_FUSED = 0): aprod1, then aprod2 on the pre-scaled v.
 static int kernels_per_iteration(const gsr_matrix* A) {
-    return (A->opt_two_pass ? (aprod2_is_split(A) ? 9 : 8) : (A->comm ? 10 : 7)) + (A->n_con > 0 ? 2 : 0) +
+    return (A->opt_two_pass ? (aprod2_is_split(A) || aprod2_fixed_split(A) ? 9 : 8) : (A->comm ? 10 : 7)) + (A->n_con > 0 ? 2 : 0) +
            (A->opt_deterministic ? 1 : 0);
 }
 
@@ -443,10 +445,10 @@ static int enqueue_iteration(gsr_matrix* A, cudaStream_t s, const cudaGraphCondi
         // bidiagonalisation, first half: u_hat <- A v - (alpha/beta) u_hat ; partials of u_hat^2
         GSR_TRY(launch_aprod1(A, W.v, W.u, &W.st->ca, W.part_u, &W.st->stop, nullptr, s));
         GSR_TRY(launch_con_aprod1(A, W.v, W.u + A->m_int, &W.st->ca, W.part_u + A->n_units, &W.st->stop, s));
-        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_units + ncp, nullptr);
+        k_scalar_beta<<<1, 1024, 0, s>>>(W.st, W.part_u, A->n_units + ncp, W.red + 3);
         // second half: v <- A^T (u_hat/beta) - beta v
         k_prescale<<<NB_N, TB_N, 0, s>>>(W.v, n, W.st);
-        GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s));
+        GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s, W.red + 3));
         GSR_TRY(launch_con_aprod2(A, W.u + A->m_int, W.v, &W.st->inv_beta, &W.st->stop, s));
         k_sumsq<<<NB_N, TB_N, 0, s>>>(W.v, n, W.part_v, &W.st->stop, 0, nullptr);
         k_scalar_main<<<1, 1024, 0, s>>>(W.st, W.part_v, W.part_w, NB_N, nullptr);
@@ -651,12 +653,12 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
             GSR_TRY(launch_con_copy_sumsq(A, b_dev + A->dims.n_rows, W.u + A->m_int, W.part_u + NB_N, s));
         k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, NB_N + (A->n_con > 0 ? 1 : 0), W.red + 2, nullptr);
         GSR_TRY(comm_allreduce_sum(A->comm, W.red + 2, 1, s));
-        k_scalar_init1<<<1, 1024, 0, s>>>(W.st, W.red + 2, 1);
+        k_scalar_init1<<<1, 1024, 0, s>>>(W.st, W.red + 2, 1, nullptr);
         count_launch();
     } else {
         if (A->n_con > 0)
             GSR_TRY(launch_con_copy_sumsq(A, b_dev + A->dims.n_rows, W.u + A->m_int, W.part_u + NB_N, s));
-        k_scalar_init1<<<1, 1024, 0, s>>>(W.st, W.part_u, NB_N + (A->n_con > 0 ? 1 : 0));
+        k_scalar_init1<<<1, 1024, 0, s>>>(W.st, W.part_u, NB_N + (A->n_con > 0 ? 1 : 0), W.red + 3);
     }
     count_launch(2);
     if (A->opt_deterministic) {
@@ -670,7 +672,8 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
         k_vnew<<<NB_N, TB_N, 0, s>>>(W.v, W.t, n, W.st, W.part_v, 0, nullptr);   // v = t / beta_1
         count_launch(2);
     } else {
-    GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s));
+    // (single GPU: ||b||^2 is known, the instrumental block takes the fixed-point pass)
+    GSR_TRY(launch_aprod2(A, W.u, W.v, &W.st->inv_beta, &W.st->stop, nullptr, s, A->comm ? nullptr : W.red + 3));
     GSR_TRY(launch_con_aprod2(A, W.u + A->m_int, W.v, &W.st->inv_beta, &W.st->stop, s));
     if (A->comm)     // replicated slice of v = A^T u: sum of the shards' contributions
         GSR_TRY(comm_allreduce_sum(A->comm, W.v + split, (size_t)(n - split), s));
@@ -835,7 +838,8 @@ int gsr_time_product(gsr_matrix* A, int which, int reps, float* ms_avg, gsr_stre
         cudaEventRecord(e0, s);
         for (int i = 0; i < nrep && rc == GSR_OK; ++i) {
             if (which == 1) rc = launch_aprod1(A, W.v, W.u, A->coef_one, W.part_u, nullptr, nullptr, s);
-            else if (which == 2) rc = launch_aprod2(A, W.u, W.v, A->coef_one, nullptr, nullptr, s);
+            else if (which == 2)   // as the solver runs it: with the norm of u_hat of its last pass, if any
+                rc = launch_aprod2(A, W.u, W.v, A->coef_one, nullptr, nullptr, s, W.solved ? W.red + 3 : nullptr);
             else if (which == 3) rc = launch_fused(A, W.v, W.u, A->coef_one, W.part_u, W.t, nullptr, nullptr, s);
             else rc = launch_aprod2_instr(A, W.u, W.t, W.red + 3, nullptr, 0, s);
         }
