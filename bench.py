@@ -323,6 +323,11 @@ def main():
     from dataclasses import replace
     from paper_2212_11675_b200 import binding as g
 
+    # NCCL logs to stdout by default (even its version line at NCCL_DEBUG=WARN): send whatever the
+    # environment asks for to stderr, so that stdout stays the one JSON line; NCCL_DEBUG is left alone
+    os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
+    if os.environ.get("NCCL_DEBUG", "VERSION").upper() == "VERSION":
+        os.environ["NCCL_DEBUG"] = "WARN"   # (at VERSION the one line NCCL prints ignores NCCL_DEBUG_FILE)
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -350,8 +355,6 @@ def main():
         b[r0:r0 + nr] = inputs.noise(cfg, r0, nr, dev)
     comm = None
     if sharded:
-        if "NCCL_DEBUG" not in os.environ:
-            os.environ["NCCL_DEBUG"] = "WARN"    # unset: keep stdout to the one JSON line
         # weak-scaled sharded system: rank r owns stars [r*S, (r+1)*S) of an N*S-star system; the
         # attitude + instrumental + global unknowns are shared, so their x_true comes from rank 0's seed
         xt0 = inputs.x_true(cfg0, dev)
