@@ -535,6 +535,21 @@ def test_while_graph_loop_equals_one_launch_per_iteration(fused):
         s.A.close()
 
 
+def test_option_values_are_validated():
+    b = _binding()
+    s = Sys(CASES["one_instr_col"])
+    try:
+        for v in (-1, 0, 1):
+            b.gsr_set_option(s.A.h, b.GSR_OPT_APROD2_SPLIT, v)
+        for key, v in ((b.GSR_OPT_APROD2_SPLIT, 2), (b.GSR_OPT_APROD2_SPLIT, -2), (99, 1), (0, 1)):
+            with pytest.raises(b.GsrError) as ei:
+                b.gsr_set_option(s.A.h, key, v)
+            assert ei.value.code == b.GSR_EINVAL
+        b.gsr_set_option(s.A.h, b.GSR_OPT_APROD2_SPLIT, -1)
+    finally:
+        s.A.close()
+
+
 def test_zz_write_sensitivity_log():
     """Not a check of its own: records the oracle's one-ulp sensitivities that bounded the
     tolerances of test_precondition_and_lsqr_parity (quoted in DESIGN.md, reading A20)."""
