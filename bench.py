@@ -68,6 +68,9 @@ def parse():
     ap.add_argument("--replicas", action="store_true",
                     help="N > 1: N independent systems (no collective) instead of one row-sharded system")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--fp64-instr", action="store_true",
+                    help="GSR_OPT_FIXED_POINT = 0: fp64 adds for the instrumental block (in the two-pass "
+                         "form aprod2 is then the one-sweep kernel gsr_aprod2 runs)")
     ap.add_argument("--while-graph", action="store_true",
                     help="run the loop as ONE conditional-WHILE CUDA graph launch (GSR_OPT_WHILE_GRAPH)")
     ap.add_argument("--two-pass", action="store_true",
@@ -369,6 +372,7 @@ def main():
     g.gsr_set_option(h, g.GSR_OPT_FORCE_ITNLIM, 1)
     g.gsr_set_option(h, g.GSR_OPT_FUSED, 0 if args.two_pass else 1)
     g.gsr_set_option(h, g.GSR_OPT_WHILE_GRAPH, 1 if args.while_graph else 0)
+    g.gsr_set_option(h, g.GSR_OPT_FIXED_POINT, 0 if args.fp64_instr else 1)
     x = torch.empty(n, dtype=torch.float64, device=dev)
     torch.cuda.synchronize()
     t_setup = time.perf_counter() - t_setup
