@@ -146,7 +146,9 @@ int gsr_aprod1(const gsr_matrix* A, const double* x_dev, double* y_dev, gsr_stre
 
 /* aprod mode 2:  x[col(i,k)] = x[col(i,k)] + A[i,k] y[i].
  * y_dev [m], x_dev [n_cols].  Asynchronous on stream.  Uses scratch inside the handle: calls
- * on the same handle must be stream-ordered. */
+ * on the same handle must be stream-ordered.  In the default two-launch form
+ * (GSR_OPT_APROD2_SPLIT) the first call allocates an m-sized work vector (8 bytes per row, y in
+ * the internal row order; counted by gsr_matrix_device_bytes; GSR_ENOMEM if it does not fit). */
 int gsr_aprod2(const gsr_matrix* A, const double* y_dev, double* x_dev, gsr_stream stream);
 
 /* ---- preconditioner (row a1; Algorithm 3 line 2) ---------------------- */
@@ -246,15 +248,16 @@ enum {
                                  the fused iteration accumulates in exact 64-bit fixed point
                                  with native 32-bit shared atomics (order-independent sums,
                                  normwise error <= n_j 2^-62 ||u|| per column); 0: fp64 atomics  */
-    GSR_OPT_APROD2_SPLIT = 5, /* how aprod2 (gsr_aprod2 and the two-pass iteration) runs.  0: one
-                                 launch that does all four blocks (Algorithm 2 as one sweep);
-                                 1: two launches -- astrometric + attitude + global blocks over
-                                 152 B of every row, then the instrumental block over the
-                                 instrumental planes alone (fp64 adds, componentwise accuracy as
-                                 before); -1 (default): the split when n_instr < 512, where the
-                                 lanes of one instruction contend for the few accumulators
-                                 (measured on B200 at 1e8 rows, 60 columns: 6.0 against 8.5 ms),
-                                 else the sweep (10 000 columns, 3e8 rows: 14.3 against 14.7)  */
+    GSR_OPT_APROD2_SPLIT = 5, /* how aprod2 (gsr_aprod2 and the two-pass iteration) runs.  1 or -1
+                                 (default): two launches -- astrometric + attitude + global blocks
+                                 over 152 B of every row with 24 warps per SM, then the
+                                 instrumental block over the instrumental planes alone (fp64
+                                 adds for an arbitrary y, componentwise accuracy as before; the
+                                 solver's own calls, which know ||y||, use the exact fixed-point
+                                 pass of GSR_OPT_FIXED_POINT there); 0: one launch that does all
+                                 four blocks (Algorithm 2 as one sweep).  Measured on B200, split
+                                 against sweep: 14.0 / 14.8 ms at 3e8 rows x 10 000 instrumental
+                                 columns, 4.2 / 5.5 ms at 1e8 x 6000, 4.9 / 9.6 ms at 1e8 x 60     */
     GSR_OPT_WHILE_GRAPH = 6   /* 1: the whole iteration loop of gsr_lsqr_solve is ONE CUDA graph
                                  launch -- a conditional WHILE node whose body is the iteration
                                  and whose condition a device kernel sets from the stop flag --

@@ -402,8 +402,17 @@ __global__ void __launch_bounds__(TPB) k_aprod1(const unsigned char* __restrict_
 // read-modify-writes, and this kernel streams 152 instead of 212 bytes per row.  With PERM the
 // scaled y of every internal row is also written to yint, so that the instrumental pass reads it
 // contiguously instead of gathering it a second time.
+// Warps per CTA of the main launch (INSTR = false).  Without the instrumental accumulators that
+// launch is bound by the latency of its serial per-tile chains, not by a pipe (ncu at 16 warps:
+// LSU 68 %, DRAM 65 %), and with 24 warps it still fits the register file (80 registers, no
+// spills) and shared memory (24 windows).  Measured at cfg3, main launch + fixed-point pass:
+// 13.9 / 13.1 / 12.7 / 13.4 ms for 16 / 20 / 24 / 28 warps.
+#ifndef GSR_NW_MAIN
+#define GSR_NW_MAIN 24
+#endif
+constexpr int NWARP_MAIN = GSR_NW_MAIN;
 template <bool SQUARE, bool PERM, bool INSTR>
-__global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict__ tiles,
+__global__ void __launch_bounds__(INSTR ? TPB : NWARP_MAIN * 32) k_aprod2(const unsigned char* __restrict__ tiles,
                                                const Unit* __restrict__ units, int n_units,
                                                int* __restrict__ counter,
                                                const double* __restrict__ y, double* __restrict__ x,
@@ -415,14 +424,15 @@ __global__ void __launch_bounds__(TPB) k_aprod2(const unsigned char* __restrict_
     extern __shared__ double sm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int ipad = INSTR ? (I + 1) & ~1 : 0;
+    constexpr int NW = INSTR ? NWARP : NWARP_MAIN;
     double* xi = sm;
     double* xw = sm + ipad + warp * 3 * ws;
-    double* ysm = sm + ipad + NWARP * 3 * ws + warp * 32;   // y of the current tile by
+    double* ysm = sm + ipad + NW * 3 * ws + warp * 32;   // y of the current tile by
                                                   // attitude slot: wide shared-memory broadcasts
                                                   // cost the LSU pipe less than shuffles
     // small I: one private copy of the instrumental accumulator per warp (copies 1.. behind the
     // y tiles), so that only lanes of the same instruction contend for an address (config 4)
-    double* xcopies = sm + ipad + NWARP * 3 * ws + NWARP * 32;
+    double* xcopies = sm + ipad + NW * 3 * ws + NW * 32;
     if (INSTR) {
         for (int i = threadIdx.x; i < I; i += TPB) xi[i] = 0.0;
         for (int i = threadIdx.x; i < (ncopy - 1) * ipad; i += TPB) xcopies[i] = 0.0;
@@ -749,7 +759,7 @@ static size_t instr_smem(const gsr_matrix* A) {
 }
 
 // shared memory of k_aprod2<., ., INSTR = false>: the windows and the y tiles only
-static int aprod2_main_smem(const gsr_matrix* A) { return NWARP * 3 * A->wstride * 8 + NWARP * 32 * 8; }
+static int aprod2_main_smem(const gsr_matrix* A) { return NWARP_MAIN * 3 * A->wstride * 8 + NWARP_MAIN * 32 * 8; }
 
 template <typename K>
 static int set_smem(K kernel, int bytes) {
@@ -799,7 +809,7 @@ int configure_product_kernels(gsr_matrix* A) {
     A->grid2 = A->sm_count * resident_ctas(k_aprod2<false, false, true>, A);
     {
         int nb = 1;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_aprod2<false, false, false>, TPB, aprod2_main_smem(A)) != cudaSuccess || nb < 1) {
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_aprod2<false, false, false>, NWARP_MAIN * 32, aprod2_main_smem(A)) != cudaSuccess || nb < 1) {
             cudaGetLastError();
             nb = 1;
         }
@@ -890,18 +900,19 @@ static int aprod2_view(const gsr_matrix* A, const TileView& v, const double* y, 
     }
     // two launches (default): everything but the instrumental block, then the instrumental pass
     // over the instrumental planes alone (fp64 adds: a caller's y has no norm bound to scale by)
-    const int grid = grid_for(A->grid2_main, nu);
+    const int need_main = (nu + NWARP_MAIN - 1) / NWARP_MAIN;
+    const int grid = A->grid2_main < need_main ? A->grid2_main : (need_main > 0 ? need_main : 1);
     const int smem = aprod2_main_smem(A);
     const double* yi = y + v.t0 * R;   // internal order: the view's slice of y
     const double* syi = sy;
     if (perm) {
         if (!A->yint) return GSR_ESTATE;
-        k_aprod2<false, true, false><<<grid, TPB, smem, s>>>(
+        k_aprod2<false, true, false><<<grid, NWARP_MAIN * 32, smem, s>>>(
             v.base, un, nu, A->unit_counter, y, x, sy, perm, S, D, I, A->win, A->wstride, 1, stop, A->yint);
         yi = A->yint + v.t0 * R;       // already scaled
         syi = nullptr;
     } else {
-        k_aprod2<false, false, false><<<grid, TPB, smem, s>>>(
+        k_aprod2<false, false, false><<<grid, NWARP_MAIN * 32, smem, s>>>(
             v.base, un, nu, A->unit_counter, y, x, sy, nullptr, S, D, I, A->win, A->wstride, 1, stop, nullptr);
     }
     count_launch();

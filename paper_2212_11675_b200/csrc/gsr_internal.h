@@ -329,14 +329,15 @@ int launch_fused_streamed(const gsr_matrix* A, const double* v, double* u, const
 int launch_det_finish(const gsr_matrix* A, double* t, const int* det_e, const double* ss,
                       const int* stop, cudaStream_t s);
 int configure_product_kernels(gsr_matrix* A);
-// aprod2 as two launches (main sweep + instrumental pass)?  Auto: when the instrumental block is
-// so narrow that the lanes of one instruction contend for its accumulators (measured: I = 60,
-// one sweep 8.5 ms, split 6.0 ms at 1e8 rows; I = 6000 / 10 000: 4.84 / 14.3 against 5.25 / 14.7)
+// aprod2 as two launches (main launch + instrumental pass)?  Default (auto): yes.  With 24 warps
+// per CTA the main launch is 13 % faster than with 16, which the one-sweep kernel cannot have (its
+// fp64 accumulators need 113 registers), and the compare-and-swap adds no longer share the LSU
+// pipe with the attitude read-modify-writes.  Measured on B200 with real vectors, split against
+// one sweep (ms): cfg3 14.0 / 14.8, cfg2 4.23 / 5.46, 1.28e8 rows x 600 columns 5.53 / 6.85,
+// cfg4 (60 columns) 4.9 / 9.6.
 // (the solver's aprod2 with a known norm: main launch + fixed-point instrumental pass)
 inline bool aprod2_fixed_split(const gsr_matrix* A) { return A->p != nullptr && !A->opt_no_fixed; }
-inline bool aprod2_is_split(const gsr_matrix* A) {
-    return A->opt_aprod2_split == 2 || (A->opt_aprod2_split == 0 && A->dims.n_instr < 512);
-}
+inline bool aprod2_is_split(const gsr_matrix* A) { return A->opt_aprod2_split != 1; }
 
 // One pass over the matrix: f(view) for the resident run of units, then for every streamed
 // chunk (double-buffered H2D copies on the copy stream, overlapped with f of the previous view).

@@ -96,7 +96,7 @@ def test_aprod1_parity(sysm):
 def test_aprod2_parity(sysm, split):
     """Algorithm 2 through the C ABI: as two launches (GSR_OPT_APROD2_SPLIT = 1:
     the instrumental block in a pass of its own), as one sweep over all four blocks (0), and in
-    the default setting (-1: the split for narrow instrumental blocks)."""
+    the default setting (-1 = the split)."""
     b = _binding()
     y = inputs.random_vector(sysm.cfg, 3, sysm.m)
     x0 = inputs.random_vector(sysm.cfg, 4, sysm.n)
@@ -109,7 +109,7 @@ def test_aprod2_parity(sysm, split):
         launches = b.gsr_launch_count() - n0
     finally:
         b.gsr_set_option(sysm.A.h, b.GSR_OPT_APROD2_SPLIT, -1)
-    two = split == 1 or (split == -1 and sysm.cfg.n_instr < 512)      # -1: by the width of the block
+    two = split != 0                                                  # -1 (default) = the split
     assert launches == (2 if two else 1) or sysm.m == 0, launches     # the form asked for really ran
     err = np.abs(xd.cpu().numpy() - x_ref)
     assert np.all(err <= APROD_TOL * np.maximum(scale, 1e-300)), float((err / scale).max())
