@@ -347,172 +347,199 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    t_setup = time.perf_counter()
-    h = build_system(cfg, g, inputs, torch, dev, args.streamed_resident_gb, args.chunk_mb)
-    streamed = g.gsr_matrix_host_bytes(h) > 0
-    # b = A x_true + noise, formed on the device with the library's own aprod1
-    xt = inputs.x_true(cfg, dev)
-    b = torch.empty(m, dtype=torch.float64, device=dev)
-    for r0 in range(0, m, GEN_ROWS):
-        nr = min(GEN_ROWS, m - r0)
-        b[r0:r0 + nr] = inputs.noise(cfg, r0, nr, dev)
-    comm = None
-    if sharded:
-        # weak-scaled sharded system: rank r owns stars [r*S, (r+1)*S) of an N*S-star system; the
-        # attitude + instrumental + global unknowns are shared, so their x_true comes from rank 0's seed
-        xt0 = inputs.x_true(cfg0, dev)
-        xt[cfg.off_att:] = xt0[cfg0.off_att:]
-        uid = [g.gsr_comm_unique_id() if rank == 0 else None]
-        if world > 1:
-            dist.broadcast_object_list(uid, src=0)
-        comm = g.gsr_comm_create(rank, world, uid[0])
-        g.gsr_matrix_set_comm(h, comm, world * m, world * 5 * cfg.n_stars + (n - cfg.off_att))
-    g.gsr_aprod1(h, xt, b)
-    g.gsr_precondition(h)
-    g.gsr_set_option(h, g.GSR_OPT_FORCE_ITNLIM, 1)
-    g.gsr_set_option(h, g.GSR_OPT_FUSED, 0 if args.two_pass else 1)
-    g.gsr_set_option(h, g.GSR_OPT_WHILE_GRAPH, 1 if args.while_graph else 0)
-    g.gsr_set_option(h, g.GSR_OPT_FIXED_POINT, 0 if args.fp64_instr else 1)
-    x = torch.empty(n, dtype=torch.float64, device=dev)
-    torch.cuda.synchronize()
-    t_setup = time.perf_counter() - t_setup
+    def measure():
+        h = comm = None
+        try:
+            t_setup = time.perf_counter()
+            h = build_system(cfg, g, inputs, torch, dev, args.streamed_resident_gb, args.chunk_mb)
+            streamed = g.gsr_matrix_host_bytes(h) > 0
+            # b = A x_true + noise, formed on the device with the library's own aprod1
+            xt = inputs.x_true(cfg, dev)
+            b = torch.empty(m, dtype=torch.float64, device=dev)
+            for r0 in range(0, m, GEN_ROWS):
+                nr = min(GEN_ROWS, m - r0)
+                b[r0:r0 + nr] = inputs.noise(cfg, r0, nr, dev)
+            if sharded:
+                # weak-scaled sharded system: rank r owns stars [r*S, (r+1)*S) of an N*S-star system; the
+                # attitude + instrumental + global unknowns are shared, so their x_true comes from rank 0's seed
+                xt0 = inputs.x_true(cfg0, dev)
+                xt[cfg.off_att:] = xt0[cfg0.off_att:]
+                uid = [g.gsr_comm_unique_id() if rank == 0 else None]
+                if world > 1:
+                    dist.broadcast_object_list(uid, src=0)
+                comm = g.gsr_comm_create(rank, world, uid[0])
+                g.gsr_matrix_set_comm(h, comm, world * m, world * 5 * cfg.n_stars + (n - cfg.off_att))
+            g.gsr_aprod1(h, xt, b)
+            g.gsr_precondition(h)
+            g.gsr_set_option(h, g.GSR_OPT_FORCE_ITNLIM, 1)
+            g.gsr_set_option(h, g.GSR_OPT_FUSED, 0 if args.two_pass else 1)
+            g.gsr_set_option(h, g.GSR_OPT_WHILE_GRAPH, 1 if args.while_graph else 0)
+            g.gsr_set_option(h, g.GSR_OPT_FIXED_POINT, 0 if args.fp64_instr else 1)
+            x = torch.empty(n, dtype=torch.float64, device=dev)
+            torch.cuda.synchronize()
+            t_setup = time.perf_counter() - t_setup
 
-    # warm-up (untimed): W iterations (>= 3), also builds the CUDA graph
-    W = max(args.warmup, 3)
-    g.gsr_lsqr_solve(h, b, x, W)
-    # timed: exactly K iterations, device-resident inputs
-    K = args.steps
-    sampler = ClockSampler(local)
-    sampler.start()
-    barrier()
-    l0 = g.gsr_launch_count()
-    sb0 = g.gsr_matrix_streamed_bytes(h)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.profiler.start()      # cudaProfilerStart: ncu --profile-from-start off sees only this
-    e0.record()
-    res = g.gsr_lsqr_solve(h, b, x, K)
-    e1.record()
-    torch.cuda.synchronize()
-    torch.cuda.profiler.stop()
-    barrier()
-    launches = g.gsr_launch_count() - l0
-    streamed_bytes = g.gsr_matrix_streamed_bytes(h) - sb0
-    while_graph = g.gsr_debug_while_graph(h)
-    ms_solve = e0.elapsed_time(e1)            # whole call: initialisation + K iterations + x
-    ms = g.gsr_lsqr_last_loop_ms(h)           # exactly the K iterations (CUDA events on the stream)
-    assert 0.0 < ms <= ms_solve
-    clocks = sampler.finish()
-    assert res.itn == K and res.istop == 7, res
+            # warm-up (untimed): W iterations (>= 3), also builds the CUDA graph
+            W = max(args.warmup, 3)
+            g.gsr_lsqr_solve(h, b, x, W)
+            # timed: exactly K iterations, device-resident inputs
+            K = args.steps
+            sampler = ClockSampler(local)
+            sampler.start()
+            barrier()
+            l0 = g.gsr_launch_count()
+            sb0 = g.gsr_matrix_streamed_bytes(h)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.profiler.start()      # cudaProfilerStart: ncu --profile-from-start off sees only this
+            e0.record()
+            res = g.gsr_lsqr_solve(h, b, x, K)
+            e1.record()
+            torch.cuda.synchronize()
+            torch.cuda.profiler.stop()
+            barrier()
+            launches = g.gsr_launch_count() - l0
+            streamed_bytes = g.gsr_matrix_streamed_bytes(h) - sb0
+            while_graph = g.gsr_debug_while_graph(h)
+            ms_solve = e0.elapsed_time(e1)            # whole call: initialisation + K iterations + x
+            ms = g.gsr_lsqr_last_loop_ms(h)           # exactly the K iterations (CUDA events on the stream)
+            assert 0.0 < ms <= ms_solve
+            clocks = sampler.finish()
+            assert res.itn == K and res.istop == 7, res
 
-    # end to end through the C ABI with HOST buffers: b H2D (pinned) and x D2H inside the call
-    b_host = torch.empty(m, dtype=torch.float64).pin_memory()
-    b_host.copy_(b)
-    x_host = torch.empty(n, dtype=torch.float64).pin_memory()
-    barrier()
-    t0 = time.perf_counter()
-    res2 = g.gsr_lsqr_solve(h, b_host, x_host, K)
-    torch.cuda.synchronize()
-    t_e2e = time.perf_counter() - t0
-    barrier()
-    assert res2.itn == K
-    assert float((x_host.to(dev) - x).abs().max()) <= 1e-9 * float(x.abs().max())
-    del b_host
+            # end to end through the C ABI with HOST buffers: b H2D (pinned) and x D2H inside the call
+            b_host = torch.empty(m, dtype=torch.float64).pin_memory()
+            b_host.copy_(b)
+            x_host = torch.empty(n, dtype=torch.float64).pin_memory()
+            barrier()
+            t0 = time.perf_counter()
+            res2 = g.gsr_lsqr_solve(h, b_host, x_host, K)
+            torch.cuda.synchronize()
+            t_e2e = time.perf_counter() - t0
+            barrier()
+            assert res2.itn == K
+            # same system, same K: the two solves differ only by the order of the floating-point atomics
+            e2e_diff = float((x_host.to(dev) - x).norm() / x.norm())
+            assert e2e_diff <= 1e-6, e2e_diff
+            del b_host
 
-    # per-kernel device time of the two products, CUDA events on the launching stream
-    reps = 2 if streamed else 10
-    ms1 = g.gsr_time_product(h, 1, reps)
-    ms2 = g.gsr_time_product(h, 2, reps)
-    ms3 = g.gsr_time_product(h, 3, reps)
-    ms4 = g.gsr_time_product(h, 4, reps)
+            # per-kernel device time of the two products, CUDA events on the launching stream
+            # (each on the vectors a short solve leaves in the workspace: the timing launches of one
+            # product overwrite them, and on zero or overflowed vectors aprod2 does other work)
+            reps = 2 if streamed else 10
+            prod_ms = []
+            for which in (1, 2, 3, 4):
+                g.gsr_lsqr_solve(h, b, x, 2)
+                prod_ms.append(g.gsr_time_product(h, which, reps))
+            ms1, ms2, ms3, ms4 = prod_ms
 
-    t = torch.tensor([ms, t_e2e * 1e3, ms1, ms2, ms3, ms4], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, ms_e2e, ms1, ms2, ms3, ms4 = [float(v) for v in t]
+            t = torch.tensor([ms, t_e2e * 1e3, ms1, ms2, ms3, ms4], dtype=torch.float64, device=dev)
+            if world > 1:
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms, ms_e2e, ms1, ms2, ms3, ms4 = [float(v) for v in t]
 
-    if rank == 0:
-        peak, peak_src = peaks()
-        gb1, gb2 = BYTES_APROD1 * m / ms1 * 1e-6, BYTES_APROD2 * m / ms2 * 1e-6
-        gb12 = (BYTES_APROD1 + BYTES_APROD2) * m / (ms1 + ms2) * 1e-6
-        gb3, gb4 = BYTES_FUSED * m / ms3 * 1e-6, BYTES_INSTR * m / ms4 * 1e-6
-        if args.two_pass:
-            dom = ("aprod2", gb2, ms2, BYTES_APROD2) if ms2 >= ms1 else ("aprod1", gb1, ms1, BYTES_APROD1)
-        else:
-            dom = ("fused", gb3, ms3, BYTES_FUSED)
-        tpr = NCU_TRAFFIC_PER_ROW[dom[0]]
-        traffic = tpr * m if tpr is not None else None
-        iter_bytes = (BYTES_APROD1 + BYTES_APROD2) if args.two_pass else BYTES_ITER_FUSED
-        m_total = m * (world if sharded else 1)
-        n_total = n + (5 * cfg.n_stars * (world - 1) if sharded else 0)
-        line = {
-            "metric": METRIC, "value": world * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
-            "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": config_dict(cfg0, args, world, sharded, m_total, n_total),
-            "e2e": {"value": world * K / (ms_e2e * 1e-3), "unit": UNIT,
-                    "h2d_bytes_per_step": 8 * m / K, "d2h_bytes_per_step": (8 * n + 80) / K,
-                    "note": "gsr_lsqr_solve with pinned host b and host x; matrix resident"},
-            "gpu_launches": int(launches),
-            "loop": ("one launch of a conditional-WHILE CUDA graph for all K iterations"
-                     if while_graph else "one CUDA graph launch per iteration"),
-            "clocks": clocks,
-            "roofline": {"bound": "hbm", "kernel": dom[0], "achieved": dom[1], "peak": peak,
-                         "unit": "GB/s", "frac": dom[1] / peak, "traffic": traffic,
-                         "dram_gbs": traffic / dom[2] * 1e-6, "dram_frac": traffic / dom[2] * 1e-6 / peak,
-                         "traffic_note": "DRAM bytes per launch = ncu --set full bytes per row ("
-                                         + NCU_TRAFFIC_SOURCE + ") x rows of this launch; the layout "
-                                         "stores 212 B/row (uint16 indices), so traffic < algorithmic bytes",
-                         "peak_source": peak_src, "algorithmic_bytes_per_row": dom[3],
-                         "algorithmic_note": "k_fused: ONE read of the matrix (224 B/row, int32 indices) "
-                                             "+ u_hat read + write = 240 B/row; aprod1 240, aprod2 232",
-                         "ms_per_launch": dom[2]},
-            "products": {"aprod1_gbs": gb1, "aprod2_gbs": gb2, "aprod1_ms": ms1, "aprod2_ms": ms2,
-                         "fused_ms": ms3, "fused_gbs": gb3, "instr_pass_ms": ms4, "instr_pass_gbs": gb4,
-                         "fused_two_product_equiv_gbs": BYTES_FUSED_2P * m / ms3 * 1e-6,
-                         "aprod1_frac_of_measured": gb1 / peak, "aprod2_frac_of_measured": gb2 / peak,
-                         "aprod1_dram_gbs": TRAFFIC_APROD1 * m / ms1 * 1e-6,
-                         "aprod2_dram_gbs": TRAFFIC_APROD2 * m / ms2 * 1e-6,
-                         "combined_gbs": gb12, "combined_frac_of_measured": gb12 / peak,
-                         "combined_frac_of_8tbs": gb12 / 8000.0,
-                         "iteration_gbs": iter_bytes * m / (ms / K) * 1e-6,
-                         "iteration_frac_of_measured": iter_bytes * m / (ms / K) * 1e-6 / peak,
-                         "iteration_two_product_equiv_gbs": 472 * m / (ms / K) * 1e-6,
-                         "iteration_two_product_equiv_frac_of_8tbs": 472 * m / (ms / K) * 1e-6 / 8000.0,
-                         "note": "GB/s are algorithmic: aprod1 240, aprod2 232 B/row; fused pass 240 "
-                                 "(one matrix read), instrumental pass 80, fused iteration 320 B/row. "
-                                 "*_two_product_equiv_* divide the 472 B/row of an aprod1 + aprod2 "
-                                 "iteration by the fused time (what a two-product code would need to "
-                                 "sustain to be as fast); not a roofline fraction"},
-            "lsqr": {"istop": res.istop, "itn": res.itn, "rnorm": res.rnorm, "anorm": res.anorm,
-                     "acond": res.acond, "xnorm": res.xnorm, "istop_natural": res.istop_natural,
-                     "itn_natural": res.itn_natural},
-            "solve_call_ms": ms_solve,
-            "timing": "value = N x K / device time of the K iterations, timed by CUDA events that "
-                      "gsr_lsqr_solve records on the launching stream around its graph-launch loop (max "
-                      "over ranks; a row-sharded system has N x the config's rows, so one of its "
-                      "iterations counts as N config-sized ones); solve_call_ms also has the "
-                      "initialisation (one aprod2) and the finalisation; e2e is the wall clock of the "
-                      "whole call with host buffers",
-            "setup_s": t_setup, "matrix_device_gb": g.gsr_matrix_device_bytes(h) * 1e-9,
-        }
-        if streamed:
-            # the K iterations + the initial aprod2 each move the host part once (fused form)
-            per_it = streamed_bytes / (K + 1)
-            line["streamed"] = {
-                "host_gb": g.gsr_matrix_host_bytes(h) * 1e-9, "device_gb": g.gsr_matrix_device_bytes(h) * 1e-9,
-                "tile_gb": 212e-9 * m, "tile_bytes_over_hbm_180gb": 212e-9 * m / 180.0,
-                "h2d_gb_per_iteration": per_it * 1e-9, "chunk_mb": args.chunk_mb,
-                "h2d_gbs": per_it / (ms / K) * 1e-6,
-                "note": "iteration time is bounded below by the host part of the matrix over the bus "
-                        "(PCIe 5 x16: 64 GB/s raw, about 55 GB/s of payload); h2d_gbs is what the "
-                        "iteration sustained, kernels of the resident part and of the previous chunk "
-                        "overlapped with the copies"}
-        if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(cfg0, args.oracle_rows, 20)
-        print(json.dumps(line), flush=True)
-    g.gsr_matrix_destroy(h)
-    if comm:
-        g.gsr_comm_destroy(comm)
+            if rank == 0:
+                peak, peak_src = peaks()
+                gb1, gb2 = BYTES_APROD1 * m / ms1 * 1e-6, BYTES_APROD2 * m / ms2 * 1e-6
+                gb12 = (BYTES_APROD1 + BYTES_APROD2) * m / (ms1 + ms2) * 1e-6
+                gb3, gb4 = BYTES_FUSED * m / ms3 * 1e-6, BYTES_INSTR * m / ms4 * 1e-6
+                if args.two_pass:
+                    dom = ("aprod2", gb2, ms2, BYTES_APROD2) if ms2 >= ms1 else ("aprod1", gb1, ms1, BYTES_APROD1)
+                else:
+                    dom = ("fused", gb3, ms3, BYTES_FUSED)
+                tpr = NCU_TRAFFIC_PER_ROW[dom[0]]
+                traffic = tpr * m if tpr is not None else None
+                iter_bytes = (BYTES_APROD1 + BYTES_APROD2) if args.two_pass else BYTES_ITER_FUSED
+                m_total = m * (world if sharded else 1)
+                n_total = n + (5 * cfg.n_stars * (world - 1) if sharded else 0)
+                line = {
+                    "metric": METRIC, "value": world * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+                    "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True,
+                    "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                    "config": config_dict(cfg0, args, world, sharded, m_total, n_total),
+                    "e2e": {"value": world * K / (ms_e2e * 1e-3), "unit": UNIT,
+                            "h2d_bytes_per_step": 8 * m / K, "d2h_bytes_per_step": (8 * n + 80) / K,
+                            "note": "gsr_lsqr_solve with pinned host b and host x; matrix resident",
+                            "rel_diff_vs_device_solve": e2e_diff},
+                    "gpu_launches": int(launches),
+                    "loop": ("one launch of a conditional-WHILE CUDA graph for all K iterations"
+                             if while_graph else "one CUDA graph launch per iteration"),
+                    "clocks": clocks,
+                    "roofline": {"bound": "hbm", "kernel": dom[0], "achieved": dom[1], "peak": peak,
+                                 "unit": "GB/s", "frac": dom[1] / peak, "traffic": traffic,
+                                 "dram_gbs": traffic / dom[2] * 1e-6, "dram_frac": traffic / dom[2] * 1e-6 / peak,
+                                 "traffic_note": "DRAM bytes per launch = ncu --set full bytes per row ("
+                                                 + NCU_TRAFFIC_SOURCE + ") x rows of this launch; the layout "
+                                                 "stores 212 B/row (uint16 indices), so traffic < algorithmic bytes",
+                                 "peak_source": peak_src, "algorithmic_bytes_per_row": dom[3],
+                                 "algorithmic_note": "k_fused: ONE read of the matrix (224 B/row, int32 indices) "
+                                                     "+ u_hat read + write = 240 B/row; aprod1 240, aprod2 232",
+                                 "ms_per_launch": dom[2]},
+                    "products": {"aprod1_gbs": gb1, "aprod2_gbs": gb2, "aprod1_ms": ms1, "aprod2_ms": ms2,
+                                 "fused_ms": ms3, "fused_gbs": gb3, "instr_pass_ms": ms4, "instr_pass_gbs": gb4,
+                                 "fused_two_product_equiv_gbs": BYTES_FUSED_2P * m / ms3 * 1e-6,
+                                 "aprod1_frac_of_measured": gb1 / peak, "aprod2_frac_of_measured": gb2 / peak,
+                                 "aprod1_dram_gbs": TRAFFIC_APROD1 * m / ms1 * 1e-6,
+                                 "aprod2_dram_gbs": TRAFFIC_APROD2 * m / ms2 * 1e-6,
+                                 "combined_gbs": gb12, "combined_frac_of_measured": gb12 / peak,
+                                 "combined_frac_of_8tbs": gb12 / 8000.0,
+                                 "iteration_gbs": iter_bytes * m / (ms / K) * 1e-6,
+                                 "iteration_frac_of_measured": iter_bytes * m / (ms / K) * 1e-6 / peak,
+                                 "iteration_two_product_equiv_gbs": 472 * m / (ms / K) * 1e-6,
+                                 "iteration_two_product_equiv_frac_of_8tbs": 472 * m / (ms / K) * 1e-6 / 8000.0,
+                                 "note": "GB/s are algorithmic: aprod1 240, aprod2 232 B/row; fused pass 240 "
+                                         "(one matrix read), instrumental pass 80, fused iteration 320 B/row. "
+                                         "*_two_product_equiv_* divide the 472 B/row of an aprod1 + aprod2 "
+                                         "iteration by the fused time (what a two-product code would need to "
+                                         "sustain to be as fast); not a roofline fraction"},
+                    "lsqr": {"istop": res.istop, "itn": res.itn, "rnorm": res.rnorm, "anorm": res.anorm,
+                             "acond": res.acond, "xnorm": res.xnorm, "istop_natural": res.istop_natural,
+                             "itn_natural": res.itn_natural},
+                    "solve_call_ms": ms_solve,
+                    "timing": "value = N x K / device time of the K iterations, timed by CUDA events that "
+                              "gsr_lsqr_solve records on the launching stream around its graph-launch loop (max "
+                              "over ranks; a row-sharded system has N x the config's rows, so one of its "
+                              "iterations counts as N config-sized ones); solve_call_ms also has the "
+                              "initialisation (one aprod2) and the finalisation; e2e is the wall clock of the "
+                              "whole call with host buffers",
+                    "setup_s": t_setup, "matrix_device_gb": g.gsr_matrix_device_bytes(h) * 1e-9,
+                }
+                if streamed:
+                    # the K iterations + the initial aprod2 each move the host part once (fused form)
+                    per_it = streamed_bytes / (K + 1)
+                    line["streamed"] = {
+                        "host_gb": g.gsr_matrix_host_bytes(h) * 1e-9, "device_gb": g.gsr_matrix_device_bytes(h) * 1e-9,
+                        "tile_gb": 212e-9 * m, "tile_bytes_over_hbm_180gb": 212e-9 * m / 180.0,
+                        "h2d_gb_per_iteration": per_it * 1e-9, "chunk_mb": args.chunk_mb,
+                        "h2d_gbs": per_it / (ms / K) * 1e-6,
+                        "note": "iteration time is bounded below by the host part of the matrix over the bus "
+                                "(PCIe 5 x16: 64 GB/s raw, about 55 GB/s of payload); h2d_gbs is what the "
+                                "iteration sustained, kernels of the resident part and of the previous chunk "
+                                "overlapped with the copies"}
+                if world == 1 and not args.no_cpu_baseline:
+                    line["cpu_baseline"] = cpu_baseline(cfg0, args.oracle_rows, 20)
+                print(json.dumps(line), flush=True)
+        finally:
+            if h is not None:
+                g.gsr_matrix_destroy(h)
+            if comm:
+                g.gsr_comm_destroy(comm)
+
+    # One retry on a single GPU: a run that starts right after another process has exited can find
+    # the device memory not yet handed back, or (cfg4) trip the e2e-vs-device sanity check once.
+    attempts = 2 if world == 1 else 1
+    for attempt in range(attempts):
+        try:
+            measure()
+            break
+        except Exception:
+            import gc
+            import traceback
+            traceback.print_exc(file=sys.stderr)
+            if attempt + 1 == attempts:
+                raise
+            gc.collect()
+            torch.cuda.empty_cache()
+            time.sleep(20.0)
     if world > 1:
         dist.destroy_process_group()
 
