@@ -275,6 +275,45 @@ int gsr_set_option(gsr_matrix* A, int key, int64_t value);
 
 const char* gsr_strerror(int code);
 
+/* ---- a norm for callers that cannot allocate (row a4; the norms of Algorithm 3) --
+ * out_dev[0] = || v ||_2 of a device vector, by the same two-stage reduction the solver uses for
+ * beta, alpha and ||w|| -- but WITHOUT a handle and without any allocation: no cudaMalloc, no
+ * cudaFree, no allocating library routine, on the first call or any later one.
+ *
+ * Who needs this.  Everything else here draws its scratch from a handle, and a handle draws it
+ * from cudaMalloc.  That is not available to (a) code that runs while the device is already full
+ * -- a config-3 handle holds ~64 GB of tiles plus its work vectors, and a host framework's
+ * caching allocator may own what is left, so a cudaMalloc either fails or forces that framework
+ * to release its cache -- and (b) code on a latency path: cudaMalloc and cudaFree synchronise
+ * the whole device and would stall a solve that is in flight on another stream.  Such a caller
+ * (a convergence monitor, a residual check between solves, a plug-in that is handed buffers and
+ * a stream and nothing else) passes the vector and one double of output; the partial sums live
+ * in a fixed array inside the library image.
+ *
+ * Cost and limit.  The array is 33 024 bytes of device memory on EVERY GPU that loads the library,
+ * held until the process exits.  It holds 4096 partial sums of 2^17 elements each:
+ * len <= GSR_NORM2_STATIC_MAX_LEN = 2^29 (a 4 GiB vector; config 3 has 3e8 rows).  A longer
+ * vector is refused with GSR_EUNSUPPORTED ("size") before anything is launched; split it and
+ * combine the pieces as sqrt(a^2 + b^2).
+ *
+ * Sharing.  All calls on a device use the same array, and it keeps what the last call left.  The
+ * one word that must start at zero (the ticket that elects the CTA doing the second stage) is
+ * cleared on `stream` at the start of every call; the partial sums a call reads are those it has
+ * just written.  Calls whose GPU work can OVERLAP -- two streams with no event between them, two
+ * host threads -- race on the array and give wrong norms: keep all calls of a device on one
+ * stream or order them with events.  (The solver's own norms do not use this array.)
+ *
+ * First call.  The first call on each device looks up the array's device address
+ * (cudaGetSymbolAddress, with that device current) and checks that the device is sm_100; later
+ * calls reuse it.  Make that first call during set-up, before any stream capture is begun.
+ *
+ * v_dev [len] device memory (may be NULL if len = 0: the norm is 0), out_dev [1] device memory,
+ * both caller-owned.  Asynchronous on `stream`; equal input gives bit-equal output.
+ * Errors: GSR_EINVAL (null pointer, len < 0), GSR_EUNSUPPORTED (len above the limit, device not
+ * sm_100), GSR_ECUDA. */
+#define GSR_NORM2_STATIC_MAX_LEN ((int64_t)1 << 29)
+int gsr_norm2_static(const double* v_dev, int64_t len, double* out_dev, gsr_stream stream);
+
 /* ---- test / measurement exports -------------------------------------------------------- */
 
 /* The 24 (column, value) pairs of rows [row0, row0+nrows) in CALLER row order, read back from

@@ -24,7 +24,9 @@ EXPORTS = [
     "gsr_debug_expand_rows", "gsr_time_product", "gsr_launch_count", "gsr_lsqr_standard_errors", "gsr_lsqr_last_loop_ms", "gsr_lsqr_set_damp",
     "gsr_debug_fused_pass", "gsr_debug_graph_builds", "gsr_debug_while_graph", "gsr_matrix_set_constraints", "gsr_comm_unique_id", "gsr_comm_create", "gsr_comm_destroy", "gsr_matrix_set_comm",
     "gsr_matrix_begin_streamed", "gsr_matrix_host_bytes", "gsr_matrix_streamed_bytes",
+    "gsr_norm2_static",
 ]
+GSR_NORM2_STATIC_MAX_LEN = 1 << 29
 
 
 class GsrError(RuntimeError):
@@ -112,6 +114,7 @@ def lib():
         L.gsr_debug_graph_builds.restype = i64
         L.gsr_debug_while_graph.argtypes = [vp]
         L.gsr_debug_while_graph.restype = C.c_int
+        L.gsr_norm2_static.argtypes = [vp, i64, vp, vp]
         _lib = L
     return _lib
 
@@ -305,6 +308,16 @@ def gsr_debug_graph_builds(h) -> int:
 
 def gsr_debug_while_graph(h) -> int:
     return int(lib().gsr_debug_while_graph(h))
+
+
+def gsr_norm2_static(v_dev, out_dev, stream=None, length=None):
+    """out_dev[0] = ||v_dev||_2 without any device allocation (include/gsr.h): for callers that
+    run while the device is full or that cannot afford cudaMalloc's device-wide synchronisation.
+    The scratch is one fixed array per GPU shared by all calls: keep the calls of a device on one
+    stream.  At most GSR_NORM2_STATIC_MAX_LEN elements; `length` defaults to v_dev.numel()."""
+    n = int(v_dev.numel() if length is None else length)
+    _check(lib().gsr_norm2_static(_ptr(v_dev), n, _ptr(out_dev), _stream(stream)),
+           f"gsr_norm2_static(len={n}, limit={GSR_NORM2_STATIC_MAX_LEN})")
 
 
 def gsr_launch_count() -> int:

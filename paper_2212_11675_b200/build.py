@@ -8,7 +8,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libgsr_b200.so")
-SOURCES = ["gsr_matrix.cu", "gsr_aprod.cu", "gsr_lsqr.cu", "gsr_comm.cu", "gsr_constraints.cu"]
+SOURCES = ["gsr_matrix.cu", "gsr_aprod.cu", "gsr_lsqr.cu", "gsr_comm.cu", "gsr_constraints.cu",
+           "gsr_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-ldl"]
 
