@@ -79,7 +79,42 @@ def parse():
                     help="row-sharded form (the default for N > 1; at N = 1 a one-rank NCCL communicator)")
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE config 5: time aprod1/aprod2 alone from 1e6 to 3e8 rows")
+    ap.add_argument("--launch-check", action="store_true",
+                    help="no GPU work: every rank joins a gloo group, rank 0 prints the number of ranks "
+                         "that answered (tests/test_bench_launch.py checks the --gpus N launcher with it)")
     return ap.parse_args()
+
+
+def free_port():
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def launch_ranks(args):
+    """`python bench.py --gpus N` outside torchrun (no WORLD_SIZE): start the N ranks ourselves, one
+    per GPU, exactly as the driver's torchrun line would, and hand their output through.  Rank 0
+    prints the one JSON line; NCCL's own lines go to stderr (see main)."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(free_port()),
+           os.path.abspath(__file__), *sys.argv[1:]]
+    return subprocess.call(cmd)
+
+
+def launch_check():
+    """The launcher's self-test: count the ranks that came up (gloo, CPU only)."""
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    n = torch.ones(1)
+    if world > 1:
+        dist.init_process_group("gloo")
+        dist.all_reduce(n)
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps({"launch_check": True, "n_gpus": world, "ranks_answered": int(n.item())}), flush=True)
 
 
 def peaks():
@@ -311,6 +346,10 @@ def run_sweep(args):
 
 def main():
     args = parse()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(launch_ranks(args))
+    if args.launch_check:
+        return launch_check()
     from paper_2212_11675_b200 import inputs
     cfg0 = inputs.named_config(args.config)
     if args.time_ordered:
@@ -347,7 +386,7 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    def measure():
+    def measure(retried=False):
         h = comm = None
         try:
             t_setup = time.perf_counter()
@@ -417,10 +456,24 @@ def main():
             t_e2e = time.perf_counter() - t0
             barrier()
             assert res2.itn == K
-            # same system, same K: the two solves differ only by the order of the floating-point atomics
+            # same system, same K: the two solves differ only by the order of the floating-point
+            # atomics.  How much that may move x is set by the Lanczos process, not by the kernels
+            # (reading A20; measured at cfg4: 4e-16 up to K = 50, 8e-14 at 75, 9e-10 at 100, and in
+            # deterministic mode bit-identical): the bar is 1e-9, or 20 x what ONE ULP of b moves the
+            # device solve itself, never above 1e-6.  Not retried.
             e2e_diff = float((x_host.to(dev) - x).norm() / x.norm())
-            assert e2e_diff <= 1e-6, e2e_diff
             del b_host
+            gen = torch.Generator(device=dev)
+            gen.manual_seed(12345 + rank)
+            ulp = torch.nextafter(b.abs(), torch.full_like(b, float("inf"))) - b.abs()
+            b_ulp = b + ulp * torch.randint(-1, 2, (m,), device=dev, generator=gen).double()
+            del ulp
+            x_ulp = torch.empty_like(x)
+            g.gsr_lsqr_solve(h, b_ulp, x_ulp, K)
+            one_ulp_sens = float((x_ulp - x).norm() / x.norm())
+            del b_ulp, x_ulp
+            e2e_bound = min(max(1e-9, 20.0 * one_ulp_sens), 1e-6)
+            assert e2e_diff <= e2e_bound, (e2e_diff, one_ulp_sens)
 
             # per-kernel device time of the two products, CUDA events on the launching stream
             # (each on the vectors a short solve leaves in the workspace: the timing launches of one
@@ -459,7 +512,8 @@ def main():
                     "e2e": {"value": world * K / (ms_e2e * 1e-3), "unit": UNIT,
                             "h2d_bytes_per_step": 8 * m / K, "d2h_bytes_per_step": (8 * n + 80) / K,
                             "note": "gsr_lsqr_solve with pinned host b and host x; matrix resident",
-                            "rel_diff_vs_device_solve": e2e_diff},
+                            "rel_diff_vs_device_solve": e2e_diff,
+                            "rel_diff_bound": e2e_bound, "one_ulp_of_b_moves_x_by": one_ulp_sens},
                     "gpu_launches": int(launches),
                     "loop": ("one launch of a conditional-WHILE CUDA graph for all K iterations"
                              if while_graph else "one CUDA graph launch per iteration"),
@@ -502,6 +556,7 @@ def main():
                               "initialisation (one aprod2) and the finalisation; e2e is the wall clock of the "
                               "whole call with host buffers",
                     "setup_s": t_setup, "matrix_device_gb": g.gsr_matrix_device_bytes(h) * 1e-9,
+                    "retried_after_enomem": retried,
                 }
                 if streamed:
                     # the K iterations + the initial aprod2 each move the host part once (fused form)
@@ -524,18 +579,19 @@ def main():
             if comm:
                 g.gsr_comm_destroy(comm)
 
-    # One retry on a single GPU: a run that starts right after another process has exited can find
-    # the device memory not yet handed back, or (cfg4) trip the e2e-vs-device sanity check once.
+    # One retry on a single GPU, for GSR_ENOMEM only: a run that starts right after another process
+    # has exited can find the device memory not yet handed back.  A failed assert is never retried;
+    # the line says whether a retry happened.
     attempts = 2 if world == 1 else 1
     for attempt in range(attempts):
         try:
-            measure()
+            measure(retried=attempt > 0)
             break
-        except Exception:
+        except g.GsrError as e:
             import gc
             import traceback
             traceback.print_exc(file=sys.stderr)
-            if attempt + 1 == attempts:
+            if e.code != g.GSR_ENOMEM or attempt + 1 == attempts:
                 raise
             gc.collect()
             torch.cuda.empty_cache()

@@ -99,7 +99,7 @@ int gsr_matrix_create(gsr_matrix** out, const gsr_dims* dims,
  *   GSR_EINVAL        n_rows < 0, n_stars < 1, n_dfa < 4, n_instr < 1, n_glob != 1;
  *                     n_cols = 5 S + 3 D + I + 1 >= 2^31 (int32 column indices);
  *                     n_rows >= 2^32 - 16 (uint32 row permutation; shard larger systems,
- *                     gsr_matrix_set_comm, or stream them, gsr_stream_*)
+ *                     gsr_matrix_set_comm, or stream them, gsr_matrix_begin_streamed)
  *   GSR_EUNSUPPORTED  n_instr > 27 520: the product kernels keep the whole instrumental block of
  *                     x (8 I bytes) in shared memory beside 32 attitude windows (227 KB per SM);
  *                     more than 4096 attitude bins: n_dfa - 3 > 4096 * bw, where the bin width bw
@@ -189,7 +189,11 @@ int gsr_lsqr_standard_errors(gsr_matrix* A, double* se_hd, gsr_stream stream);
  * constraint coefficients in the column norms and scales them too.
  * On a row shard (gsr_matrix_set_comm) every constraint row is given to exactly ONE rank (rank 0
  * is the natural owner; the others pass none), in that rank's LOCAL column numbering: it may
- * touch the owner's own astrometric columns and any replicated column.
+ * touch the owner's own astrometric columns and any replicated column.  After
+ * gsr_matrix_set_comm the call re-checks that n_rows_global still covers this rank's rows plus
+ * n_con (GSR_EINVAL otherwise).  Constraint rows on a shard have run through the library only with
+ * a one-rank communicator (no box with two GPUs was available); the world-2 case is covered by
+ * tests/test_sharding_gloo.py on the CPU, which restates the recurrences and does not call it.
  * Errors: GSR_EINVAL (bad row_ptr, column out of range), GSR_ESTATE.  Synchronous. */
 int gsr_matrix_set_constraints(gsr_matrix* A, int64_t n_con, const int64_t* row_ptr_hd,
                                const int32_t* col_hd, const double* val_hd);
@@ -262,8 +266,9 @@ enum {
                                  launch -- a conditional WHILE node whose body is the iteration
                                  and whose condition a device kernel sets from the stop flag --
                                  so neither the stop decision nor a launch crosses to the host
-                                 between iterations (config 1, launch-bound: 60.4 against 62.8 us
-                                 per iteration; immaterial at 1e8 rows and above).  Ignored with
+                                 between iterations (config 1, launch-bound: measured 60.5 against
+                                 59.0 us per iteration with per-iteration launches, i.e. no gain,
+                                 DESIGN.md 5.6; immaterial at 1e8 rows and above).  Ignored with
                                  a communicator or on a streamed handle.  0 (default): one
                                  graph launch per iteration, the stop flag polled from pinned
                                  memory every 32 (fixed-count mode: 256) -- the default because

@@ -11,7 +11,9 @@ import os
 from dataclasses import dataclass
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libgsr_b200.so")
+# GSR_B200_LIB: another build of the SAME sources (the -DGSR_BOUNDS_CHECK one of build.build);
+# never a fallback -- if the named file is missing, loading fails
+LIB_PATH = os.environ.get("GSR_B200_LIB") or os.path.join(_HERE, "libgsr_b200.so")
 
 GSR_OK, GSR_EINVAL, GSR_ENOMEM, GSR_ECUDA, GSR_ESTATE, GSR_EUNSUPPORTED, GSR_ERANGE = 0, -1, -2, -3, -4, -5, -6
 GSR_OPT_FORCE_ITNLIM, GSR_OPT_DETERMINISTIC, GSR_OPT_FUSED, GSR_OPT_FIXED_POINT = 1, 2, 3, 4

@@ -22,18 +22,22 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if force or _stale():
+def build(force: bool = False, verbose: bool = False, extra_flags=(), out: str | None = None) -> str:
+    """Build the library.  `extra_flags` (e.g. ["-DGSR_BOUNDS_CHECK"]: device asserts on the index
+    computations of the product kernels) and `out` give a second, instrumented library beside
+    the product one; binding.py loads it when GSR_B200_LIB names it (tests/test_gpu_bounds.py)."""
+    target = out or LIB
+    if force or out is not None or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [nvcc, *NVCC_FLAGS, "-I", os.path.join(_ROOT, "include"), "-I", CSRC, "-o", tmp,
+        tmp = target + f".tmp{os.getpid()}"
+        cmd = [nvcc, *NVCC_FLAGS, *extra_flags, "-I", os.path.join(_ROOT, "include"), "-I", CSRC, "-o", tmp,
                *[os.path.join(CSRC, s) for s in SOURCES]]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
             print(" ".join(cmd))
         subprocess.check_call(cmd)
-        os.replace(tmp, LIB)
-    return LIB
+        os.replace(tmp, target)
+    return target
 
 
 if __name__ == "__main__":

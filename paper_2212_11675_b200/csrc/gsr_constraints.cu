@@ -174,6 +174,9 @@ int gsr_matrix_set_constraints(gsr_matrix* A, int64_t n_con, const int64_t* row_
     if (!A || n_con < 0) return GSR_EINVAL;
     if (A->state != 1 || A->p != nullptr || A->ws.st != nullptr) return GSR_ESTATE;   // before precondition / solve
     if (n_con > 0 && !row_ptr_hd) return GSR_EINVAL;
+    // on a row shard gsr_matrix_set_comm was told the total number of rows: it must still cover
+    // this rank's observations and the constraint rows it is being given now
+    if (A->comm && A->m_global < A->dims.n_rows + n_con) return GSR_EINVAL;
     free_constraints(A);
     if (!A->comm) A->m_global = A->dims.n_rows;   // (sharded: gsr_matrix_set_comm was told the total)
     if (n_con == 0) return GSR_OK;

@@ -93,7 +93,7 @@ __global__ void __launch_bounds__(TB_N) k_scatter_rows(const double* __restrict_
 __global__ void __launch_bounds__(TB_N) k_sumsq(const double* __restrict__ v, int64_t len,
                                                 double* __restrict__ part, const int* __restrict__ stop,
                                                 int64_t split, double* __restrict__ parta) {
-    if (*stop) return;
+    if (stop && *stop) return;
     __shared__ double red[TB_N / 32];
     double q = 0.0, qa = 0.0;
     for (int64_t i = (int64_t)blockIdx.x * TB_N + threadIdx.x; i < len; i += (int64_t)gridDim.x * TB_N) {
@@ -407,6 +407,7 @@ int ensure_workspace(gsr_matrix* A) {
     GSR_TRY(dev_alloc(A, (void**)&W.st, sizeof(LsqrState)));
     GSR_CUDA_TRY(cudaMemset(W.u, 0, (size_t)(A->m_int + A->n_con) * 8));
     GSR_CUDA_TRY(cudaMemset(W.st, 0, sizeof(LsqrState)));
+    GSR_CUDA_TRY(cudaMemset(W.red, 0, 4 * 8));
     GSR_CUDA_TRY(cudaMallocHost((void**)&W.stop_host, 64));
     return GSR_OK;
 }
@@ -702,7 +703,9 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
         GSR_CUDA_TRY(cudaEventCreate(&W.ev1));
     }
     GSR_CUDA_TRY(cudaEventRecord(W.ev0, s));   // device time of the iterations alone (bench.py)
-    const int64_t batch = !use_graph ? 1 : A->opt_force_itnlim ? 256 : 32;
+    // (fixed-count mode never stops early; with a communicator every launch that follows the stop
+    // still runs its two all-reduces, so the stop flag is polled more often there)
+    const int64_t batch = !use_graph ? 1 : A->opt_force_itnlim ? 256 : A->comm ? 8 : 32;
     int64_t launched = 0;
     W.last_loop_while = use_graph && W.wgraph != nullptr && A->opt_while;
     if (W.last_loop_while) {
@@ -833,13 +836,23 @@ int gsr_time_product(gsr_matrix* A, int which, int reps, float* ms_avg, gsr_stre
         rc = launch_fused(A, W.v, W.u, A->coef_one, W.part_u, W.t, nullptr, nullptr, s);
         k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, A->n_units, W.red + 3, nullptr);
     }
+    // aprod2 as the solver runs it: on one GPU with the sum of u_hat^2, which sends the instrumental
+    // block through the fixed-point pass (its scale is 2^(61 - exponent of that sum)); on a row shard
+    // the solver's two-pass form does not exist and the fp64 pass is what is timed.  The sum is
+    // formed HERE from the u_hat in the workspace: red[3] of an earlier solve is stale once a
+    // which = 1 timing has overwritten u_hat, and a wrong scale lets the conversion saturate.
+    const bool with_ss = which == 2 && W.solved && !A->comm;
+    if (with_ss) {
+        k_sumsq<<<NB_N, TB_N, 0, s>>>(W.u, A->m_int, W.part_u, nullptr, 0, nullptr);
+        k_sum_partials<<<1, 1024, 0, s>>>(W.part_u, NB_N, W.red + 3, nullptr);
+    }
     for (int pass = 0; pass < 2 && rc == GSR_OK; ++pass) {   // pass 0: warm-up
         int nrep = pass == 0 ? 1 : reps;
         cudaEventRecord(e0, s);
         for (int i = 0; i < nrep && rc == GSR_OK; ++i) {
             if (which == 1) rc = launch_aprod1(A, W.v, W.u, A->coef_one, W.part_u, nullptr, nullptr, s);
             else if (which == 2)   // as the solver runs it: with the norm of u_hat of its last pass, if any
-                rc = launch_aprod2(A, W.u, W.v, A->coef_one, nullptr, nullptr, s, W.solved ? W.red + 3 : nullptr);
+                rc = launch_aprod2(A, W.u, W.v, A->coef_one, nullptr, nullptr, s, with_ss ? W.red + 3 : nullptr);
             else if (which == 3) rc = launch_fused(A, W.v, W.u, A->coef_one, W.part_u, W.t, nullptr, nullptr, s);
             else rc = launch_aprod2_instr(A, W.u, W.t, W.red + 3, nullptr, 0, s);
         }

@@ -31,6 +31,7 @@ constexpr int SN_MAX_PARTS = 4096;               // partial sums the array can h
 constexpr int SN_HEAD = 32;                      // doubles before the partials: word 0 = ticket
 static_assert(SN_CHUNK * SN_MAX_PARTS == GSR_NORM2_STATIC_MAX_LEN, "gsr.h states the limit");
 constexpr size_t STATIC_BYTES = (size_t)(SN_HEAD + SN_MAX_PARTS) * 8;
+static_assert(STATIC_BYTES == 33024, "gsr.h and README.md state the size of the array");
 
 // The scratch itself.  In DEVICE code this name is the array.  In HOST code it is only a stand-in
 // symbol: its host address is not a device address and must never be handed to a kernel (the kernel

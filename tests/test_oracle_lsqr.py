@@ -258,6 +258,23 @@ def test_variance_monotone_and_scaled_by_p():
     assert np.max(np.abs(r.var - var_ref)) <= 1e-11 * np.max(var_ref)
 
 
+def test_standard_errors_of_an_underdetermined_system_use_one_degree_of_freedom():
+    """m <= n: there are no residual degrees of freedom, and Paige & Saunders then divide by 1
+    (the `dof = 1` branch of orc_standard_errors): se_j = rnorm * sqrt(var_j), with var from the
+    dense projected inverse normal matrix as above."""
+    cfg, star, att, instr, vals = small_system(seed=9, counts=(3, 2, 4), n_dfa=6, n_instr=8)
+    o = make_oracle(cfg, star, att, instr, vals)
+    assert o.m == 9 and o.m < o.n
+    A = csr_from_raw(cfg, star, att, instr, vals)[0].toarray()
+    b = np.random.default_rng(8).standard_normal(o.m)
+    k = 4
+    r = o.lsqr(b, k, force_itnlim=True, want_se=True)
+    Q = _krylov_basis(A, b, k)
+    var_ref = np.einsum("ij,jk,ik->i", Q, np.linalg.inv(Q.T @ (A.T @ (A @ Q))), Q)
+    res = np.linalg.norm(b - A @ r.x)
+    assert np.allclose(r.se, res * np.sqrt(var_ref / 1.0), rtol=1e-9, atol=1e-12 * r.se.max())
+
+
 # ---- row f4: damping (Paige & Saunders' damp; the paper's solver is undamped)
 
 @pytest.mark.parametrize("damp", [0.3, 2.5])
