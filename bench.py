@@ -48,6 +48,10 @@ BYTES_ITER_FUSED = BYTES_FUSED + BYTES_INSTR    # 320 B/row per fused iteration
 NCU_TRAFFIC_PER_ROW = {"aprod1": 228.6, "aprod2": 221.1, "fused": 230.1, "aprod2_instr": 68.1}
 NCU_TRAFFIC_SOURCE = "profiles/r2_fused_ncu_full.md (k_fused), profiles/r2_aprod_ncu_full.md (products), cfg3"
 GEN_ROWS = 1 << 23                              # rows generated and appended per chunk
+# The oracle (OpenMP build, 16 host cores of a B200 box) on the WHOLE system, measured once by the
+# opt-in full-size parity job (profiles/r3_fullsize_parity.md): seconds for the config's own
+# iteration count.  Reported beside the sampled figure, which stays what the short default run times.
+ORACLE_FULL_SIZE = {"cfg2": (100, 81.2), "cfg3": (50, 138.2), "cfg4": (100, 83.2)}
 
 
 def parse():
@@ -79,6 +83,8 @@ def parse():
                     help="row-sharded form (the default for N > 1; at N = 1 a one-rank NCCL communicator)")
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE config 5: time aprod1/aprod2 alone from 1e6 to 3e8 rows")
+    ap.add_argument("--sweep-rows", default=None,
+                    help="--sweep: comma-separated row counts instead of the whole 1e6 ... 3e8 ladder")
     ap.add_argument("--launch-check", action="store_true",
                     help="no GPU work: every rank joins a gloo group, rank 0 prints the number of ranks "
                          "that answered (tests/test_bench_launch.py checks the --gpus N launcher with it)")
@@ -232,6 +238,11 @@ def cpu_baseline(cfg, rows, steps):
     allc = oracle_sample(cfg, rows, steps, omp=True)
     allc["one_core"] = {k: one[k] for k in ("value", "unit", "cores", "sample", "seconds")}
     allc["host"] = host_info()
+    if cfg.name in ORACLE_FULL_SIZE:
+        k, sec = ORACLE_FULL_SIZE[cfg.name]
+        allc["full_size_measured"] = {"value": k / sec, "unit": UNIT, "cores": 16, "iterations": k, "seconds": sec,
+                                      "source": "profiles/r3_fullsize_parity.md (whole system, not extrapolated; "
+                                                "recorded once, not re-timed by this run)"}
     return allc
 
 
@@ -301,6 +312,8 @@ def run_sweep(args):
     dev = torch.device("cuda", 0)
     peak, peak_src = peaks()
     sizes = [1_000_000 * 2 ** k for k in range(9)] + [300_000_000]
+    if args.sweep_rows:
+        sizes = [int(float(v)) for v in args.sweep_rows.split(",")]
     for m in sizes:
         cfg = inputs.named_config(f"cfg5_{m}")
         if args.time_ordered:
@@ -326,6 +339,22 @@ def run_sweep(args):
             e1.record()
             torch.cuda.synchronize()
             api.append(e0.elapsed_time(e1) / 5)
+        # the same products through the internal-order API: a caller that iterates converts once
+        # (gsr_vector_to_internal / _from_internal) and then pays no gather or scatter per product
+        yi = torch.empty(g.gsr_matrix_internal_rows(h), dtype=torch.float64, device=dev)
+        g.gsr_vector_to_internal(h, y, yi)
+        internal = []
+        for fn, a, b in ((g.gsr_aprod1_internal, x, yi), (g.gsr_aprod2_internal, yi, x),
+                         (g.gsr_vector_to_internal, y, yi), (g.gsr_vector_from_internal, yi, y)):
+            fn(h, a, b)
+            e0.record()
+            for _ in range(5):
+                fn(h, a, b)
+            e1.record()
+            torch.cuda.synchronize()
+            internal.append(e0.elapsed_time(e1) / 5)
+        del yi
+        pair_internal = (BYTES_APROD1 + BYTES_APROD2) * m / (internal[0] + internal[1]) * 1e-6
         row = {"workload": cfg.name, "rows": m, "cols": cfg.n_cols,
                "row_order": "time-ordered inside a star" if args.time_ordered else "uniform random knots",
                "l2": "L2-assisted" if 224 * m < 1e9 else "HBM",
@@ -337,6 +366,12 @@ def run_sweep(args):
                "aprod1_caller_order_ms": api[0], "aprod2_caller_order_ms": api[1],
                "aprod1_caller_order_gbs": BYTES_APROD1 * m / api[0] * 1e-6,
                "aprod2_caller_order_gbs": BYTES_APROD2 * m / api[1] * 1e-6,
+               "pair_caller_order_frac_of_8tbs": (BYTES_APROD1 + BYTES_APROD2) * m / (api[0] + api[1]) * 1e-6 / 8000.0,
+               "aprod1_internal_api_ms": internal[0], "aprod2_internal_api_ms": internal[1],
+               "aprod1_internal_api_gbs": BYTES_APROD1 * m / internal[0] * 1e-6,
+               "aprod2_internal_api_gbs": BYTES_APROD2 * m / internal[1] * 1e-6,
+               "pair_internal_api_gbs": pair_internal, "pair_internal_api_frac_of_8tbs": pair_internal / 8000.0,
+               "to_internal_ms": internal[2], "from_internal_ms": internal[3],
                "peak": peak, "peak_source": peak_src}
         print(json.dumps(row), flush=True)
         g.gsr_matrix_destroy(h)

@@ -151,6 +151,29 @@ int gsr_aprod1(const gsr_matrix* A, const double* x_dev, double* y_dev, gsr_stre
  * the internal row order; counted by gsr_matrix_device_bytes; GSR_ENOMEM if it does not fit). */
 int gsr_aprod2(const gsr_matrix* A, const double* y_dev, double* x_dev, gsr_stream stream);
 
+/* The same two products on vectors kept in the library's INTERNAL row order.  gsr_aprod1/2 take y
+ * in the caller's row order and pay for it inside the kernel: the rows of a 32-row tile are
+ * scattered over their ingest segment, so every tile gathers (scatters) its 32 entries of y one by
+ * one -- measured at 3e8 rows 4.86 / 4.38 TB/s against 7.18 / 4.82 TB/s in the internal order
+ * (profiles/r2_cfg5_sweep.md).  LSQR only ever touches m-sized vectors through A and A^T, so a
+ * caller that iterates (the solver itself does this) converts ONCE and then runs every product at
+ * the internal-order rate:
+ *     gsr_matrix_internal_rows   length of an internal-order vector: the rows padded to whole
+ *                                tiles per attitude bin, plus the constraint rows (-1 before
+ *                                finalize)
+ *     gsr_vector_to_internal     yint[i] = y[row of internal position i], 0 in padding positions
+ *     gsr_vector_from_internal   the inverse; padding positions are dropped
+ *     gsr_aprod1_internal        yint += A x      (Algorithm 1)
+ *     gsr_aprod2_internal        x += A^T yint    (Algorithm 2)
+ * Padding positions belong to all-zero rows: aprod1 leaves them as they are, aprod2 ignores them.
+ * All pointers are device memory owned by the caller; asynchronous on `stream`; same stream-order
+ * rule as the other products.  aprod2 runs as GSR_OPT_APROD2_SPLIT says. */
+int64_t gsr_matrix_internal_rows(const gsr_matrix* A);
+int gsr_vector_to_internal(const gsr_matrix* A, const double* y_dev, double* yint_dev, gsr_stream stream);
+int gsr_vector_from_internal(const gsr_matrix* A, const double* yint_dev, double* y_dev, gsr_stream stream);
+int gsr_aprod1_internal(const gsr_matrix* A, const double* x_dev, double* yint_dev, gsr_stream stream);
+int gsr_aprod2_internal(const gsr_matrix* A, const double* yint_dev, double* x_dev, gsr_stream stream);
+
 /* ---- preconditioner (row a1; Algorithm 3 line 2) ---------------------- */
 
 /* p_j = 1/||A_j||_2 (1 for an empty column); every stored coefficient is multiplied by

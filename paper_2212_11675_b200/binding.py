@@ -26,7 +26,8 @@ EXPORTS = [
     "gsr_debug_expand_rows", "gsr_time_product", "gsr_launch_count", "gsr_lsqr_standard_errors", "gsr_lsqr_last_loop_ms", "gsr_lsqr_set_damp",
     "gsr_debug_fused_pass", "gsr_debug_graph_builds", "gsr_debug_while_graph", "gsr_matrix_set_constraints", "gsr_comm_unique_id", "gsr_comm_create", "gsr_comm_destroy", "gsr_matrix_set_comm",
     "gsr_matrix_begin_streamed", "gsr_matrix_host_bytes", "gsr_matrix_streamed_bytes",
-    "gsr_norm2_static",
+    "gsr_norm2_static", "gsr_matrix_internal_rows", "gsr_vector_to_internal", "gsr_vector_from_internal",
+    "gsr_aprod1_internal", "gsr_aprod2_internal",
 ]
 GSR_NORM2_STATIC_MAX_LEN = 1 << 29
 
@@ -117,6 +118,11 @@ def lib():
         L.gsr_debug_while_graph.argtypes = [vp]
         L.gsr_debug_while_graph.restype = C.c_int
         L.gsr_norm2_static.argtypes = [vp, i64, vp, vp]
+        L.gsr_matrix_internal_rows.argtypes = [vp]
+        L.gsr_matrix_internal_rows.restype = i64
+        for name in ("gsr_vector_to_internal", "gsr_vector_from_internal", "gsr_aprod1_internal",
+                     "gsr_aprod2_internal"):
+            getattr(L, name).argtypes = [vp, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -221,6 +227,27 @@ def gsr_aprod1(h, x_dev, y_dev, stream=None):
 
 def gsr_aprod2(h, y_dev, x_dev, stream=None):
     _check(lib().gsr_aprod2(h, _ptr(y_dev), _ptr(x_dev), _stream(stream)), "gsr_aprod2")
+
+
+def gsr_matrix_internal_rows(h) -> int:
+    return int(lib().gsr_matrix_internal_rows(h))
+
+
+def gsr_vector_to_internal(h, y_dev, yint_dev, stream=None):
+    _check(lib().gsr_vector_to_internal(h, _ptr(y_dev), _ptr(yint_dev), _stream(stream)), "gsr_vector_to_internal")
+
+
+def gsr_vector_from_internal(h, yint_dev, y_dev, stream=None):
+    _check(lib().gsr_vector_from_internal(h, _ptr(yint_dev), _ptr(y_dev), _stream(stream)),
+           "gsr_vector_from_internal")
+
+
+def gsr_aprod1_internal(h, x_dev, yint_dev, stream=None):
+    _check(lib().gsr_aprod1_internal(h, _ptr(x_dev), _ptr(yint_dev), _stream(stream)), "gsr_aprod1_internal")
+
+
+def gsr_aprod2_internal(h, yint_dev, x_dev, stream=None):
+    _check(lib().gsr_aprod2_internal(h, _ptr(yint_dev), _ptr(x_dev), _stream(stream)), "gsr_aprod2_internal")
 
 
 def gsr_precondition(h, p_out=None, stream=None):

@@ -1015,11 +1015,77 @@ int launch_colsumsq(const gsr_matrix* A, double* q, cudaStream_t s) {
     return pass(A, s, [&](const TileView& v) { return aprod2_view(A, v, nullptr, q, nullptr, nullptr, nullptr, true, nullptr, s); });
 }
 
+// caller row order <-> internal row order of an m-sized vector (gsr_vector_to_internal /
+// gsr_vector_from_internal): streaming passes over perm; rows move only inside their ingest
+// segment (2^22 rows = 32 MB of doubles), so the scattered side stays in L2
+__global__ void __launch_bounds__(256) k_rows_to_internal(const double* __restrict__ src,
+                                                          const uint32_t* __restrict__ perm,
+                                                          double* __restrict__ dst, int64_t len_int) {
+    for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < len_int; i += (int64_t)gridDim.x * 256) {
+        const uint32_t pe = perm[i];
+        dst[i] = pe != PERM_PAD ? src[pe] : 0.0;     // padding rows of a tile hold zero
+    }
+}
+__global__ void __launch_bounds__(256) k_rows_from_internal(const double* __restrict__ src,
+                                                            const uint32_t* __restrict__ perm,
+                                                            double* __restrict__ dst, int64_t len_int) {
+    for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < len_int; i += (int64_t)gridDim.x * 256) {
+        const uint32_t pe = perm[i];
+        if (pe != PERM_PAD) dst[pe] = src[i];
+    }
+}
+
 }  // namespace gsr
 
 using namespace gsr;
 
 extern "C" {
+
+int64_t gsr_matrix_internal_rows(const gsr_matrix* A) { return (A && A->state == 1) ? A->m_int + A->n_con : -1; }
+
+int gsr_vector_to_internal(const gsr_matrix* A, const double* y_dev, double* yint_dev, gsr_stream stream) {
+    if (!A || ((!y_dev || !yint_dev) && A->dims.n_rows + A->n_con > 0)) return GSR_EINVAL;
+    if (A->state != 1) return GSR_ESTATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (A->m_int > 0) {
+        k_rows_to_internal<<<A->sm_count * 8, 256, 0, s>>>(y_dev, A->perm, yint_dev, A->m_int);
+        count_launch();
+        GSR_CUDA_TRY(cudaGetLastError());
+    }
+    if (A->n_con > 0)   // constraint rows keep their order, after the observations
+        GSR_CUDA_TRY(cudaMemcpyAsync(yint_dev + A->m_int, y_dev + A->dims.n_rows, (size_t)A->n_con * 8,
+                                     cudaMemcpyDeviceToDevice, s));
+    return GSR_OK;
+}
+
+int gsr_vector_from_internal(const gsr_matrix* A, const double* yint_dev, double* y_dev, gsr_stream stream) {
+    if (!A || ((!y_dev || !yint_dev) && A->dims.n_rows + A->n_con > 0)) return GSR_EINVAL;
+    if (A->state != 1) return GSR_ESTATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (A->m_int > 0) {
+        k_rows_from_internal<<<A->sm_count * 8, 256, 0, s>>>(yint_dev, A->perm, y_dev, A->m_int);
+        count_launch();
+        GSR_CUDA_TRY(cudaGetLastError());
+    }
+    if (A->n_con > 0)
+        GSR_CUDA_TRY(cudaMemcpyAsync(y_dev + A->dims.n_rows, yint_dev + A->m_int, (size_t)A->n_con * 8,
+                                     cudaMemcpyDeviceToDevice, s));
+    return GSR_OK;
+}
+
+int gsr_aprod1_internal(const gsr_matrix* A, const double* x_dev, double* yint_dev, gsr_stream stream) {
+    if (!A || !x_dev || (!yint_dev && A->m_int + A->n_con > 0)) return GSR_EINVAL;
+    if (A->state != 1) return GSR_ESTATE;
+    GSR_TRY(launch_aprod1(A, x_dev, yint_dev, A->coef_one, nullptr, nullptr, nullptr, (cudaStream_t)stream));
+    return launch_con_aprod1(A, x_dev, yint_dev + A->m_int, A->coef_one, nullptr, nullptr, (cudaStream_t)stream);
+}
+
+int gsr_aprod2_internal(const gsr_matrix* A, const double* yint_dev, double* x_dev, gsr_stream stream) {
+    if (!A || !x_dev || (!yint_dev && A->m_int + A->n_con > 0)) return GSR_EINVAL;
+    if (A->state != 1) return GSR_ESTATE;
+    GSR_TRY(launch_aprod2(A, yint_dev, x_dev, A->coef_one, nullptr, nullptr, (cudaStream_t)stream));
+    return launch_con_aprod2(A, yint_dev + A->m_int, x_dev, A->coef_one, nullptr, (cudaStream_t)stream);
+}
 
 int gsr_aprod1(const gsr_matrix* A, const double* x_dev, double* y_dev, gsr_stream stream) {
     if (!A || !x_dev || (!y_dev && A->dims.n_rows > 0)) return GSR_EINVAL;

@@ -124,7 +124,9 @@ struct TileView {
 // pass over the matrix handles the resident run of units with one launch and the rest in
 // CHUNKS (runs of whole units, at most chunk_cap tiles) that a copy stream brings into one of
 // two device buffers while the other is being consumed: H2D copy of chunk c+1 || kernels of
-// chunk c.  All ordering is by events, the host never waits inside a pass.
+// chunk c.  All ordering is by events, the host never waits inside a pass; in fixed-count mode
+// the solver enqueues several iterations per poll of the stop flag, so that the copy stream does
+// not idle across the n-sized tail kernels and the host round trip between iterations either.
 struct Chunk {
     int u0, u1;
     int64_t t0, t1;
@@ -143,6 +145,10 @@ struct StreamStore {
     int res_units = 0;                   // units [0, res_units) lie wholly below res_cap
     std::vector<Chunk>* chunks = nullptr;
     int64_t h2d_bytes = 0;               // bytes copied host -> device so far (bench.py)
+    bool need_fork = true;               // the next pass must order its copies after the work queued on
+                                         // the compute stream: set by ingest and by every pass that
+                                         // wrote tiles back; read-only passes leave it false, so the
+                                         // first copies of a pass overlap the tail of the previous one
 };
 
 // Device-resident LSQR scalars (row a9): every kernel of the iteration reads its coefficients

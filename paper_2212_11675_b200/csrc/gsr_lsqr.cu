@@ -705,7 +705,11 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
     GSR_CUDA_TRY(cudaEventRecord(W.ev0, s));   // device time of the iterations alone (bench.py)
     // (fixed-count mode never stops early; with a communicator every launch that follows the stop
     // still runs its two all-reduces, so the stop flag is polled more often there)
-    const int64_t batch = !use_graph ? 1 : A->opt_force_itnlim ? 256 : A->comm ? 8 : 32;
+    // Streamed handles: nothing in an iteration needs a host value (every kernel checks the stop
+    // flag), so fixed-count mode enqueues 8 iterations per poll and the copy stream never waits for
+    // the host; in standard mode a launch that follows the stop would still move the whole host
+    // part over the bus, so the flag is polled after every iteration there.
+    const int64_t batch = !use_graph ? (A->opt_force_itnlim ? 8 : 1) : A->opt_force_itnlim ? 256 : A->comm ? 8 : 32;
     int64_t launched = 0;
     W.last_loop_while = use_graph && W.wgraph != nullptr && A->opt_while;
     if (W.last_loop_while) {
@@ -719,8 +723,10 @@ int gsr_lsqr_solve(gsr_matrix* A, const double* b_hd, double* x_hd, int64_t itnl
             for (int64_t i = 0; i < nb; ++i) GSR_CUDA_TRY(cudaGraphLaunch(W.graph, s));
             count_launch(nb * kernels_per_iteration(A));
         } else {
-            GSR_TRY(enqueue_iteration(A, s));   // (its launchers count their own launches)
-            count_launch(5);
+            for (int64_t i = 0; i < nb; ++i) {
+                GSR_TRY(enqueue_iteration(A, s));   // (its launchers count their own launches)
+                count_launch(5);
+            }
         }
         launched += nb;
         GSR_CUDA_TRY(cudaMemcpyAsync(W.stop_host, &W.st->stop, sizeof(int), cudaMemcpyDeviceToHost, s));

@@ -344,10 +344,15 @@ int for_each_view(gsr_matrix* A, cudaStream_t s, const std::function<int(const T
     StreamStore& so = A->so;
     const std::vector<Chunk>& chunks = *so.chunks;
     const size_t nc = chunks.size();
-    // the copy stream starts after whatever the caller has queued on s so far (a write-back of an
-    // earlier pass included), then runs ahead of the kernels by up to two chunks
-    GSR_CUDA_TRY(cudaEventRecord(so.fork, s));
-    GSR_CUDA_TRY(cudaStreamWaitEvent(so.copy, so.fork, 0));
+    // After ingest or a write-back pass the copy stream starts after whatever has been queued on s
+    // so far (the tiles it reads were written there).  After a read-only pass nothing it reads can
+    // change: the copies only wait for their buffer (done[b]) and run ahead of the kernels by up to
+    // two chunks -- across the end of the previous pass too.
+    if (so.need_fork) {
+        GSR_CUDA_TRY(cudaEventRecord(so.fork, s));
+        GSR_CUDA_TRY(cudaStreamWaitEvent(so.copy, so.fork, 0));
+        so.need_fork = false;
+    }
     for (size_t c = 0; c < nc && c < 2; ++c) GSR_TRY(issue_chunk_copy(A, c));
     if (so.res_units > 0) {
         const Unit& last = (*A->units_host)[so.res_units - 1];
@@ -373,6 +378,7 @@ int for_each_view(gsr_matrix* A, cudaStream_t s, const std::function<int(const T
         GSR_CUDA_TRY(cudaEventRecord(so.done[b], s));
         if (c + 2 < nc) GSR_TRY(issue_chunk_copy(A, c + 2));
     }
+    if (writeback) so.need_fork = true;
     return GSR_OK;
 }
 
