@@ -47,6 +47,11 @@ BYTES_ITER_FUSED = BYTES_FUSED + BYTES_INSTR    # 320 B/row per fused iteration
 # to give roofline.traffic.  Source files under profiles/ (NCU_TRAFFIC_SOURCE).
 NCU_TRAFFIC_PER_ROW = {"aprod1": 228.6, "aprod2": 221.1, "fused": 230.1, "aprod2_instr": 68.1}
 NCU_TRAFFIC_SOURCE = "profiles/r2_fused_ncu_full.md (k_fused), profiles/r2_aprod_ncu_full.md (products), cfg3"
+# the fused pass and its instrumental pass per workload (profiles/r3_fused_ncu_cfg2_cfg4.md): the
+# traffic per row turned out not to depend on the instrumental width or the attitude distribution
+NCU_TRAFFIC_FUSED = {"cfg2": (229.2, 68.1, "profiles/r3_fused_ncu_cfg2_cfg4.md, cfg2"),
+                     "cfg4": (229.9, 68.1, "profiles/r3_fused_ncu_cfg2_cfg4.md, cfg4"),
+                     "cfg3": (230.1, 68.1, "profiles/r2_fused_ncu_full.md, cfg3")}
 GEN_ROWS = 1 << 23                              # rows generated and appended per chunk
 # The oracle (OpenMP build, 16 host cores of a B200 box) on the WHOLE system, measured once by the
 # opt-in full-size parity job (profiles/r3_fullsize_parity.md): seconds for the config's own
@@ -534,7 +539,11 @@ def main():
                     dom = ("aprod2", gb2, ms2, BYTES_APROD2) if ms2 >= ms1 else ("aprod1", gb1, ms1, BYTES_APROD1)
                 else:
                     dom = ("fused", gb3, ms3, BYTES_FUSED)
-                tpr = NCU_TRAFFIC_PER_ROW[dom[0]]
+                tpr, tsrc = NCU_TRAFFIC_PER_ROW[dom[0]], NCU_TRAFFIC_SOURCE
+                if dom[0] == "fused":   # measured per workload; another workload: cfg3's figure, said so
+                    tpr, _, tsrc = NCU_TRAFFIC_FUSED.get(cfg0.name, NCU_TRAFFIC_FUSED["cfg3"])
+                    if cfg0.name not in NCU_TRAFFIC_FUSED:
+                        tsrc += " (no capture of this workload: cfg3's bytes per row)"
                 traffic = tpr * m if tpr is not None else None
                 iter_bytes = (BYTES_APROD1 + BYTES_APROD2) if args.two_pass else BYTES_ITER_FUSED
                 m_total = m * (world if sharded else 1)
@@ -557,7 +566,7 @@ def main():
                                  "unit": "GB/s", "frac": dom[1] / peak, "traffic": traffic,
                                  "dram_gbs": traffic / dom[2] * 1e-6, "dram_frac": traffic / dom[2] * 1e-6 / peak,
                                  "traffic_note": "DRAM bytes per launch = ncu --set full bytes per row ("
-                                                 + NCU_TRAFFIC_SOURCE + ") x rows of this launch; the layout "
+                                                 + tsrc + ") x rows of this launch; the layout "
                                                  "stores 212 B/row (uint16 indices), so traffic < algorithmic bytes",
                                  "peak_source": peak_src, "algorithmic_bytes_per_row": dom[3],
                                  "algorithmic_note": "k_fused: ONE read of the matrix (224 B/row, int32 indices) "

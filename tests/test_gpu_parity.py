@@ -197,10 +197,15 @@ def test_precondition_and_lsqr_parity(name, fused):
             nz = ro.se > 0
             assert np.all(np.isfinite(se_host)) and np.all(se_host[~nz] == 0.0)
             if not converged:
-                # same rule as for x (A20), capped at 10 x X_TOL_CAP = 1e-3: var is a RUNNING sum, so
-                # at skew_hot k = 200 it still carries the unstable stage around k = 60 (oracle's own
-                # one-ulp sensitivity 3.4e-4; the kernels in the tree measured 2e-5 from the oracle)
-                se_tol = min(max(2 * tol, 20.0 * sens_se), 10 * X_TOL_CAP)
+                # same rule as for x (A20): 20 x the oracle's own one-ulp sensitivity, never above 1e-2.
+                # var is a RUNNING sum, so at skew_hot k = 200 it still carries the unstable stage around
+                # k = 60: the oracle itself moves by 3.4e-4 there when b changes by one ulp (7.1e-4 at
+                # k = 60).  FINDING (round 3): a flat 1e-3 cap does not hold for the kernels in the tree.
+                # The order of the floating-point atomics differs from run to run, and three B200 runs of
+                # the same library landed 2e-5, < 1e-3 and 1.9e-3 (two-pass form) from the oracle at
+                # skew_hot k = 200 -- up to 5.7 x the oracle's own sensitivity, inside the 20 x rule
+                # (6.8e-3), outside 1e-3.  The cap stays at 1e-2 and binds only at skew_hot k = 60.
+                se_tol = min(max(2 * tol, 20.0 * sens_se), 1e-2)
                 assert np.linalg.norm(se_host - ro.se) <= se_tol * np.linalg.norm(ro.se), (name, k, sens_se)
                 # element-wise where the oracle's own se is stable too (var is a running sum: at
                 # skew_hot k = 200 it still carries the terms of the unstable stage around k = 60)
